@@ -1,0 +1,310 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the GPUMCD hot path on B200 (one JSON line on stdout).
+
+    python bench.py --gpus N --steps K --warmup W            # the CUDA library (this repo)
+    python bench.py --impl reference --steps K --warmup W    # the CPU oracle, timed as it stands
+
+A "step" is one gpumcd_run of the whole hot path (source, photon and electron transport with all
+secondaries, tally, finalize) over one batch of synthetic histories.  Workload at N = 1: config 2 of
+BASELINE.json (15 MeV electrons, 10x10 cm^2 field, 1e6 histories, 128^3 water at 0.25 cm), the
+configuration the metric is quoted on.  --config selects another one.
+
+Metric: coupled photon-electron histories/s (value) and condensed-history steps/s (ch_steps_per_s).
+Multi-GPU (--gpus N under torchrun): every rank simulates its own disjoint history range (weak
+scaling) and the dose grids are summed with one all-reduce per step.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+# thread-instructions one condensed-history step needs at minimum, and the
+# issue peak = 148 SMs x 4 schedulers x 32 lanes x 1 inst/clk x max SM clock.
+ALG_INST_PER_CH_STEP = 330.0
+N_SM, N_SCHED, LANES = 148, 4, 32
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return d, "measured"
+    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback"
+
+
+class ClockSampler:
+    """Samples nvidia-smi clocks / throttle reasons every 200 ms while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if self.proc:
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=2)
+            except subprocess.TimeoutExpired:
+                self.proc.kill()
+        sm, smax, reasons = [], [], set()
+        for r in self.rows:
+            try:
+                sm.append(float(r[0]))
+                smax.append(float(r[1]))
+            except (ValueError, IndexError):
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(smax) if smax else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def oracle_rate(w, seconds: float, threads: int = 0):
+    """Time the oracle, as it stands, on a bounded sample of workload ``w`` sized for ~``seconds``."""
+    import oracle
+    probe = max(2000, min(20000, w.n_histories))
+    t0 = time.perf_counter()
+    r = oracle.run_workload(w, probe, n_threads=threads)
+    dt = time.perf_counter() - t0
+    n = int(min(w.n_histories, max(probe, probe * seconds / max(dt, 1e-3))))
+    t0 = time.perf_counter()
+    r = oracle.run_workload(w, n, n_threads=threads)
+    dt = time.perf_counter() - t0
+    return n, dt, r.counters
+
+
+def reference_arm(args):
+    """The base contract's reference arm for this tier: the CPU oracle on the box's host cores."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    import oracle
+    from paper_1101_1245_b200.inputs import make_config
+    w = make_config(args.config)
+    cores = os.cpu_count() or 1
+    n = args.ref_histories
+    for _ in range(args.warmup):
+        oracle.run_workload(w, max(n // 10, 1000))
+    t0 = time.perf_counter()
+    steps_ch = 0
+    for k in range(args.steps):
+        r = oracle.run(w.density, w.material, w.voxel_cm, w.tables, w.source, n, seed=w.seed + k)
+        steps_ch += r.counters["ch_steps"]
+    dt = time.perf_counter() - t0
+    value = args.steps * n / dt
+    line = {
+        "impl": "reference", "metric": "coupled photon-electron histories/s", "value": value, "unit": "histories/s",
+        "ch_steps_per_s": steps_ch / dt, "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": w.name, "histories_per_step": n, "note": "bounded sample of the workload per step"},
+        "cpu_baseline": {"value": value, "unit": "histories/s", "cores": cores, "kind": "oracle",
+                         "sample": f"{n} histories of {w.name} per step, {args.steps} steps"},
+        "e2e": {"value": value, "unit": "histories/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=2)
+    ap.add_argument("--histories", type=int, default=0, help="override histories per step (0 = the config's)")
+    ap.add_argument("--scheduler", type=int, default=-1)
+    ap.add_argument("--ref-histories", type=int, default=50_000)
+    ap.add_argument("--cpu-seconds", type=float, default=15.0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.impl == "reference":
+        return reference_arm(args)
+
+    import torch
+
+    import paper_1101_1245_b200 as g
+    from paper_1101_1245_b200 import build as cuda_build
+    from paper_1101_1245_b200.inputs import make_config
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the hot path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+    if rank == 0:
+        cuda_build.build()
+    if dist:
+        dist.barrier()
+    g.load_library()
+
+    w = make_config(args.config)
+    n = args.histories or w.n_histories
+    rho = torch.from_numpy(w.density).to(dev)
+    mat = torch.from_numpy(w.material).to(dev)
+    dose = torch.empty(rho.shape, dtype=torch.float32, device=dev)
+    opts = {}
+    if args.scheduler >= 0:
+        opts["scheduler"] = args.scheduler
+    opt = g.gpumcd_default_options(**opts)
+    ctx = g.gpumcd_create(rho, mat, w.voxel_cm, w.tables, opt)
+    g.gpumcd_set_source(ctx, w.source)
+    g.gpumcd_set_history_offset(ctx, rank * n)       # disjoint history ranges per rank
+    g.gpumcd_set_profiling(ctx, True)
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev)   # > 126 MB L2
+
+    def step(seed):
+        g.gpumcd_run(ctx, n, seed, dose)
+        if dist:
+            dist.all_reduce(dose)                     # "the resulting dose arrays are summed" (L188)
+
+    for k in range(args.warmup):
+        step(w.seed + k)
+    torch.cuda.synchronize()
+
+    sampler = ClockSampler(local)
+    sampler.start()
+    if dist:
+        dist.barrier()
+    torch.cuda.synchronize()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    ch_steps = flights = launches = 0
+    ms_e = ms_p = 0.0
+    n_e = n_p = 0
+    wall0 = time.perf_counter()
+    for k in range(args.steps):
+        flush.fill_(k & 0xFF)                          # evict the phantom / tally / tables from L2
+        torch.cuda.synchronize()
+        ev[k][0].record()
+        step(w.seed + 100 + k)
+        ev[k][1].record()
+        torch.cuda.synchronize()
+        c = g.gpumcd_get_counters(ctx)
+        p = g.gpumcd_get_profile(ctx)
+        ch_steps += c["ch_steps"]
+        flights += c["photon_flights"]
+        launches += p["launches"]
+        ms_e += p["ms_electron"]; ms_p += p["ms_photon"]
+        n_e += p["n_electron"]; n_p += p["n_photon"]
+    if dist:
+        dist.barrier()
+    torch.cuda.synchronize()
+    wall = time.perf_counter() - wall0
+    clocks = sampler.stop()
+    t_ms = sum(a.elapsed_time(b) for a, b in ev)
+    if dist:
+        tt = torch.tensor([t_ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        t_ms = float(tt.item())
+        agg = torch.tensor([ch_steps, flights], dtype=torch.float64, device=dev)
+        dist.all_reduce(agg)
+        ch_steps, flights = (float(x) for x in agg.tolist())
+    t_s = t_ms * 1e-3
+    value = world * args.steps * n / t_s
+
+    # ---- roofline of the dominant kernel (electron transport): issue-rate bound
+    peaks, peak_kind = measured_peaks()
+    peak_inst = N_SM * N_SCHED * LANES * peaks.get("sm_max_mhz", 1965.0) * 1e6
+    local_ch = ch_steps / world
+    achieved = ALG_INST_PER_CH_STEP * local_ch / (ms_e * 1e-3) if ms_e > 0 else None
+    roofline = {"bound": "alu", "kernel": "electron transport", "achieved": achieved, "peak": peak_inst,
+                "unit": "thread-inst/s", "frac": (achieved / peak_inst) if achieved else None, "traffic": None,
+                "peak_source": f"148 SMs x 4 x 32 x sm_max_mhz ({peak_kind})",
+                "kernel_ms_per_step": ms_e / args.steps, "kernel_launches_per_step": n_e / args.steps,
+                "kernel_share_of_step": ms_e / t_ms if t_ms else None,
+                "alg_inst_per_ch_step": ALG_INST_PER_CH_STEP}
+
+    # ---- end to end through the host entry points (volumes and dose in host memory)
+    e2e = None
+    if not args.no_e2e:
+        rho_h = torch.from_numpy(w.density).pin_memory()
+        mat_h = torch.from_numpy(w.material).pin_memory()
+        dose_h = torch.empty(rho.shape, dtype=torch.float32).pin_memory()
+        reps, tot = 0, 0.0
+        for k in range(1 + min(args.steps, 3)):
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            with g.gpumcd_create_host(rho_h.numpy(), mat_h.numpy(), w.voxel_cm, w.tables, opt) as c2:
+                g.gpumcd_set_source(c2, w.source)
+                g.gpumcd_set_history_offset(c2, rank * n)
+                g.gpumcd_run_host(c2, n, w.seed + 200 + k, dose_h.numpy())
+            torch.cuda.synchronize()
+            if k > 0:
+                tot += time.perf_counter() - t0
+                reps += 1
+        e2e_t = tot / reps
+        if dist:
+            tt = torch.tensor([e2e_t], dtype=torch.float64, device=dev)
+            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+            e2e_t = float(tt.item())
+        tab_bytes = 4 * (w.tables.photon.size + w.tables.electron.size + w.tables.ms_a.size)
+        e2e = {"value": world * n / e2e_t, "unit": "histories/s", "h2d_bytes_per_step": int(rho.numel() * 5 + tab_bytes),
+               "d2h_bytes_per_step": int(rho.numel() * 4), "ms_per_step": e2e_t * 1e3,
+               "what": "gpumcd_create_host + set_source + run_host + destroy, wall clock"}
+
+    g.gpumcd_destroy(ctx)
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        ns, dt, oc = oracle_rate(w, args.cpu_seconds)
+        cpu = {"value": ns / dt, "unit": "histories/s", "cores": os.cpu_count(), "kind": "oracle",
+               "ch_steps_per_s": oc["ch_steps"] / dt,
+               "sample": f"first {ns} histories of {w.name}, OpenMP over all host cores, {dt:.1f} s"}
+
+    if rank == 0:
+        line = {
+            "metric": "coupled photon-electron histories/s", "value": value, "unit": "histories/s",
+            "ch_steps_per_s": ch_steps / t_s, "photon_flights_per_s": flights / t_s,
+            "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": t_ms / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": w.name, "histories_per_step_per_gpu": n, "scheduler": int(opt.scheduler),
+                       "wave_size": int(opt.wave_size), "l2": "flushed between timed steps (512 MiB write)",
+                       "tally": "fp64 atomics", "parallelism": f"histories x{world}"},
+            "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu,
+            "wall_s_timed_region": wall,
+        }
+        print(json.dumps(line))
+    if dist:
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

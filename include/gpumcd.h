@@ -1,0 +1,180 @@
+/*
+ * gpumcd.h -- C ABI of the B200-native GPUMCD hot path.
+ *
+ * Coupled photon-electron Monte Carlo transport through a voxelised phantom with energy
+ * deposited into a 3-D dose grid (arxiv 1101.1245; Sec. II.A photons, II.B electrons,
+ * II.C GPU implementation).  The calls follow the paper's statement of the problem:
+ *   inputs  - a density volume and a composition-id volume,
+ *             cross-section / stopping-power tables (L170), a source (L166),
+ *             cutoffs P_cut (L45) and E_c (L79), the step bound e_s-max (L108);
+ *   output  - the dose array (L188).
+ *
+ * Conventions
+ *   - Every call returns a gpumcd_status; nothing throws or aborts across this boundary.
+ *   - Pointers named *_dev are CUDA device pointers on the current device; *_host are host
+ *     pointers.  The library copies what it needs at create time: the caller keeps ownership of
+ *     everything it passes in and may free it as soon as the call returns.
+ *   - Volumes are C arrays [nz][ny][nx]; voxel (ix,iy,iz) has index ix + nx*(iy + ny*iz) and
+ *     spans [ix*h,(ix+1)*h) x ...; the beam enters the z = 0 face travelling along +z.
+ *     nx, ny, nz <= 1024.
+ *   - Units: MeV (kinetic for electrons), cm, g/cm^3.  Dose is MeV/g per primary history
+ *     (x 1.602e-10 = Gy per history).
+ *   - History ids are 0 .. n_histories-1.  A particle's random stream is Philox4x32-10 with
+ *     counter (hist_lo, hist_hi, track, ctr) and key (seed_lo, seed_hi) (DESIGN.md "Random
+ *     numbers"), so the same (seed, n_histories) gives the same result up to the order of the
+ *     fp64 additions into the tally.
+ */
+#ifndef GPUMCD_H
+#define GPUMCD_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct gpumcd_ctx gpumcd_ctx; /* opaque, owned by the library */
+
+typedef enum {
+    GPUMCD_OK = 0,
+    GPUMCD_ERR_INVALID_ARG = -1,   /* null pointer, bad size, material id out of range, density <= 0 */
+    GPUMCD_ERR_CUDA = -2,          /* a CUDA runtime call failed; see gpumcd_last_error */
+    GPUMCD_ERR_OOM = -3,           /* device allocation failed */
+    GPUMCD_ERR_BANK_OVERFLOW = -4, /* a particle queue filled up; the run's result is invalid
+                                      (the paper silently discards secondaries here, L166) */
+    GPUMCD_ERR_NO_SOURCE = -5,     /* gpumcd_run before gpumcd_set_source */
+    GPUMCD_ERR_TABLE_RANGE = -6    /* a source energy lies outside [e_min, e_max] of the tables */
+} gpumcd_status;
+
+/* Material tables, HOST arrays, copied at create.  All columns are mass
+ * coefficients on a grid uniform in ln E between e_min and e_max (n_energy nodes), looked up by
+ * linear interpolation in ln E and multiplied by the voxel density (Eq. 2).
+ *   photon  [n_materials][3][n_energy] : Compton, photoelectric, pair              cm^2/g
+ *   electron[n_materials][4][n_energy] : restricted stopping power L (Eq. 6)   MeV cm^2/g,
+ *                                        hard Moller, hard bremsstrahlung,
+ *                                        inverse first transport mean free path    cm^2/g
+ *   ms_a    [n_K] : multiple-scattering shape parameter a(K) on a uniform ln K grid
+ * e_cut is the electron kinetic cutoff E_c = K_cut the tables were built with; p_cut is the
+ * photon cutoff P_cut = k_c of the bremsstrahlung tables. */
+typedef struct {
+    int32_t n_materials; /* 1..8 */
+    int32_t n_energy;    /* >= 2 */
+    float e_min, e_max;  /* MeV */
+    const float *photon;
+    const float *electron;
+    int32_t n_K;
+    float lnK_min, lnK_max;
+    const float *ms_a;
+    float e_cut;
+    float p_cut;
+} gpumcd_tables;
+
+typedef struct {
+    float es_max_cm;       /* e_s-max of Eq. 4 (L108); default 0.5                                 */
+    float f_eloss_max;     /* largest fraction of its energy an electron may lose in one step; 0.25 */
+    float boundary_nudge;  /* fraction of the voxel size added to d_vox of Eq. 4; 1e-4             */
+    int32_t pair_mode;     /* 1 (default): the 2 m_e c^2 of a pair event leaves as two 0.511 MeV
+                              photons; 0: it is deposited at the vertex (L74 is silent)            */
+    int32_t photon_only;   /* 1: every electron is deposited where it is born; default 0           */
+    float majorant_scale;  /* >= 1, inflates the Woodcock majorants (Eq. 3; test hook); default 1  */
+    uint32_t wave_size;    /* primaries generated per wave; default 2^20                           */
+    uint32_t bank_factor;  /* queue capacity = bank_factor * wave_size records (the paper's d, L166);
+                              default 8                                                            */
+    int32_t scheduler;     /* 0: one launch per pass, host reads the queue counts (L166);
+                              1: persistent cooperative kernel, no host round trips               */
+    int32_t reserved;
+} gpumcd_options;
+
+typedef struct {
+    int32_t particle;    /* 0 photon, 1 electron */
+    int32_t shape;       /* 0 pencil beam, 1 parallel rectangular field */
+    float cx, cy;        /* field centre on the z = 0 face, cm */
+    float wx, wy;        /* full field widths, cm (ignored for a pencil beam) */
+    float energy;        /* MeV, used when n_spec == 0 */
+    int32_t n_spec;      /* number of spectrum bins, 0 = monoenergetic */
+    const float *spec_E; /* HOST, n_spec+1 bin edges, MeV, increasing */
+    const float *spec_w; /* HOST, n_spec non-negative bin weights; energy is uniform inside a bin */
+} gpumcd_source;
+
+typedef struct {
+    uint64_t n_histories;
+    uint64_t photon_flights, photon_compton, photon_photo, photon_pair, photon_fict;
+    uint64_t ch_steps, hard_moller, hard_brems, hard_fict;
+    uint64_t pushes_e, pushes_g;
+    uint64_t bank_high_water; /* largest queue occupancy seen, records */
+    uint64_t overflow_count;  /* records dropped because a queue was full; must be 0 */
+    double e_incident, e_dep_continuous, e_dep_cutoff, e_escaped, e_pair_rest; /* MeV */
+} gpumcd_counters;
+
+/* Fill *opt with the defaults listed above. */
+int gpumcd_default_options(gpumcd_options *opt);
+
+/* Build a context for one phantom: copies the volumes and tables to
+ * library-owned device memory, finds the largest density of every material, builds the Woodcock
+ * majorants mu_max(E) (Eq. 3) and M_e(E) (L110-113) and allocates the particle queues and the
+ * fp64 energy tally.  opt == NULL selects the defaults.  Synchronous.
+ * gpumcd_create takes DEVICE volumes, gpumcd_create_host takes HOST volumes (the copy to the
+ * device is part of the call; this is the entry bench.py's end-to-end figure times). */
+int gpumcd_create(gpumcd_ctx **out, const float *density_dev, const uint8_t *material_dev, int nx,
+                  int ny, int nz, float voxel_cm, const gpumcd_tables *tables,
+                  const gpumcd_options *opt);
+int gpumcd_create_host(gpumcd_ctx **out, const float *density_host, const uint8_t *material_host,
+                       int nx, int ny, int nz, float voxel_cm, const gpumcd_tables *tables,
+                       const gpumcd_options *opt);
+
+/* Select the source (PAPER.md L166 initParticle): particle type, energy or spectrum, geometry. */
+int gpumcd_set_source(gpumcd_ctx *ctx, const gpumcd_source *src);
+
+/* Simulate n_histories primaries and all their secondaries (Sec. II.A-II.C) and write
+ * the dose grid.  dose_out_dev: caller-owned float[nx*ny*nz] on the device, OVERWRITTEN.
+ * cuda_stream: a cudaStream_t (NULL = default stream); all work is enqueued on it.  With
+ * scheduler 1 the call returns without waiting for the device; with scheduler 0 it waits between
+ * passes.  Errors detected on the device (queue overflow) are reported by gpumcd_get_counters. */
+int gpumcd_run(gpumcd_ctx *ctx, uint64_t n_histories, uint64_t seed, float *dose_out_dev,
+               void *cuda_stream);
+
+/* Same, with the dose copied into HOST memory; returns after the copy has completed. */
+int gpumcd_run_host(gpumcd_ctx *ctx, uint64_t n_histories, uint64_t seed, float *dose_out_host,
+                    void *cuda_stream);
+
+/* Photon-only replay run: like gpumcd_run with photon_only = 1 but the output is, per history,
+ * the ordered event codes of the primary track, 3 bits each, first event in the low bits, at most
+ * 21 events: 1 Compton, 2 photoelectric, 3 pair, 4 escaped, 5 absorbed below P_cut.
+ * trace_out_dev: caller-owned uint64[n_histories] on the device, OVERWRITTEN. */
+int gpumcd_run_trace(gpumcd_ctx *ctx, uint64_t n_histories, uint64_t seed, uint64_t *trace_out_dev,
+                     void *cuda_stream);
+
+/* Counters and energy accounts of the last run.  Waits for that run's stream.  Returns
+ * GPUMCD_ERR_BANK_OVERFLOW if the run dropped a particle. */
+int gpumcd_get_counters(gpumcd_ctx *ctx, gpumcd_counters *host_out);
+
+/* Copy the fp64 energy tally of the last run (MeV per voxel) to a caller-owned
+ * double[nx*ny*nz] on the device, on the stream of that run. */
+int gpumcd_get_energy_tally(gpumcd_ctx *ctx, double *edep_out_dev);
+
+/* Shift the history ids of the following runs: they simulate histories first_history ..
+ * first_history + n_histories - 1 (disjoint ranges on different GPUs give independent samples of
+ * the same stream family).  Default 0.  Trace output is indexed from first_history. */
+int gpumcd_set_history_offset(gpumcd_ctx *ctx, uint64_t first_history);
+
+/* Per-kernel device times of the last run, measured with CUDA events on the run's stream, and the
+ * number of kernels the run launched.  Recording is off by default (it adds events around every
+ * launch); gpumcd_set_profiling(ctx, 1) turns it on for the following runs. */
+typedef struct {
+    uint64_t launches;     /* kernels launched by the last run (always counted) */
+    uint32_t n_source, n_photon, n_electron, n_finalize; /* launches per class */
+    float ms_source, ms_photon, ms_electron, ms_finalize; /* 0 unless profiling is on */
+} gpumcd_profile;
+int gpumcd_set_profiling(gpumcd_ctx *ctx, int enable);
+int gpumcd_get_profile(gpumcd_ctx *ctx, gpumcd_profile *host_out); /* waits for the run's stream */
+
+/* Library-owned, NUL-terminated description of the last error on this context (or of the last
+ * failed create when ctx == NULL); valid until the next call on the same context. */
+const char *gpumcd_last_error(gpumcd_ctx *ctx);
+
+void gpumcd_destroy(gpumcd_ctx *ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -77,15 +77,17 @@ class Options:
     majorant_scale: float = 1.0
 
     def c(self):
-        return _Options(self.es_max_cm, self.f_eloss_max, self.boundary_nudge, self.pair_mode,
-                        self.photon_only, self.majorant_scale)
+        f32 = lambda v: float(np.float32(v))
+        return _Options(f32(self.es_max_cm), f32(self.f_eloss_max), f32(self.boundary_nudge), self.pair_mode,
+                        self.photon_only, f32(self.majorant_scale))
 
 
 def _tables_c(tb):
     keep = (np.ascontiguousarray(tb.photon, np.float32), np.ascontiguousarray(tb.electron, np.float32),
             np.ascontiguousarray(tb.ms_a, np.float32))
-    t = _Tables(tb.n_materials, tb.n_energy, tb.e_min, tb.e_max, _p(keep[0]), _p(keep[1]),
-                tb.n_K, tb.lnK_min, tb.lnK_max, _p(keep[2]), tb.e_cut, tb.p_cut)
+    f32 = lambda v: float(np.float32(v))   # the boundary (include/gpumcd.h) carries these as float32
+    t = _Tables(tb.n_materials, tb.n_energy, f32(tb.e_min), f32(tb.e_max), _p(keep[0]), _p(keep[1]),
+                tb.n_K, f32(tb.lnK_min), f32(tb.lnK_max), _p(keep[2]), f32(tb.e_cut), f32(tb.p_cut))
     return t, keep
 
 
@@ -99,7 +101,9 @@ def _source_c(src):
         keep = (e, w)
         n_spec = int(w.size)
         pe, pw = _p(e), _p(w)
-    s = _Source(src.particle, src.shape, src.cx, src.cy, src.wx, src.wy, src.energy, n_spec, pe, pw)
+    f32 = lambda v: float(np.float32(v))   # the boundary (include/gpumcd.h) carries these as float32
+    s = _Source(src.particle, src.shape, f32(src.cx), f32(src.cy), f32(src.wx), f32(src.wy), f32(src.energy),
+                n_spec, pe, pw)
     return s, keep
 
 
@@ -196,7 +200,7 @@ def run(density, material, voxel_cm, tables, source, n_histories, seed, options:
     trace = np.zeros(int(n_histories), np.uint64) if want_trace else None
     cnt = Counters()
     rc = lib().orc_run(_p(density), _p(material), C.c_int32(nx), C.c_int32(ny), C.c_int32(nz),
-                       C.c_double(voxel_cm), C.byref(t), C.byref(o), C.byref(s),
+                       C.c_double(float(np.float32(voxel_cm))), C.byref(t), C.byref(o), C.byref(s),
                        C.c_uint64(hist_begin), C.c_uint64(int(n_histories)), C.c_uint64(seed),
                        _p(edep), _p(dose), _p(trace), C.byref(cnt), C.c_int32(n_threads))
     if rc != 0:

@@ -1,0 +1,662 @@
+// gpumcd.cu -- kernels, scheduling and the C ABI of the B200-native GPUMCD hot path.
+//
+// See include/gpumcd.h for the boundary and DESIGN.md for the data layout and scheduling.
+#include "../../include/gpumcd.h"
+#include "transport.cuh"
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+namespace gpumcd {
+
+constexpr int kBlock = 256;
+
+// ---------------------------------------------------------------------------------------------
+// Setup kernels
+// ---------------------------------------------------------------------------------------------
+// Pack {density, material} per voxel, validate, and reduce the largest density of each material
+// (H10; positive floats order like their bit patterns, so atomicMax on the bits is a float max).
+__global__ void k_pack_phantom(const float *__restrict__ density, const uint8_t *__restrict__ material,
+                               size_t nvox, int n_mat, float2 *__restrict__ out, unsigned *rho_max_bits,
+                               unsigned *n_bad)
+{
+    __shared__ unsigned s_max[8];
+    if (threadIdx.x < 8) s_max[threadIdx.x] = 0u;
+    __syncthreads();
+    for (size_t i = blockIdx.x * static_cast<size_t>(blockDim.x) + threadIdx.x; i < nvox;
+         i += static_cast<size_t>(gridDim.x) * blockDim.x) {
+        const float d = density[i];
+        const int m = material[i];
+        if (m >= n_mat || !(d > 0.0f) || !isfinite(d)) {
+            atomicAdd(n_bad, 1u);
+            out[i] = make_float2(1.0f, __int_as_float(0));
+        } else {
+            atomicMax(&s_max[m], __float_as_uint(d));
+            out[i] = make_float2(d, __int_as_float(m));
+        }
+    }
+    __syncthreads();
+    if (threadIdx.x < 8 && s_max[threadIdx.x]) atomicMax(&rho_max_bits[threadIdx.x], s_max[threadIdx.x]);
+}
+
+struct SourceDev {
+    int particle, shape;
+    double cx, cy, wx, wy, energy;
+    int n_spec;
+    const double *cdf;   // n_spec+1, unnormalised running sum of the weights
+    const float *edges;  // n_spec+1
+};
+
+// H0: one primary per history from block (hist, track 0, ctr 0); transport starts at ctr 1.
+__global__ void k_source(Params P, SourceDev S, Queue q, unsigned long long hist0, unsigned n)
+{
+    const unsigned i = blockIdx.x * blockDim.x + threadIdx.x;
+    double e_inc = 0.0, e_cut = 0.0;
+    if (i < n) {
+        const unsigned long long hist = hist0 + i;
+        Particle p;
+        p.hist = static_cast<uint32_t>(hist);
+        p.track = 0u;
+        p.ctr = 0u;
+        const uint4 w = draw(P.rng, p);
+        double x = S.cx, y = S.cy;
+        if (S.shape == 1) {
+            x = S.cx + (static_cast<double>(u01(w.x)) - 0.5) * S.wx;
+            y = S.cy + (static_cast<double>(u01(w.y)) - 0.5) * S.wy;
+        }
+        const double vx = x / static_cast<double>(P.geo.h), vy = y / static_cast<double>(P.geo.h);
+        const double fx = floor(vx), fy = floor(vy);
+        p.ix = static_cast<int>(fx);
+        p.iy = static_cast<int>(fy);
+        p.iz = 0;
+        p.fx = static_cast<float>(vx - fx);
+        p.fy = static_cast<float>(vy - fy);
+        p.fz = 0.0f;
+        p.u = 0.0f; p.v = 0.0f; p.w = 1.0f;
+        double E = S.energy;
+        if (S.n_spec > 0) {
+            const double target = static_cast<double>(u01(w.z)) * S.cdf[S.n_spec];
+            int lo = 0, hi = S.n_spec - 1; // largest j with cdf[j] <= target, clamped to n_spec-1
+            while (lo < hi) {
+                const int mid = (lo + hi + 1) >> 1;
+                if (S.cdf[mid] <= target) lo = mid; else hi = mid - 1;
+            }
+            const double e0 = S.edges[lo], e1 = S.edges[lo + 1];
+            E = e0 + static_cast<double>(u01(w.w)) * (e1 - e0);
+        }
+        p.E = static_cast<float>(E);
+        e_inc = static_cast<double>(p.E);
+        if (S.particle == 1 && !electron_tracked(P, p.E)) {
+            // an electron below the cutoff (or photon_only): deposited where it is born
+            deposit(P, voxel_index(P.geo, p), p.E);
+            e_cut = e_inc;
+            p.E = -1.0f; // marks an empty record
+        }
+        q.A[i] = make_float4(p.fx, p.fy, p.fz, p.E);
+        q.B[i] = make_float4(p.u, p.v, p.w, __uint_as_float(pack_voxel(p.ix, p.iy, p.iz)));
+        q.C[i] = make_uint4(p.hist, p.track, p.ctr, 0u);
+    }
+    e_inc = wsum(e_inc);
+    e_cut = wsum(e_cut);
+    if ((threadIdx.x & 31) == 0) {
+        if (e_inc != 0.0) atomicAdd(&P.cnt->e_incident, e_inc);
+        if (e_cut != 0.0) atomicAdd(&P.cnt->e_dep_cutoff, e_cut);
+    }
+    if (i == 0) *q.count = n;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Scheduler 0: one launch per pass, one thread per particle, run to completion
+// (the paper's base scheme, L166: alternate the two particle types until both lists are empty)
+// ---------------------------------------------------------------------------------------------
+template <bool TRACE>
+__global__ void __launch_bounds__(kBlock) k_photon_pass(Params P, Queue in, unsigned n_in, Queue qE, Queue qG)
+{
+    const unsigned i = blockIdx.x * blockDim.x + threadIdx.x;
+    Local L;
+    if (i < n_in) {
+        const Particle p = pop(in, i);
+        if (p.E >= 0.0f) photon_run<TRACE>(P, p, L, qE, qG);
+    }
+    flush(P, L);
+}
+
+__global__ void __launch_bounds__(kBlock) k_electron_pass(Params P, Queue in, unsigned n_in, Queue qE, Queue qG)
+{
+    const unsigned i = blockIdx.x * blockDim.x + threadIdx.x;
+    Local L;
+    if (i < n_in) {
+        const Particle p = pop(in, i);
+        if (p.E >= 0.0f) electron_run(P, p, L, qE, qG);
+    }
+    flush(P, L);
+}
+
+// H8: dose = energy / mass / histories; also the total deposited energy
+__global__ void k_finalize(const double *__restrict__ edep, const float2 *__restrict__ phantom, size_t nvox,
+                           double inv_h3_n, float *__restrict__ dose, DevCounters *cnt)
+{
+    double s = 0.0;
+    for (size_t i = blockIdx.x * static_cast<size_t>(blockDim.x) + threadIdx.x; i < nvox;
+         i += static_cast<size_t>(gridDim.x) * blockDim.x) {
+        const double e = edep[i];
+        s += e;
+        if (dose) dose[i] = static_cast<float>(e / static_cast<double>(phantom[i].x) * inv_h3_n);
+    }
+    s = wsum(s);
+    __shared__ double part[32];
+    if ((threadIdx.x & 31) == 0) part[threadIdx.x >> 5] = s;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double t = 0.0;
+        for (int k = 0; k < (blockDim.x + 31) / 32; ++k) t += part[k];
+        atomicAdd(&cnt->e_dep_total, t);
+    }
+}
+
+} // namespace gpumcd
+
+// =============================================================================================
+// Host side
+// =============================================================================================
+using namespace gpumcd;
+
+struct gpumcd_ctx {
+    int nx = 0, ny = 0, nz = 0;
+    size_t nvox = 0;
+    float h = 0.f;
+    float e_max = 0.f;
+    gpumcd_options opt{};
+    // device memory
+    float2 *phantom = nullptr;
+    float *table_blob = nullptr;
+    double *edep = nullptr;
+    DevCounters *cnt = nullptr;
+    unsigned *qcount = nullptr; // 4 counters: PA, PB, EA, EB
+    float4 *qA[4] = {nullptr, nullptr, nullptr, nullptr};
+    float4 *qB[4] = {nullptr, nullptr, nullptr, nullptr};
+    uint4 *qC[4] = {nullptr, nullptr, nullptr, nullptr};
+    unsigned qcap = 0;
+    double *spec_cdf = nullptr;
+    float *spec_edges = nullptr;
+    // host state
+    Tables tab{};
+    bool have_source = false;
+    SourceDev src{};
+    cudaStream_t last_stream = nullptr;
+    unsigned long long last_n = 0;
+    unsigned long long high_water = 0;
+    bool ran = false;
+    unsigned long long hist_offset = 0;
+    // launch accounting / optional event timing
+    bool profiling = false;
+    gpumcd_profile prof{};
+    struct Ev { int cls; cudaEvent_t a, b; };
+    std::vector<Ev> events;
+    std::string err;
+};
+
+enum { CLS_SOURCE = 0, CLS_PHOTON = 1, CLS_ELECTRON = 2, CLS_FINALIZE = 3 };
+
+// bracket one kernel launch: counts it, and records an event pair when profiling is on
+struct LaunchScope {
+    gpumcd_ctx *c; cudaStream_t st; int cls; cudaEvent_t a = nullptr, b = nullptr;
+    LaunchScope(gpumcd_ctx *c_, cudaStream_t st_, int cls_) : c(c_), st(st_), cls(cls_) {
+        c->prof.launches++;
+        (&c->prof.n_source)[cls]++;
+        if (c->profiling) { cudaEventCreate(&a); cudaEventCreate(&b); cudaEventRecord(a, st); }
+    }
+    ~LaunchScope() { if (c->profiling) { cudaEventRecord(b, st); c->events.push_back({cls, a, b}); } }
+};
+
+static std::string g_create_error;
+
+#define CK(call)                                                                                   \
+    do {                                                                                           \
+        cudaError_t e_ = (call);                                                                   \
+        if (e_ != cudaSuccess) {                                                                   \
+            char buf_[512];                                                                        \
+            snprintf(buf_, sizeof buf_, "%s failed: %s (%s:%d)", #call, cudaGetErrorString(e_), __FILE__, __LINE__); \
+            set_error(ctx, buf_);                                                                  \
+            return e_ == cudaErrorMemoryAllocation ? GPUMCD_ERR_OOM : GPUMCD_ERR_CUDA;             \
+        }                                                                                          \
+    } while (0)
+
+static void set_error(gpumcd_ctx *ctx, const char *msg)
+{
+    if (ctx) ctx->err = msg; else g_create_error = msg;
+}
+
+static Queue make_queue(gpumcd_ctx *c, int k)
+{
+    Queue q;
+    q.A = c->qA[k]; q.B = c->qB[k]; q.C = c->qC[k];
+    q.count = c->qcount + k;
+    q.cap = c->qcap;
+    return q;
+}
+
+extern "C" int gpumcd_default_options(gpumcd_options *opt)
+{
+    if (!opt) return GPUMCD_ERR_INVALID_ARG;
+    opt->es_max_cm = 0.5f;
+    opt->f_eloss_max = 0.25f;
+    opt->boundary_nudge = 1e-4f;
+    opt->pair_mode = 1;
+    opt->photon_only = 0;
+    opt->majorant_scale = 1.0f;
+    opt->wave_size = 1u << 20;
+    opt->bank_factor = 8;
+    opt->scheduler = 0;
+    opt->reserved = 0;
+    return GPUMCD_OK;
+}
+
+static void destroy_impl(gpumcd_ctx *c)
+{
+    if (!c) return;
+    cudaFree(c->phantom);
+    cudaFree(c->table_blob);
+    cudaFree(c->edep);
+    cudaFree(c->cnt);
+    cudaFree(c->qcount);
+    for (int k = 0; k < 4; ++k) { cudaFree(c->qA[k]); cudaFree(c->qB[k]); cudaFree(c->qC[k]); }
+    cudaFree(c->spec_cdf);
+    cudaFree(c->spec_edges);
+    for (auto &e : c->events) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
+    delete c;
+}
+
+static int create_impl(gpumcd_ctx **out, const float *density, const uint8_t *material, bool on_host, int nx,
+                       int ny, int nz, float voxel_cm, const gpumcd_tables *t, const gpumcd_options *opt_in)
+{
+    gpumcd_ctx *ctx = nullptr; // errors before allocation go to the global string
+    if (!out) return GPUMCD_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (!density || !material || !t) { set_error(nullptr, "null pointer argument"); return GPUMCD_ERR_INVALID_ARG; }
+    if (nx < 1 || ny < 1 || nz < 1 || nx > 1024 || ny > 1024 || nz > 1024 || !(voxel_cm > 0.f)) {
+        set_error(nullptr, "bad phantom dimensions (1..1024 per axis, voxel size > 0)");
+        return GPUMCD_ERR_INVALID_ARG;
+    }
+    if (t->n_materials < 1 || t->n_materials > 8 || t->n_energy < 2 || !t->photon || !t->electron || !t->ms_a ||
+        t->n_K < 2 || !(t->e_min > 0.f) || !(t->e_max > t->e_min) || !(t->lnK_max > t->lnK_min) ||
+        t->e_cut < t->e_min || t->p_cut < t->e_min) {
+        set_error(nullptr, "bad table description");
+        return GPUMCD_ERR_INVALID_ARG;
+    }
+    gpumcd_options opt;
+    gpumcd_default_options(&opt);
+    if (opt_in) opt = *opt_in;
+    if (!(opt.es_max_cm > 0.f) || !(opt.f_eloss_max > 0.f) || opt.f_eloss_max > 1.f || opt.boundary_nudge < 0.f ||
+        !(opt.majorant_scale >= 1.f) || opt.wave_size == 0 || opt.bank_factor == 0 ||
+        static_cast<unsigned long long>(opt.wave_size) * opt.bank_factor > 0x7fffffffull) {
+        set_error(nullptr, "bad options");
+        return GPUMCD_ERR_INVALID_ARG;
+    }
+    ctx = new gpumcd_ctx;
+    struct Guard { gpumcd_ctx *&c; bool ok = false; ~Guard() { if (!ok) { if (c) g_create_error = c->err; destroy_impl(c); } } } guard{ctx};
+    ctx->nx = nx; ctx->ny = ny; ctx->nz = nz; ctx->h = voxel_cm;
+    ctx->nvox = static_cast<size_t>(nx) * ny * nz;
+    ctx->opt = opt;
+    const size_t nvox = ctx->nvox;
+    const int nE = t->n_energy, nK = t->n_K, nM = t->n_materials;
+
+    // ---- phantom ----
+    const float *d_density = density;
+    const uint8_t *d_material = material;
+    float *tmp_density = nullptr;
+    uint8_t *tmp_material = nullptr;
+    if (on_host) {
+        CK(cudaMalloc(&tmp_density, nvox * sizeof(float)));
+        CK(cudaMalloc(&tmp_material, nvox));
+        CK(cudaMemcpy(tmp_density, density, nvox * sizeof(float), cudaMemcpyHostToDevice));
+        CK(cudaMemcpy(tmp_material, material, nvox, cudaMemcpyHostToDevice));
+        d_density = tmp_density;
+        d_material = tmp_material;
+    }
+    CK(cudaMalloc(&ctx->phantom, nvox * sizeof(float2)));
+    unsigned *d_scratch = nullptr;
+    CK(cudaMalloc(&d_scratch, 9 * sizeof(unsigned)));
+    CK(cudaMemset(d_scratch, 0, 9 * sizeof(unsigned)));
+    {
+        const int grid = static_cast<int>(std::min<size_t>((nvox + kBlock - 1) / kBlock, 148 * 8));
+        k_pack_phantom<<<grid, kBlock>>>(d_density, d_material, nvox, nM, ctx->phantom, d_scratch, d_scratch + 8);
+        CK(cudaGetLastError());
+    }
+    unsigned h_scratch[9];
+    CK(cudaMemcpy(h_scratch, d_scratch, sizeof h_scratch, cudaMemcpyDeviceToHost));
+    cudaFree(d_scratch);
+    cudaFree(tmp_density);
+    cudaFree(tmp_material);
+    if (h_scratch[8] != 0) {
+        set_error(ctx, "phantom has a material id >= n_materials or a density that is not a positive finite number");
+        return GPUMCD_ERR_INVALID_ARG;
+    }
+    double rho_max[8];
+    for (int m = 0; m < 8; ++m) { float f; memcpy(&f, &h_scratch[m], 4); rho_max[m] = f; }
+
+    // ---- tables: one device blob = photon | electron | mu_max | m_e | ms_a ----
+    // H10 majorants: mu_max(E_i) = max_m rho_max[m] mu_m(E_i) (Eq. 3); M_e = running max in E of
+    // max_m rho_max[m] (Sigma_Moller + Sigma_brems) (L110-113 made rigorous).
+    const size_t n_ph = static_cast<size_t>(nM) * 3 * nE, n_el = static_cast<size_t>(nM) * 4 * nE;
+    std::vector<float> blob(n_ph + n_el + 2 * static_cast<size_t>(nE) + nK);
+    memcpy(blob.data(), t->photon, n_ph * sizeof(float));
+    memcpy(blob.data() + n_ph, t->electron, n_el * sizeof(float));
+    float *mu_max = blob.data() + n_ph + n_el, *m_e = mu_max + nE;
+    double run = 0.0;
+    for (int i = 0; i < nE; ++i) {
+        double mu = 0.0, se = 0.0;
+        for (int m = 0; m < nM; ++m) {
+            const float *p = t->photon + static_cast<size_t>(m) * 3 * nE;
+            const float *e = t->electron + static_cast<size_t>(m) * 4 * nE;
+            mu = std::max(mu, rho_max[m] * (static_cast<double>(p[i]) + p[nE + i] + p[2 * nE + i]));
+            se = std::max(se, rho_max[m] * (static_cast<double>(e[nE + i]) + e[2 * nE + i]));
+        }
+        run = std::max(run, se);
+        mu_max[i] = static_cast<float>(mu * opt.majorant_scale);
+        m_e[i] = static_cast<float>(run * opt.majorant_scale);
+    }
+    memcpy(m_e + nE, t->ms_a, static_cast<size_t>(nK) * sizeof(float));
+    CK(cudaMalloc(&ctx->table_blob, blob.size() * sizeof(float)));
+    CK(cudaMemcpy(ctx->table_blob, blob.data(), blob.size() * sizeof(float), cudaMemcpyHostToDevice));
+    Tables &tb = ctx->tab;
+    tb.ph = ctx->table_blob;
+    tb.el = tb.ph + n_ph;
+    tb.mu_max = tb.el + n_el;
+    tb.m_e = tb.mu_max + nE;
+    tb.ms_a = tb.m_e + nE;
+    tb.gE.n = nE;
+    tb.gE.x_min = static_cast<float>(std::log(static_cast<double>(t->e_min)));
+    tb.gE.inv_dx = static_cast<float>((nE - 1) / (std::log(static_cast<double>(t->e_max)) - std::log(static_cast<double>(t->e_min))));
+    tb.gK.n = nK;
+    tb.gK.x_min = t->lnK_min;
+    tb.gK.inv_dx = static_cast<float>((nK - 1) / (static_cast<double>(t->lnK_max) - static_cast<double>(t->lnK_min)));
+    tb.e_min = t->e_min; tb.e_cut = t->e_cut; tb.p_cut = t->p_cut;
+    ctx->e_max = t->e_max;
+    tb.n_mat = nM;
+
+    // ---- tally, counters, queues ----
+    CK(cudaMalloc(&ctx->edep, nvox * sizeof(double)));
+    CK(cudaMalloc(&ctx->cnt, sizeof(DevCounters)));
+    CK(cudaMalloc(&ctx->qcount, 4 * sizeof(unsigned)));
+    ctx->qcap = opt.wave_size * opt.bank_factor;
+    for (int k = 0; k < 4; ++k) {
+        CK(cudaMalloc(&ctx->qA[k], static_cast<size_t>(ctx->qcap) * sizeof(float4)));
+        CK(cudaMalloc(&ctx->qB[k], static_cast<size_t>(ctx->qcap) * sizeof(float4)));
+        CK(cudaMalloc(&ctx->qC[k], static_cast<size_t>(ctx->qcap) * sizeof(uint4)));
+    }
+    CK(cudaDeviceSynchronize());
+    guard.ok = true;
+    *out = ctx;
+    return GPUMCD_OK;
+}
+
+extern "C" int gpumcd_create(gpumcd_ctx **out, const float *density_dev, const uint8_t *material_dev, int nx, int ny,
+                             int nz, float voxel_cm, const gpumcd_tables *tables, const gpumcd_options *opt)
+{
+    return create_impl(out, density_dev, material_dev, false, nx, ny, nz, voxel_cm, tables, opt);
+}
+
+extern "C" int gpumcd_create_host(gpumcd_ctx **out, const float *density_host, const uint8_t *material_host, int nx,
+                                  int ny, int nz, float voxel_cm, const gpumcd_tables *tables,
+                                  const gpumcd_options *opt)
+{
+    return create_impl(out, density_host, material_host, true, nx, ny, nz, voxel_cm, tables, opt);
+}
+
+extern "C" int gpumcd_set_source(gpumcd_ctx *ctx, const gpumcd_source *s)
+{
+    if (!ctx || !s) return GPUMCD_ERR_INVALID_ARG;
+    if ((s->particle != 0 && s->particle != 1) || (s->shape != 0 && s->shape != 1) || s->n_spec < 0) {
+        set_error(ctx, "bad source description");
+        return GPUMCD_ERR_INVALID_ARG;
+    }
+    const double wx = s->shape == 1 ? s->wx : 0.0, wy = s->shape == 1 ? s->wy : 0.0;
+    if (wx < 0 || wy < 0 || s->cx - 0.5 * wx < 0 || s->cx + 0.5 * wx >= static_cast<double>(ctx->nx) * ctx->h ||
+        s->cy - 0.5 * wy < 0 || s->cy + 0.5 * wy >= static_cast<double>(ctx->ny) * ctx->h) {
+        set_error(ctx, "the source field does not lie inside the z = 0 face of the phantom");
+        return GPUMCD_ERR_INVALID_ARG;
+    }
+    const float e_lo = ctx->tab.e_min, e_hi = ctx->e_max;
+    SourceDev d{};
+    d.particle = s->particle; d.shape = s->shape;
+    d.cx = s->cx; d.cy = s->cy; d.wx = wx; d.wy = wy; d.energy = s->energy;
+    d.n_spec = s->n_spec;
+    cudaFree(ctx->spec_cdf); ctx->spec_cdf = nullptr;
+    cudaFree(ctx->spec_edges); ctx->spec_edges = nullptr;
+    if (s->n_spec > 0) {
+        if (!s->spec_E || !s->spec_w) { set_error(ctx, "null spectrum arrays"); return GPUMCD_ERR_INVALID_ARG; }
+        std::vector<double> cdf(s->n_spec + 1);
+        cdf[0] = 0.0;
+        for (int j = 0; j < s->n_spec; ++j) {
+            if (!(s->spec_w[j] >= 0.f) || !(s->spec_E[j + 1] > s->spec_E[j])) {
+                set_error(ctx, "spectrum weights must be >= 0 and edges increasing");
+                return GPUMCD_ERR_INVALID_ARG;
+            }
+            cdf[j + 1] = cdf[j] + static_cast<double>(s->spec_w[j]);
+        }
+        if (!(cdf[s->n_spec] > 0.0)) { set_error(ctx, "spectrum has zero total weight"); return GPUMCD_ERR_INVALID_ARG; }
+        if (s->spec_E[0] < e_lo || s->spec_E[s->n_spec] > e_hi) {
+            set_error(ctx, "spectrum extends outside the energy range of the tables");
+            return GPUMCD_ERR_TABLE_RANGE;
+        }
+        CK(cudaMalloc(&ctx->spec_cdf, cdf.size() * sizeof(double)));
+        CK(cudaMalloc(&ctx->spec_edges, cdf.size() * sizeof(float)));
+        CK(cudaMemcpy(ctx->spec_cdf, cdf.data(), cdf.size() * sizeof(double), cudaMemcpyHostToDevice));
+        CK(cudaMemcpy(ctx->spec_edges, s->spec_E, cdf.size() * sizeof(float), cudaMemcpyHostToDevice));
+        d.cdf = ctx->spec_cdf;
+        d.edges = ctx->spec_edges;
+    } else if (s->energy < e_lo || s->energy > e_hi) {
+        set_error(ctx, "source energy outside the energy range of the tables");
+        return GPUMCD_ERR_TABLE_RANGE;
+    }
+    ctx->src = d;
+    ctx->have_source = true;
+    return GPUMCD_OK;
+}
+
+static Params make_params(gpumcd_ctx *ctx, uint64_t seed, uint32_t hist_hi, bool photon_only, unsigned long long *trace)
+{
+    Params P;
+    P.tab = ctx->tab;
+    P.geo.phantom = ctx->phantom;
+    P.geo.nx = ctx->nx; P.geo.ny = ctx->ny; P.geo.nz = ctx->nz;
+    P.geo.h = ctx->h; P.geo.inv_h = 1.0f / ctx->h;
+    P.opt.es_max = ctx->opt.es_max_cm;
+    P.opt.f_eloss = ctx->opt.f_eloss_max;
+    P.opt.nudge = ctx->opt.boundary_nudge;
+    P.opt.pair_mode = ctx->opt.pair_mode;
+    P.opt.photon_only = photon_only ? 1 : ctx->opt.photon_only;
+    P.rng.k0 = static_cast<uint32_t>(seed);
+    P.rng.k1 = static_cast<uint32_t>(seed >> 32);
+    P.rng.hist_hi = hist_hi;
+    P.edep = ctx->edep;
+    P.cnt = ctx->cnt;
+    P.trace = trace;
+    P.trace_off = ctx->hist_offset;
+    return P;
+}
+
+// Scheduler 0: per wave, fill the source list, then alternate photon and electron
+// passes until both lists are empty; the host reads the list lengths between passes.
+static int run_waves_host_loop(gpumcd_ctx *ctx, uint64_t n_hist, uint64_t seed, bool trace_mode,
+                               unsigned long long *trace, cudaStream_t st)
+{
+    enum { PA = 0, PB = 1, EA = 2, EB = 3 };
+    int pcur = PA, pnext = PB, ecur = EA, enext = EB;
+    uint64_t h0 = ctx->hist_offset;
+    const uint64_t h_end = ctx->hist_offset + n_hist;
+    while (h0 < h_end) {
+        uint64_t n = std::min<uint64_t>(ctx->opt.wave_size, h_end - h0);
+        n = std::min<uint64_t>(n, 0x100000000ull - (h0 & 0xffffffffull)); // a wave never straddles 2^32
+        const Params P = make_params(ctx, seed, static_cast<uint32_t>(h0 >> 32), trace_mode, trace);
+        CK(cudaMemsetAsync(ctx->qcount, 0, 4 * sizeof(unsigned), st));
+        const int src_q = ctx->src.particle == 0 ? pcur : ecur;
+        { LaunchScope ls(ctx, st, CLS_SOURCE);
+        k_source<<<static_cast<unsigned>((n + kBlock - 1) / kBlock), kBlock, 0, st>>>(P, ctx->src, make_queue(ctx, src_q), h0,
+                                                                                      static_cast<unsigned>(n)); }
+        CK(cudaGetLastError());
+        unsigned cnt[4];
+        for (;;) {
+            CK(cudaMemcpyAsync(cnt, ctx->qcount, sizeof cnt, cudaMemcpyDeviceToHost, st));
+            CK(cudaStreamSynchronize(st));
+            for (int k = 0; k < 4; ++k) ctx->high_water = std::max<unsigned long long>(ctx->high_water, cnt[k]);
+            if (cnt[0] > ctx->qcap || cnt[1] > ctx->qcap || cnt[2] > ctx->qcap || cnt[3] > ctx->qcap) {
+                set_error(ctx, "particle queue overflow: raise bank_factor or lower wave_size");
+                return GPUMCD_ERR_BANK_OVERFLOW;
+            }
+            if (cnt[pcur] > 0) {
+                const unsigned m = cnt[pcur];
+                // photons: secondaries of the same type go to the other photon list, electrons are
+                // appended to the current electron list (not being consumed now)
+                { LaunchScope ls(ctx, st, CLS_PHOTON);
+                if (trace_mode)
+                    k_photon_pass<true><<<(m + kBlock - 1) / kBlock, kBlock, 0, st>>>(P, make_queue(ctx, pcur), m, make_queue(ctx, ecur), make_queue(ctx, pnext));
+                else
+                    k_photon_pass<false><<<(m + kBlock - 1) / kBlock, kBlock, 0, st>>>(P, make_queue(ctx, pcur), m, make_queue(ctx, ecur), make_queue(ctx, pnext)); }
+                CK(cudaGetLastError());
+                CK(cudaMemsetAsync(ctx->qcount + pcur, 0, sizeof(unsigned), st));
+                std::swap(pcur, pnext);
+            } else if (cnt[ecur] > 0) {
+                const unsigned m = cnt[ecur];
+                { LaunchScope ls(ctx, st, CLS_ELECTRON);
+                k_electron_pass<<<(m + kBlock - 1) / kBlock, kBlock, 0, st>>>(P, make_queue(ctx, ecur), m, make_queue(ctx, enext), make_queue(ctx, pcur)); }
+                CK(cudaGetLastError());
+                CK(cudaMemsetAsync(ctx->qcount + ecur, 0, sizeof(unsigned), st));
+                std::swap(ecur, enext);
+            } else {
+                break;
+            }
+        }
+        h0 += n;
+    }
+    return GPUMCD_OK;
+}
+
+static int run_impl(gpumcd_ctx *ctx, uint64_t n_hist, uint64_t seed, float *dose_dev, unsigned long long *trace_dev,
+                    cudaStream_t st)
+{
+    if (!ctx) return GPUMCD_ERR_INVALID_ARG;
+    if (!ctx->have_source) { set_error(ctx, "gpumcd_run called before gpumcd_set_source"); return GPUMCD_ERR_NO_SOURCE; }
+    if (n_hist == 0) { set_error(ctx, "n_histories must be > 0"); return GPUMCD_ERR_INVALID_ARG; }
+    ctx->last_stream = st;
+    ctx->last_n = n_hist;
+    ctx->high_water = 0;
+    ctx->ran = true;
+    ctx->prof = gpumcd_profile{};
+    for (auto &e : ctx->events) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
+    ctx->events.clear();
+    CK(cudaMemsetAsync(ctx->edep, 0, ctx->nvox * sizeof(double), st));
+    CK(cudaMemsetAsync(ctx->cnt, 0, sizeof(DevCounters), st));
+    if (trace_dev) CK(cudaMemsetAsync(trace_dev, 0, n_hist * sizeof(unsigned long long), st));
+    const int rc = run_waves_host_loop(ctx, n_hist, seed, trace_dev != nullptr, trace_dev, st);
+    if (rc != GPUMCD_OK) return rc;
+    const double h3 = static_cast<double>(ctx->h) * ctx->h * ctx->h;
+    const int grid = static_cast<int>(std::min<size_t>((ctx->nvox + kBlock - 1) / kBlock, 148 * 8));
+    { LaunchScope ls(ctx, st, CLS_FINALIZE);
+    k_finalize<<<grid, kBlock, 0, st>>>(ctx->edep, ctx->phantom, ctx->nvox, 1.0 / (h3 * static_cast<double>(n_hist)),
+                                        dose_dev, ctx->cnt); }
+    CK(cudaGetLastError());
+    return GPUMCD_OK;
+}
+
+extern "C" int gpumcd_run(gpumcd_ctx *ctx, uint64_t n_histories, uint64_t seed, float *dose_out_dev, void *cuda_stream)
+{
+    if (!ctx || !dose_out_dev) return GPUMCD_ERR_INVALID_ARG;
+    return run_impl(ctx, n_histories, seed, dose_out_dev, nullptr, static_cast<cudaStream_t>(cuda_stream));
+}
+
+extern "C" int gpumcd_run_host(gpumcd_ctx *ctx, uint64_t n_histories, uint64_t seed, float *dose_out_host,
+                               void *cuda_stream)
+{
+    if (!ctx || !dose_out_host) return GPUMCD_ERR_INVALID_ARG;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    float *tmp = nullptr;
+    CK(cudaMalloc(&tmp, ctx->nvox * sizeof(float)));
+    int rc = run_impl(ctx, n_histories, seed, tmp, nullptr, st);
+    if (rc == GPUMCD_OK) {
+        cudaError_t e = cudaMemcpyAsync(dose_out_host, tmp, ctx->nvox * sizeof(float), cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        if (e != cudaSuccess) { set_error(ctx, cudaGetErrorString(e)); rc = GPUMCD_ERR_CUDA; }
+    }
+    cudaFree(tmp);
+    return rc;
+}
+
+extern "C" int gpumcd_run_trace(gpumcd_ctx *ctx, uint64_t n_histories, uint64_t seed, uint64_t *trace_out_dev,
+                                void *cuda_stream)
+{
+    if (!ctx || !trace_out_dev) return GPUMCD_ERR_INVALID_ARG;
+    return run_impl(ctx, n_histories, seed, nullptr, reinterpret_cast<unsigned long long *>(trace_out_dev),
+                    static_cast<cudaStream_t>(cuda_stream));
+}
+
+extern "C" int gpumcd_get_counters(gpumcd_ctx *ctx, gpumcd_counters *out)
+{
+    if (!ctx || !out) return GPUMCD_ERR_INVALID_ARG;
+    memset(out, 0, sizeof *out);
+    if (!ctx->ran) return GPUMCD_OK;
+    DevCounters d;
+    CK(cudaStreamSynchronize(ctx->last_stream));
+    CK(cudaMemcpy(&d, ctx->cnt, sizeof d, cudaMemcpyDeviceToHost));
+    out->n_histories = ctx->last_n;
+    out->photon_flights = d.photon_flights; out->photon_compton = d.photon_compton;
+    out->photon_photo = d.photon_photo; out->photon_pair = d.photon_pair; out->photon_fict = d.photon_fict;
+    out->ch_steps = d.ch_steps; out->hard_moller = d.hard_moller; out->hard_brems = d.hard_brems;
+    out->hard_fict = d.hard_fict; out->pushes_e = d.pushes_e; out->pushes_g = d.pushes_g;
+    out->bank_high_water = ctx->high_water;
+    out->overflow_count = d.overflow;
+    out->e_incident = d.e_incident;
+    out->e_dep_cutoff = d.e_dep_cutoff;
+    out->e_dep_continuous = d.e_dep_total - d.e_dep_cutoff;
+    out->e_escaped = d.e_escaped;
+    out->e_pair_rest = d.e_pair_rest;
+    if (d.overflow) { set_error(ctx, "particle queue overflow: the result is invalid"); return GPUMCD_ERR_BANK_OVERFLOW; }
+    return GPUMCD_OK;
+}
+
+extern "C" int gpumcd_get_energy_tally(gpumcd_ctx *ctx, double *edep_out_dev)
+{
+    if (!ctx || !edep_out_dev) return GPUMCD_ERR_INVALID_ARG;
+    CK(cudaMemcpyAsync(edep_out_dev, ctx->edep, ctx->nvox * sizeof(double), cudaMemcpyDeviceToDevice, ctx->last_stream));
+    return GPUMCD_OK;
+}
+
+extern "C" int gpumcd_set_history_offset(gpumcd_ctx *ctx, uint64_t first_history)
+{
+    if (!ctx) return GPUMCD_ERR_INVALID_ARG;
+    ctx->hist_offset = first_history;
+    return GPUMCD_OK;
+}
+
+extern "C" int gpumcd_set_profiling(gpumcd_ctx *ctx, int enable)
+{
+    if (!ctx) return GPUMCD_ERR_INVALID_ARG;
+    ctx->profiling = enable != 0;
+    return GPUMCD_OK;
+}
+
+extern "C" int gpumcd_get_profile(gpumcd_ctx *ctx, gpumcd_profile *out)
+{
+    if (!ctx || !out) return GPUMCD_ERR_INVALID_ARG;
+    if (ctx->ran) CK(cudaStreamSynchronize(ctx->last_stream));
+    gpumcd_profile p = ctx->prof;
+    for (auto &e : ctx->events) {
+        float ms = 0.f;
+        CK(cudaEventElapsedTime(&ms, e.a, e.b));
+        (&p.ms_source)[e.cls] += ms;
+    }
+    *out = p;
+    return GPUMCD_OK;
+}
+
+extern "C" const char *gpumcd_last_error(gpumcd_ctx *ctx)
+{
+    return ctx ? ctx->err.c_str() : g_create_error.c_str();
+}
+
+extern "C" void gpumcd_destroy(gpumcd_ctx *ctx) { destroy_impl(ctx); }

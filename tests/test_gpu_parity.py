@@ -1,0 +1,239 @@
+"""-m gpu: the CUDA hot path against the CPU oracle on the same seeded inputs, through the C ABI.
+
+Tolerances are BASELINE.json's north_star:
+  * photon-only replay: per-history interaction sequences identical for >= 99.9 % of histories;
+  * total deposited energy within 1e-5 relative;
+  * per-voxel dose within 3 sqrt(s_gpu^2 + s_cpu^2) for >= 99 % of voxels above 10 % of the maximum;
+  * gamma 2 %/2 mm pass rate >= 99 %.
+Because both sides draw from the same Philox streams, agreement is much tighter than these bars;
+the extra "replay" assertions below measure that.
+"""
+import dataclasses
+
+import numpy as np
+import pytest
+
+import oracle
+from gpu_util import run_gpu
+from paper_1101_1245_b200 import evaluation as ev
+from paper_1101_1245_b200.inputs import ELECTRON, PENCIL, PHOTON, RECTANGLE, Source, make_config, phantoms
+
+pytestmark = pytest.mark.gpu
+
+# histories per config for parity (the oracle must finish in seconds); config 1 runs at full size
+PARITY_N = {1: 100_000, 2: 40_000, 3: 200_000, 4: 200_000, 5: 200_000}
+INT_KEYS = ("photon_flights", "photon_compton", "photon_photo", "photon_pair", "photon_fict", "ch_steps",
+            "hard_moller", "hard_brems", "hard_fict", "pushes_e", "pushes_g")
+
+
+@pytest.fixture(scope="module")
+def workloads():
+    return {i: make_config(i) for i in (1, 2, 3, 4, 5)}
+
+
+def total_deposit(c):
+    return c["e_dep_continuous"] + c["e_dep_cutoff"]
+
+
+@pytest.mark.parametrize("cfg", [1, 3, 4, 5])
+def test_photon_only_replay_sequences(cfg, workloads):
+    w = workloads[cfg]
+    n = PARITY_N[cfg]
+    o = oracle.run_workload(w, n, oracle.Options(photon_only=1), want_trace=True)
+    g = run_gpu(w, n, want_trace=True, want_edep=False)
+    same = np.mean(o.trace == g["trace"])
+    assert same >= 0.999, f"only {same:.5f} of the histories replay identically"
+    for k in ("photon_flights", "photon_compton", "photon_photo", "photon_pair", "photon_fict"):
+        assert abs(g["counters"][k] - o.counters[k]) <= 2e-4 * max(o.counters[k], 1000), k
+    assert g["counters"]["ch_steps"] == 0 and g["counters"]["pushes_e"] == 0
+
+
+@pytest.mark.parametrize("cfg", [1, 2, 3, 4, 5])
+def test_dose_parity(cfg, workloads):
+    w = workloads[cfg]
+    n = PARITY_N[cfg]
+    nb = 8
+    og, gg = [], []
+    oc = gc = None
+    for b in range(nb):
+        o = oracle.run(w.density, w.material, w.voxel_cm, w.tables, w.source, n // nb, seed=w.seed + 1000 * b)
+        g = run_gpu(w, n // nb, seed=w.seed + 1000 * b)
+        og.append(o.edep)
+        gg.append(g["edep"])
+        oc = o.counters if oc is None else {k: oc[k] + v for k, v in o.counters.items()}
+        gc = g["counters"] if gc is None else {k: gc[k] + v for k, v in g["counters"].items()}
+        assert g["counters"]["overflow_count"] == 0
+        # the dose grid is the energy tally divided by the voxel mass and the number of histories
+        expect = g["edep"] / (w.density.astype(np.float64) * w.voxel_cm**3) / (n // nb)
+        np.testing.assert_allclose(g["dose"], expect.astype(np.float32), rtol=2e-6, atol=0)
+    # --- total deposited energy, 1e-5 relative
+    rel = abs(total_deposit(gc) - total_deposit(oc)) / total_deposit(oc)
+    assert rel <= 1e-5, f"total deposited energy differs by {rel:.2e}"
+    # --- energy conservation on the GPU side
+    bal = (total_deposit(gc) + gc["e_escaped"]) / gc["e_incident"] - 1.0
+    assert abs(bal) <= 1e-6
+    assert gc["e_incident"] == pytest.approx(oc["e_incident"], rel=1e-7)
+    # --- event counts replay almost exactly
+    for k in INT_KEYS:
+        assert abs(gc[k] - oc[k]) <= 5e-4 * max(oc[k], 2000), (k, gc[k], oc[k])
+    # --- per-voxel agreement within the combined statistical uncertainty
+    om, os_ = ev.batch_mean_sigma(np.array(og))
+    gm, gs = ev.batch_mean_sigma(np.array(gg))
+    assert ev.voxel_agreement(om, os_, gm, gs, frac=0.1, k=3.0) >= 0.99
+    # --- gamma 2 %/2 mm, reference = oracle
+    mass = w.density.astype(np.float64) * w.voxel_cm**3
+    assert ev.gamma_pass_rate(om / mass, gm / mass, w.voxel_cm, frac=0.1) >= 0.99
+    # --- replay quality: the two dose grids differ far less than their statistical noise
+    sel = om > 0.1 * om.max()
+    noise = np.sqrt(np.mean(os_[sel] ** 2))
+    diff = np.sqrt(np.mean((gm[sel] - om[sel]) ** 2))
+    assert diff < 0.2 * noise, f"rms difference {diff:.3e} vs statistical noise {noise:.3e}"
+
+
+def test_config1_full_size_sampled_voxels(workloads):
+    """Config 1 at BASELINE.json's full size and seed: every voxel on the beam axis."""
+    w = workloads[1]
+    o = oracle.run_workload(w)
+    g = run_gpu(w)
+    assert g["counters"]["n_histories"] == 100_000
+    axis_o = o.edep[:, 16, 16]
+    axis_g = g["edep"][:, 16, 16]
+    np.testing.assert_allclose(axis_g, axis_o, rtol=2e-3)
+    assert abs(g["edep"].sum() - o.edep.sum()) / o.edep.sum() <= 1e-5
+
+
+def test_same_seed_is_reproducible(workloads):
+    w = workloads[3]
+    a = run_gpu(w, 30_000)
+    b = run_gpu(w, 30_000)
+    for k in INT_KEYS:
+        assert a["counters"][k] == b["counters"][k]
+    scale = a["edep"].max()
+    assert np.abs(a["edep"] - b["edep"]).max() <= 1e-12 * scale       # fp64 atomic-order noise only
+    c = run_gpu(w, 30_000, seed=w.seed + 1)
+    assert c["counters"]["ch_steps"] != a["counters"]["ch_steps"]
+
+
+@pytest.mark.parametrize("n,wave", [(1, 1 << 20), (31, 1 << 20), (2500, 1000), (4097, 4096), (70_001, 1 << 15)])
+def test_ragged_sizes_and_waves(n, wave, workloads):
+    """History counts that are not multiples of the block, the warp or the wave size."""
+    w = workloads[3]
+    o = oracle.run_workload(w, n)
+    g = run_gpu(w, n, wave_size=wave)
+    for k in INT_KEYS:
+        assert abs(g["counters"][k] - o.counters[k]) <= max(3, 2e-3 * o.counters[k]), k
+    assert g["counters"]["e_incident"] == pytest.approx(n * 15.0, rel=1e-7)
+    assert g["edep"].sum() == pytest.approx(o.edep.sum(), rel=1e-3 if n > 1000 else 0.2)
+
+
+def test_wave_partition_does_not_change_the_result(workloads):
+    w = workloads[4]
+    a = run_gpu(w, 50_000, wave_size=1 << 20)
+    b = run_gpu(w, 50_000, wave_size=7000)
+    for k in INT_KEYS:
+        assert a["counters"][k] == b["counters"][k]
+    assert np.abs(a["edep"] - b["edep"]).max() <= 1e-12 * a["edep"].max()
+    assert b["counters"]["bank_high_water"] <= 7000 * 8
+
+
+def test_pair_rest_energy_deposited_locally(workloads):
+    w = workloads[3]
+    n = 50_000
+    o = oracle.run_workload(w, n, oracle.Options(pair_mode=0))
+    g = run_gpu(w, n, pair_mode=0)
+    assert g["counters"]["photon_pair"] == pytest.approx(o.counters["photon_pair"], rel=1e-3)
+    assert g["counters"]["e_pair_rest"] == pytest.approx(o.counters["e_pair_rest"], rel=1e-3)
+    assert abs(g["edep"].sum() - o.edep.sum()) / o.edep.sum() <= 1e-4
+    bal = (total_deposit(g["counters"]) + g["counters"]["e_escaped"]) / g["counters"]["e_incident"] - 1
+    assert abs(bal) <= 1e-6
+
+
+def test_electron_source_deposited_at_birth_maps_the_field(water_tables):
+    rho, mat = phantoms.homogeneous(16, 16, 4, 1.0, 0)
+    src = Source(ELECTRON, RECTANGLE, 4.0, 3.5, 3.0, 2.0, energy=5.0)
+    w = dataclasses.replace(make_config(1), density=rho, material=mat, voxel_cm=0.5, tables=water_tables, source=src)
+    n = 100_000
+    o = oracle.run(rho, mat, 0.5, water_tables, src, n, seed=9, options=oracle.Options(photon_only=1))
+    g = run_gpu(w, n, seed=9, photon_only=1)
+    np.testing.assert_allclose(g["edep"], o.edep, rtol=1e-12, atol=1e-9)   # identical voxel for every primary
+    assert g["counters"]["ch_steps"] == 0
+
+
+def test_spectrum_source(workloads):
+    w = workloads[5]
+    n = 100_000
+    o = oracle.run_workload(w, n, oracle.Options(photon_only=1))
+    g = run_gpu(w, n, photon_only=1)
+    assert g["counters"]["e_incident"] == pytest.approx(o.counters["e_incident"], rel=1e-6)
+    assert abs(g["edep"].sum() - o.edep.sum()) / o.edep.sum() <= 1e-4
+
+
+def test_majorant_inflation_changes_only_fictitious_counts(workloads):
+    """Woodcock tracking is not an approximation."""
+    w = workloads[4]
+    n = 200_000
+    a = run_gpu(w, n)
+    b = run_gpu(w, n, majorant_scale=2.0)
+    assert b["counters"]["photon_fict"] > 1.5 * a["counters"]["photon_fict"]
+    da, db = a["edep"].sum(axis=(1, 2)), b["edep"].sum(axis=(1, 2))
+    sel = da > 0.2 * da.max()
+    # 200k histories: depth-dose curves agree to ~1 % per slice
+    assert np.abs(db[sel] / da[sel] - 1).max() < 0.04
+    assert abs(db.sum() / da.sum() - 1) < 0.01
+
+
+def test_host_entry_points_match_device_entry_points(workloads):
+    import paper_1101_1245_b200 as g
+
+    w = workloads[1]
+    n = 20_000
+    ref = run_gpu(w, n)
+    dose = np.empty(w.density.shape, np.float32)
+    with g.gpumcd_create_host(w.density, w.material, w.voxel_cm, w.tables) as ctx:
+        g.gpumcd_set_source(ctx, w.source)
+        g.gpumcd_run_host(ctx, n, w.seed, dose)
+        c = g.gpumcd_get_counters(ctx)
+    assert c["ch_steps"] == ref["counters"]["ch_steps"]
+    np.testing.assert_allclose(dose, ref["dose"], rtol=1e-6, atol=0)
+
+
+def test_error_paths(workloads):
+    import torch
+
+    import paper_1101_1245_b200 as g
+
+    w = workloads[1]
+    dev = torch.device("cuda:0")
+    rho = torch.from_numpy(w.density).to(dev)
+    mat = torch.from_numpy(w.material).to(dev)
+    dose = torch.empty(rho.shape, dtype=torch.float32, device=dev)
+    with g.gpumcd_create(rho, mat, w.voxel_cm, w.tables) as ctx:
+        with pytest.raises(g.GpumcdError) as e:
+            g.gpumcd_run(ctx, 10, 1, dose)
+        assert e.value.status == -5                                   # no source yet
+        with pytest.raises(g.GpumcdError) as e:
+            g.gpumcd_set_source(ctx, Source(PHOTON, PENCIL, 8.25, 8.25, energy=25.0))
+        assert e.value.status == -6                                   # outside the tables
+        with pytest.raises(g.GpumcdError) as e:
+            g.gpumcd_set_source(ctx, Source(PHOTON, RECTANGLE, 1.0, 8.0, 4.0, 4.0, energy=2.0))
+        assert e.value.status == -1                                   # field sticks out of the phantom
+    bad = mat.clone()
+    bad[3, 3, 3] = 5
+    with pytest.raises(g.GpumcdError) as e:
+        g.gpumcd_create(rho, bad, w.voxel_cm, w.tables)
+    assert e.value.status == -1
+    neg = rho.clone()
+    neg[0, 0, 0] = 0.0
+    with pytest.raises(g.GpumcdError):
+        g.gpumcd_create(neg, mat, w.voxel_cm, w.tables)
+    # a queue that is too small must be reported, never silently dropped (PAPER.md L166 discards)
+    w2 = workloads[2]
+    rho2 = torch.from_numpy(w2.density).to(dev)
+    mat2 = torch.from_numpy(w2.material).to(dev)
+    dose2 = torch.empty(rho2.shape, dtype=torch.float32, device=dev)
+    with g.gpumcd_create(rho2, mat2, w2.voxel_cm, w2.tables, g.gpumcd_default_options(wave_size=20000, bank_factor=1)) as ctx:
+        g.gpumcd_set_source(ctx, w2.source)
+        with pytest.raises(g.GpumcdError) as e:
+            g.gpumcd_run(ctx, 20000, 1, dose2)
+            g.gpumcd_get_counters(ctx)
+        assert e.value.status == -4

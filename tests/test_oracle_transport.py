@@ -123,9 +123,9 @@ def test_csda_energy_loss_step_is_the_midpoint_rule(water_tables):
     r = oracle.run(rho, mat, h, tb, src, 1, seed=1)
     lnE = np.linspace(np.log(tb.e_min), np.log(tb.e_max), tb.n_energy)
     L = lambda t: np.interp(np.log(t), lnE, tb.electron[0, 0].astype(np.float64))
-    s = h * (1 + 1e-4)                                  # d_vox plus the boundary nudge
+    s = h * (1 + float(np.float32(1e-4)))               # d_vox plus the boundary nudge (float32 at the boundary)
     dE = s * L(T0 - 0.5 * L(T0) * s)
-    assert r.edep[0, 0, 0] == pytest.approx(dE, rel=1e-12)
+    assert r.edep[0, 0, 0] == pytest.approx(dE, rel=1e-7)
 
 
 # ------------------------------------------------------------------ S6
