@@ -80,8 +80,10 @@ typedef struct {
     uint32_t wave_size;    /* primaries generated per wave; default 2^20                           */
     uint32_t bank_factor;  /* queue capacity = bank_factor * wave_size records (the paper's d, L166);
                               default 8                                                            */
-    int32_t scheduler;     /* 0: one launch per pass, host reads the queue counts (L166);
-                              1: persistent cooperative kernel, no host round trips               */
+    int32_t scheduler;     /* 1 (default): one persistent cooperative kernel per run, lanes refilled,
+                              hard events sorted, no host round trips;
+                              0: the paper's scheme (L166): one launch per pass, one thread per
+                              particle, the host reads the queue counts between passes            */
     int32_t reserved;
 } gpumcd_options;
 

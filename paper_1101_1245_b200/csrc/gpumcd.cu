@@ -2,7 +2,7 @@
 //
 // See include/gpumcd.h for the boundary and DESIGN.md for the data layout and scheduling.
 #include "../../include/gpumcd.h"
-#include "transport.cuh"
+#include "persistent.cuh"
 
 #include <algorithm>
 #include <cmath>
@@ -43,52 +43,13 @@ __global__ void k_pack_phantom(const float *__restrict__ density, const uint8_t 
     if (threadIdx.x < 8 && s_max[threadIdx.x]) atomicMax(&rho_max_bits[threadIdx.x], s_max[threadIdx.x]);
 }
 
-struct SourceDev {
-    int particle, shape;
-    double cx, cy, wx, wy, energy;
-    int n_spec;
-    const double *cdf;   // n_spec+1, unnormalised running sum of the weights
-    const float *edges;  // n_spec+1
-};
-
 // H0: one primary per history from block (hist, track 0, ctr 0); transport starts at ctr 1.
 __global__ void k_source(Params P, SourceDev S, Queue q, unsigned long long hist0, unsigned n)
 {
     const unsigned i = blockIdx.x * blockDim.x + threadIdx.x;
     double e_inc = 0.0, e_cut = 0.0;
     if (i < n) {
-        const unsigned long long hist = hist0 + i;
-        Particle p;
-        p.hist = static_cast<uint32_t>(hist);
-        p.track = 0u;
-        p.ctr = 0u;
-        const uint4 w = draw(P.rng, p);
-        double x = S.cx, y = S.cy;
-        if (S.shape == 1) {
-            x = S.cx + (static_cast<double>(u01(w.x)) - 0.5) * S.wx;
-            y = S.cy + (static_cast<double>(u01(w.y)) - 0.5) * S.wy;
-        }
-        const double vx = x / static_cast<double>(P.geo.h), vy = y / static_cast<double>(P.geo.h);
-        const double fx = floor(vx), fy = floor(vy);
-        p.ix = static_cast<int>(fx);
-        p.iy = static_cast<int>(fy);
-        p.iz = 0;
-        p.fx = static_cast<float>(vx - fx);
-        p.fy = static_cast<float>(vy - fy);
-        p.fz = 0.0f;
-        p.u = 0.0f; p.v = 0.0f; p.w = 1.0f;
-        double E = S.energy;
-        if (S.n_spec > 0) {
-            const double target = static_cast<double>(u01(w.z)) * S.cdf[S.n_spec];
-            int lo = 0, hi = S.n_spec - 1; // largest j with cdf[j] <= target, clamped to n_spec-1
-            while (lo < hi) {
-                const int mid = (lo + hi + 1) >> 1;
-                if (S.cdf[mid] <= target) lo = mid; else hi = mid - 1;
-            }
-            const double e0 = S.edges[lo], e1 = S.edges[lo + 1];
-            E = e0 + static_cast<double>(u01(w.w)) * (e1 - e0);
-        }
-        p.E = static_cast<float>(E);
+        Particle p = make_primary(P, S, hist0 + i);
         e_inc = static_cast<double>(p.E);
         if (S.particle == 1 && !electron_tracked(P, p.E)) {
             // an electron below the cutoff (or photon_only): deposited where it is born
@@ -183,6 +144,14 @@ struct gpumcd_ctx {
     unsigned qcap = 0;
     double *spec_cdf = nullptr;
     float *spec_edges = nullptr;
+    // scheduler 1 (persistent kernel)
+    unsigned *heads = nullptr;      // 4 pop heads
+    float4 *privA = nullptr, *privB = nullptr;
+    uint4 *privC = nullptr;
+    unsigned priv_ready = 0;        // ready-stack capacity per warp
+    int p_grid = 0;                 // CTAs of the persistent kernel (one per SM)
+    bool smem_tables = false;
+    unsigned table_floats = 0;
     // host state
     Tables tab{};
     bool have_source = false;
@@ -251,7 +220,7 @@ extern "C" int gpumcd_default_options(gpumcd_options *opt)
     opt->majorant_scale = 1.0f;
     opt->wave_size = 1u << 20;
     opt->bank_factor = 8;
-    opt->scheduler = 0;
+    opt->scheduler = 1;
     opt->reserved = 0;
     return GPUMCD_OK;
 }
@@ -267,6 +236,8 @@ static void destroy_impl(gpumcd_ctx *c)
     for (int k = 0; k < 4; ++k) { cudaFree(c->qA[k]); cudaFree(c->qB[k]); cudaFree(c->qC[k]); }
     cudaFree(c->spec_cdf);
     cudaFree(c->spec_edges);
+    cudaFree(c->heads);
+    cudaFree(c->privA); cudaFree(c->privB); cudaFree(c->privC);
     for (auto &e : c->events) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
     delete c;
 }
@@ -343,7 +314,8 @@ static int create_impl(gpumcd_ctx **out, const float *density, const uint8_t *ma
     // H10 majorants: mu_max(E_i) = max_m rho_max[m] mu_m(E_i) (Eq. 3); M_e = running max in E of
     // max_m rho_max[m] (Sigma_Moller + Sigma_brems) (L110-113 made rigorous).
     const size_t n_ph = static_cast<size_t>(nM) * 3 * nE, n_el = static_cast<size_t>(nM) * 4 * nE;
-    std::vector<float> blob(n_ph + n_el + 2 * static_cast<size_t>(nE) + nK);
+    const size_t blob_len = n_ph + n_el + 2 * static_cast<size_t>(nE) + nK;
+    std::vector<float> blob((blob_len + 3) & ~static_cast<size_t>(3), 0.0f); // padded for 16-byte bulk copies
     memcpy(blob.data(), t->photon, n_ph * sizeof(float));
     memcpy(blob.data() + n_ph, t->electron, n_el * sizeof(float));
     float *mu_max = blob.data() + n_ph + n_el, *m_e = mu_max + nE;
@@ -364,11 +336,11 @@ static int create_impl(gpumcd_ctx **out, const float *density, const uint8_t *ma
     CK(cudaMalloc(&ctx->table_blob, blob.size() * sizeof(float)));
     CK(cudaMemcpy(ctx->table_blob, blob.data(), blob.size() * sizeof(float), cudaMemcpyHostToDevice));
     Tables &tb = ctx->tab;
-    tb.ph = ctx->table_blob;
-    tb.el = tb.ph + n_ph;
-    tb.mu_max = tb.el + n_el;
-    tb.m_e = tb.mu_max + nE;
-    tb.ms_a = tb.m_e + nE;
+    tb.blob = ctx->table_blob;
+    tb.off_el = static_cast<unsigned>(n_ph);
+    tb.off_mu = static_cast<unsigned>(n_ph + n_el);
+    tb.off_me = tb.off_mu + nE;
+    tb.off_ms = tb.off_me + nE;
     tb.gE.n = nE;
     tb.gE.x_min = static_cast<float>(std::log(static_cast<double>(t->e_min)));
     tb.gE.inv_dx = static_cast<float>((nE - 1) / (std::log(static_cast<double>(t->e_max)) - std::log(static_cast<double>(t->e_min))));
@@ -378,6 +350,7 @@ static int create_impl(gpumcd_ctx **out, const float *density, const uint8_t *ma
     tb.e_min = t->e_min; tb.e_cut = t->e_cut; tb.p_cut = t->p_cut;
     ctx->e_max = t->e_max;
     tb.n_mat = nM;
+    ctx->table_floats = static_cast<unsigned>(blob.size());
 
     // ---- tally, counters, queues ----
     CK(cudaMalloc(&ctx->edep, nvox * sizeof(double)));
@@ -388,6 +361,35 @@ static int create_impl(gpumcd_ctx **out, const float *density, const uint8_t *ma
         CK(cudaMalloc(&ctx->qA[k], static_cast<size_t>(ctx->qcap) * sizeof(float4)));
         CK(cudaMalloc(&ctx->qB[k], static_cast<size_t>(ctx->qcap) * sizeof(float4)));
         CK(cudaMalloc(&ctx->qC[k], static_cast<size_t>(ctx->qcap) * sizeof(uint4)));
+    }
+    if (opt.scheduler == 1) {
+        int dev = 0, n_sm = 0, coop = 0, max_smem = 0;
+        CK(cudaGetDevice(&dev));
+        CK(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
+        CK(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev));
+        CK(cudaDeviceGetAttribute(&max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+        if (!coop) { set_error(ctx, "device does not support cooperative launches (scheduler 1)"); return GPUMCD_ERR_CUDA; }
+        const size_t table_bytes = static_cast<size_t>(ctx->table_floats) * sizeof(float);
+        ctx->smem_tables = table_bytes + 2048 <= static_cast<size_t>(max_smem);
+        const size_t dyn = ctx->smem_tables ? table_bytes : 0;
+        if (ctx->smem_tables) {
+            CK(cudaFuncSetAttribute(k_persistent<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(dyn)));
+            CK(cudaFuncSetAttribute(k_persistent<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(dyn)));
+        }
+        int per_sm = 0;
+        if (ctx->smem_tables)
+            CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_persistent<false, true>, kPThreads, dyn));
+        else
+            CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_persistent<false, false>, kPThreads, 0));
+        if (per_sm < 1) { set_error(ctx, "persistent kernel does not fit on an SM"); return GPUMCD_ERR_CUDA; }
+        ctx->p_grid = n_sm; // one CTA per SM
+        ctx->priv_ready = 1024;
+        const size_t n_warps = static_cast<size_t>(ctx->p_grid) * (kPThreads / 32);
+        const size_t recs = n_warps * (ctx->priv_ready + kHardCap);
+        CK(cudaMalloc(&ctx->privA, recs * sizeof(float4)));
+        CK(cudaMalloc(&ctx->privB, recs * sizeof(float4)));
+        CK(cudaMalloc(&ctx->privC, recs * sizeof(uint4)));
+        CK(cudaMalloc(&ctx->heads, 4 * sizeof(unsigned)));
     }
     CK(cudaDeviceSynchronize());
     guard.ok = true;
@@ -537,6 +539,46 @@ static int run_waves_host_loop(gpumcd_ctx *ctx, uint64_t n_hist, uint64_t seed, 
     return GPUMCD_OK;
 }
 
+// Scheduler 1: the whole run is one cooperative launch (split only where the history id crosses 2^32).
+static int run_persistent(gpumcd_ctx *ctx, uint64_t n_hist, uint64_t seed, float *dose_dev, unsigned long long *trace,
+                          cudaStream_t st)
+{
+    CK(cudaMemsetAsync(ctx->qcount, 0, 4 * sizeof(unsigned), st));
+    CK(cudaMemsetAsync(ctx->heads, 0, 4 * sizeof(unsigned), st));
+    const double h3 = static_cast<double>(ctx->h) * ctx->h * ctx->h;
+    uint64_t h0 = ctx->hist_offset;
+    const uint64_t h_end = ctx->hist_offset + n_hist;
+    while (h0 < h_end) {
+        const uint64_t n = std::min<uint64_t>(h_end - h0, 0x100000000ull - (h0 & 0xffffffffull));
+        PersistArgs a{};
+        a.P = make_params(ctx, seed, static_cast<uint32_t>(h0 >> 32), trace != nullptr, trace);
+        a.S = ctx->src;
+        a.qP[0] = make_queue(ctx, 0);
+        a.qP[1] = make_queue(ctx, 1);
+        a.qE = make_queue(ctx, 2);
+        a.heads = ctx->heads;
+        a.privA = ctx->privA; a.privB = ctx->privB; a.privC = ctx->privC;
+        a.priv_ready = ctx->priv_ready;
+        a.hist0 = h0;
+        a.n_hist = n;
+        a.wave = ctx->opt.wave_size;
+        a.table_floats = ctx->table_floats;
+        a.inv_h3_n = 1.0 / (h3 * static_cast<double>(n_hist));
+        a.dose = dose_dev;
+        a.nvox = ctx->nvox;
+        a.finalize = (h0 + n == h_end) ? 1 : 0;
+        void *args[] = {&a};
+        const void *fn;
+        if (ctx->smem_tables) fn = trace ? (const void *)k_persistent<true, true> : (const void *)k_persistent<false, true>;
+        else fn = trace ? (const void *)k_persistent<true, false> : (const void *)k_persistent<false, false>;
+        const size_t dyn = ctx->smem_tables ? static_cast<size_t>(ctx->table_floats) * sizeof(float) : 0;
+        { LaunchScope ls(ctx, st, CLS_ELECTRON);
+        CK(cudaLaunchCooperativeKernel(fn, dim3(ctx->p_grid), dim3(kPThreads), args, dyn, st)); }
+        h0 += n;
+    }
+    return GPUMCD_OK;
+}
+
 static int run_impl(gpumcd_ctx *ctx, uint64_t n_hist, uint64_t seed, float *dose_dev, unsigned long long *trace_dev,
                     cudaStream_t st)
 {
@@ -553,6 +595,7 @@ static int run_impl(gpumcd_ctx *ctx, uint64_t n_hist, uint64_t seed, float *dose
     CK(cudaMemsetAsync(ctx->edep, 0, ctx->nvox * sizeof(double), st));
     CK(cudaMemsetAsync(ctx->cnt, 0, sizeof(DevCounters), st));
     if (trace_dev) CK(cudaMemsetAsync(trace_dev, 0, n_hist * sizeof(unsigned long long), st));
+    if (ctx->opt.scheduler == 1) return run_persistent(ctx, n_hist, seed, dose_dev, trace_dev, st);
     const int rc = run_waves_host_loop(ctx, n_hist, seed, trace_dev != nullptr, trace_dev, st);
     if (rc != GPUMCD_OK) return rc;
     const double h3 = static_cast<double>(ctx->h) * ctx->h * ctx->h;

@@ -1,0 +1,407 @@
+// persistent.cuh -- scheduler 1: one persistent cooperative kernel per gpumcd_run (H7).
+//
+// The paper alternates one launch per particle type until both lists are empty
+// and reports small gains from stream compaction and a persistent "pool" (L180-182, Tab. VI).
+// On B200 the transport kernels are issue-bound with most lanes idle (profiles/r01_*), so the
+// scheduler is built around keeping all 32 lanes of a warp in the SAME code:
+//   * one CTA per SM stays resident for the whole run; tables are staged into shared memory once
+//     with TMA bulk copies (cp.async.bulk + mbarrier);
+//   * a warp steps 32 particles in lock step and refills finished lanes at once, first from its
+//     private stack of same-type secondaries, then from the phase's input queue (atomic head);
+//   * electrons whose step ended on a hard-event candidate are swapped out into a per-warp buffer
+//     and processed 32 at a time (event-based sorting), so neither the step code nor the
+//     Moller / bremsstrahlung samplers run with a handful of active lanes;
+//   * photons born in an electron phase and electrons born in a photon phase go to global queues
+//     (ballot + popc prefix, one atomic per warp) that the next phase consumes; phases are separated
+//     by grid-wide barriers, so a queue is never read and written at the same time.
+#pragma once
+
+#include <cooperative_groups.h>
+
+#include "transport.cuh"
+
+namespace gpumcd {
+
+namespace cg = cooperative_groups;
+
+constexpr int kPThreads = 512;    // threads per persistent CTA (one CTA per SM)
+constexpr unsigned kHardCap = 64; // per-warp buffer of pending hard events
+constexpr unsigned kFull = 0xffffffffu;
+
+struct SourceDev {
+    int particle, shape;
+    double cx, cy, wx, wy, energy;
+    int n_spec;
+    const double *cdf;  // n_spec+1, unnormalised running sum of the weights
+    const float *edges; // n_spec+1
+};
+
+// H0: primary of one history from block (hist, track 0, ctr 0); transport starts at ctr 1.
+__device__ __forceinline__ Particle make_primary(const Params &P, const SourceDev &S, unsigned long long hist)
+{
+    Particle p;
+    p.hist = static_cast<uint32_t>(hist);
+    p.track = 0u;
+    p.ctr = 0u;
+    const uint4 w = draw(P.rng, p);
+    double x = S.cx, y = S.cy;
+    if (S.shape == 1) {
+        x = S.cx + (static_cast<double>(u01(w.x)) - 0.5) * S.wx;
+        y = S.cy + (static_cast<double>(u01(w.y)) - 0.5) * S.wy;
+    }
+    const double vx = x / static_cast<double>(P.geo.h), vy = y / static_cast<double>(P.geo.h);
+    const double fx = floor(vx), fy = floor(vy);
+    p.ix = static_cast<int>(fx);
+    p.iy = static_cast<int>(fy);
+    p.iz = 0;
+    p.fx = static_cast<float>(vx - fx);
+    p.fy = static_cast<float>(vy - fy);
+    p.fz = 0.0f;
+    p.u = 0.0f; p.v = 0.0f; p.w = 1.0f;
+    double E = S.energy;
+    if (S.n_spec > 0) {
+        const double target = static_cast<double>(u01(w.z)) * S.cdf[S.n_spec];
+        int lo = 0, hi = S.n_spec - 1; // largest j with cdf[j] <= target, clamped to n_spec-1
+        while (lo < hi) {
+            const int mid = (lo + hi + 1) >> 1;
+            if (S.cdf[mid] <= target) lo = mid; else hi = mid - 1;
+        }
+        const double e0 = S.edges[lo], e1 = S.edges[lo + 1];
+        E = e0 + static_cast<double>(u01(w.w)) * (e1 - e0);
+    }
+    p.E = static_cast<float>(E);
+    return p;
+}
+
+// ---- TMA bulk copy of the table blob into shared memory (G7) --------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void *p)
+{
+    return static_cast<uint32_t>(__cvta_generic_to_shared(p));
+}
+__device__ __forceinline__ void stage_tables(float *dst, const float *src, unsigned n_floats, uint64_t *bar)
+{
+    const uint32_t bar_a = smem_u32(bar);
+    if (threadIdx.x == 0) {
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bar_a));
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        const unsigned bytes = n_floats * 4u; // multiple of 16 (blob is padded)
+        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar_a), "r"(bytes) : "memory");
+        unsigned off = 0;
+        while (off < bytes) {
+            const unsigned chunk = min(bytes - off, 32768u);
+            asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::
+                             "r"(smem_u32(reinterpret_cast<const char *>(dst) + off)),
+                         "l"(reinterpret_cast<const char *>(src) + off), "r"(chunk), "r"(bar_a)
+                         : "memory");
+            off += chunk;
+        }
+    }
+    unsigned done = 0;
+    while (!done) {
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], 0;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                     : "=r"(done)
+                     : "r"(bar_a)
+                     : "memory");
+    }
+}
+
+// ---- records in arbitrary arrays --------------------------------------------------------------
+__device__ __forceinline__ void store_rec(float4 *A, float4 *B, uint4 *C, size_t i, const Particle &c, uint32_t extra)
+{
+    A[i] = make_float4(c.fx, c.fy, c.fz, c.E);
+    B[i] = make_float4(c.u, c.v, c.w, __uint_as_float(pack_voxel(c.ix, c.iy, c.iz)));
+    C[i] = make_uint4(c.hist, c.track, c.ctr, extra);
+}
+__device__ __forceinline__ Particle load_rec(const float4 *A, const float4 *B, const uint4 *C, size_t i, uint32_t &extra)
+{
+    const float4 a = A[i];
+    const float4 b = B[i];
+    const uint4 c = C[i];
+    Particle p;
+    p.fx = a.x; p.fy = a.y; p.fz = a.z; p.E = a.w;
+    p.u = b.x; p.v = b.y; p.w = b.z;
+    const uint32_t vox = __float_as_uint(b.w);
+    p.ix = vox & 1023u; p.iy = (vox >> 10) & 1023u; p.iz = vox >> 20;
+    p.hist = c.x; p.track = c.y; p.ctr = c.z;
+    extra = c.w;
+    return p;
+}
+
+struct PersistArgs {
+    Params P;
+    SourceDev S;
+    Queue qP[2];       // photon queues, alternating by phase
+    Queue qE;          // electron queue (filled by photon phases, drained by electron phases)
+    unsigned *heads;   // pop heads: [0],[1] photon queues, [2] electron queue, [3] source
+    float4 *privA;     // per-warp private records: ready stack [priv_ready] then hard buffer [kHardCap]
+    float4 *privB;
+    uint4 *privC;
+    unsigned priv_ready;           // capacity of a warp's ready stack
+    unsigned long long hist0;      // first history of the run (low word never wraps inside a launch)
+    unsigned long long n_hist;
+    unsigned wave;
+    unsigned table_floats;         // length of the table blob, padded to a multiple of 4 floats
+    double inv_h3_n;
+    float *dose;                   // or nullptr
+    size_t nvox;
+    int finalize;                  // 0 for all but the last launch of a run split at a 2^32 history boundary
+};
+
+// ---------------------------------------------------------------------------------------------
+// Photon phase: every warp steps 32 photons; finished lanes are refilled from the input.
+// SRC: the input is the source itself (primaries generated on the fly), else queue `in`.
+// ---------------------------------------------------------------------------------------------
+template <bool TRACE, bool SRC>
+__device__ void photon_phase(const Params &P, const float *__restrict__ TB, const SourceDev &S,
+                             unsigned long long hist_base, const Queue &in, unsigned n_in, unsigned *head,
+                             const Queue &qE, const Queue &qG)
+{
+    Local L; // flushed at the end of the phase, so its registers are free in the other phase
+    const int lane = threadIdx.x & 31;
+    const unsigned lt = (1u << lane) - 1u;
+    Particle p;
+    Trace tr;
+    bool alive = false, exhausted = (n_in == 0);
+    for (;;) {
+        const unsigned dead = __ballot_sync(kFull, !alive);
+        const int k = __popc(dead);
+        if (!exhausted && (k >= 8 || dead == kFull)) {
+            unsigned base = 0;
+            if (lane == 0) base = atomicAdd(head, static_cast<unsigned>(k));
+            base = __shfl_sync(kFull, base, 0);
+            const unsigned idx = base + __popc(dead & lt);
+            if (!alive && idx < n_in) {
+                uint32_t extra;
+                if (SRC) {
+                    p = make_primary(P, S, hist_base + idx);
+                    L.e_inc += static_cast<double>(p.E);
+                } else {
+                    p = load_rec(in.A, in.B, in.C, idx, extra);
+                }
+                alive = true;
+                tr = Trace{};
+            }
+            if (base + k >= n_in) exhausted = true;
+        }
+        if (__ballot_sync(kFull, alive) == 0u) {
+            if (exhausted) break;
+            continue;
+        }
+        if (alive) {
+            if (!photon_step<TRACE>(P, TB, p, L, qE, qG, tr)) {
+                write_trace<TRACE>(P, p, tr);
+                alive = false;
+            }
+        }
+    }
+    flush(P, L);
+}
+
+// ---------------------------------------------------------------------------------------------
+// Electron phase: lock-step condensed-history steps with lane refill and event-sorted hard events.
+// ---------------------------------------------------------------------------------------------
+template <bool SRC>
+__device__ void electron_phase(const Params &P, const float *__restrict__ TB, const SourceDev &S,
+                               unsigned long long hist_base, const Queue &in, unsigned n_in, unsigned *head,
+                               const Queue &qG, float4 *pA, float4 *pB, uint4 *pC, unsigned ready_cap)
+{
+    Local L;
+    const int lane = threadIdx.x & 31;
+    const unsigned lt = (1u << lane) - 1u;
+    // private records of this warp: [0, ready_cap) ready stack, [ready_cap, ready_cap + kHardCap) hard buffer
+    float4 *hA = pA + ready_cap, *hB = pB + ready_cap;
+    uint4 *hC = pC + ready_cap;
+    Particle p;
+    float lnT = 0.f, M = 0.f;
+    bool alive = false, exhausted = (n_in == 0);
+    unsigned n_ready = 0, n_hard = 0;
+    for (;;) {
+        // ---- refill dead lanes: private stack first, then the phase input
+        const unsigned dead = __ballot_sync(kFull, !alive);
+        if (dead) {
+            const unsigned k = __popc(dead), rank = __popc(dead & lt);
+            const unsigned take = min(k, n_ready);
+            if (!alive && rank < take) {
+                uint32_t extra;
+                p = load_rec(pA, pB, pC, n_ready - 1u - rank, extra);
+                lnT = logf(p.E);
+                alive = true;
+            }
+            n_ready -= take;
+            const unsigned want = k - take;
+            if (want > 0 && !exhausted && (want >= 8 || take + want == 32u)) {
+                unsigned base = 0;
+                if (lane == 0) base = atomicAdd(head, want);
+                base = __shfl_sync(kFull, base, 0);
+                const unsigned idx = base + rank - take;
+                if (!alive && rank >= take && idx < n_in) {
+                    uint32_t extra;
+                    if (SRC) {
+                        p = make_primary(P, S, hist_base + idx);
+                        L.e_inc += static_cast<double>(p.E);
+                        if (electron_tracked(P, p.E)) {
+                            alive = true;
+                        } else { // below the cutoff (or photon_only): deposited where it is born
+                            deposit(P, voxel_index(P.geo, p), p.E);
+                            L.e_cut += static_cast<double>(p.E);
+                        }
+                    } else {
+                        p = load_rec(in.A, in.B, in.C, idx, extra);
+                        alive = true;
+                    }
+                    lnT = logf(p.E);
+                }
+                if (base + want >= n_in) exhausted = true;
+            }
+        }
+        const unsigned am = __ballot_sync(kFull, alive);
+        // ---- hard events, 32 at a time (or whatever is left when nothing else can run)
+        if (n_hard >= 32u || (n_hard > 0u && am == 0u && n_ready == 0u && exhausted)) {
+            const unsigned nb = min(32u, n_hard);
+            Particle q, c;
+            int st = ST_DEAD, ct = 0;
+            if (static_cast<unsigned>(lane) < nb) {
+                uint32_t mbits;
+                q = load_rec(hA, hB, hC, n_hard - 1u - lane, mbits);
+                float qlnT = logf(q.E);
+                st = electron_hard(P, TB, q, qlnT, __uint_as_float(mbits), L, c, ct);
+            }
+            n_hard -= nb;
+            // bremsstrahlung photons -> global photon queue of the next photon phase
+            const unsigned gm = __ballot_sync(kFull, ct == 2);
+            if (gm) {
+                unsigned base = 0;
+                if (lane == 0) base = atomicAdd(qG.count, static_cast<unsigned>(__popc(gm)));
+                base = __shfl_sync(kFull, base, 0);
+                if (ct == 2) {
+                    const unsigned slot = base + __popc(gm & lt);
+                    if (slot < qG.cap) store_rec(qG.A, qG.B, qG.C, slot, c, 0u);
+                    else atomicAdd(&P.cnt->overflow, 1ull);
+                }
+            }
+            // knock-on electrons and the surviving primaries -> this warp's ready stack
+            const unsigned em = __ballot_sync(kFull, ct == 1);
+            if (ct == 1) {
+                const unsigned slot = n_ready + __popc(em & lt);
+                if (slot < ready_cap) store_rec(pA, pB, pC, slot, c, 0u);
+                else atomicAdd(&P.cnt->overflow, 1ull);
+            }
+            n_ready = min(n_ready + __popc(em), ready_cap);
+            const bool cont = (static_cast<unsigned>(lane) < nb) && st == ST_ALIVE;
+            const unsigned cm = __ballot_sync(kFull, cont);
+            if (cont) {
+                const unsigned slot = n_ready + __popc(cm & lt);
+                if (slot < ready_cap) store_rec(pA, pB, pC, slot, q, 0u);
+                else atomicAdd(&P.cnt->overflow, 1ull);
+            }
+            n_ready = min(n_ready + __popc(cm), ready_cap);
+            __syncwarp();
+            continue;
+        }
+        if (am == 0u) {
+            if (exhausted && n_ready == 0u) break;
+            continue;
+        }
+        // ---- one condensed-history step for every live lane
+        int st = ST_ALIVE;
+        if (alive) st = electron_step(P, TB, p, lnT, M, L);
+        const bool hard = alive && st == ST_HARD;
+        const unsigned hm = __ballot_sync(kFull, hard);
+        if (hard) {
+            store_rec(hA, hB, hC, n_hard + __popc(hm & lt), p, __float_as_uint(M));
+            alive = false;
+        }
+        n_hard += __popc(hm);
+        if (st == ST_DEAD) alive = false;
+        __syncwarp();
+    }
+    flush(P, L);
+}
+
+// ---------------------------------------------------------------------------------------------
+// The persistent kernel
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ unsigned ld_volatile(const unsigned *p) { return *reinterpret_cast<const volatile unsigned *>(p); }
+
+template <bool TRACE, bool SMEM_TABLES>
+__global__ void __launch_bounds__(kPThreads, 1) k_persistent(const PersistArgs a)
+{
+    extern __shared__ __align__(128) float smem[];
+    __shared__ uint64_t bar;
+    cg::grid_group grid = cg::this_grid();
+
+    const Params &P = a.P;
+    const float *TB = P.tab.blob;
+    if (SMEM_TABLES) {
+        stage_tables(smem, P.tab.blob, a.table_floats, &bar);
+        TB = smem;
+    }
+    const unsigned gwarp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const size_t stride = static_cast<size_t>(a.priv_ready) + kHardCap;
+    float4 *pA = a.privA + gwarp * stride, *pB = a.privB + gwarp * stride;
+    uint4 *pC = a.privC + gwarp * stride;
+    const bool leader = (blockIdx.x == 0 && threadIdx.x == 0);
+
+    unsigned long long done = 0;
+    while (done < a.n_hist) {
+        const unsigned n = static_cast<unsigned>(min(static_cast<unsigned long long>(a.wave), a.n_hist - done));
+        const unsigned long long hist_base = a.hist0 + done;
+        // all queue counters and heads are zero here
+        int cur = 0;
+        unsigned nP = (a.S.particle == 0) ? n : 0u, nE = (a.S.particle == 1) ? n : 0u;
+        bool first = true;
+        for (;;) {
+            // ---- photon phase: reads qP[cur] (or the source), fills qE and qP[cur^1]
+            if (nP) {
+                if (first && a.S.particle == 0)
+                    photon_phase<TRACE, true>(P, TB, a.S, hist_base, a.qP[cur], nP, a.heads + 3, a.qE, a.qP[cur ^ 1]);
+                else
+                    photon_phase<TRACE, false>(P, TB, a.S, hist_base, a.qP[cur], nP, a.heads + cur, a.qE, a.qP[cur ^ 1]);
+            }
+            grid.sync();
+            if (leader) { *a.qP[cur].count = 0u; a.heads[cur] = 0u; a.heads[3] = 0u; }
+            if (!(first && a.S.particle == 1)) nE = min(ld_volatile(a.qE.count), a.qE.cap);
+            grid.sync();
+            // ---- electron phase: reads qE (or the source), fills qP[cur^1]; knock-ons stay in the warp
+            if (nE) {
+                if (first && a.S.particle == 1)
+                    electron_phase<true>(P, TB, a.S, hist_base, a.qE, nE, a.heads + 3, a.qP[cur ^ 1], pA, pB, pC, a.priv_ready);
+                else
+                    electron_phase<false>(P, TB, a.S, hist_base, a.qE, nE, a.heads + 2, a.qP[cur ^ 1], pA, pB, pC, a.priv_ready);
+            }
+            grid.sync();
+            if (leader) { *a.qE.count = 0u; a.heads[2] = 0u; a.heads[3] = 0u; }
+            cur ^= 1;
+            nP = min(ld_volatile(a.qP[cur].count), a.qP[cur].cap);
+            nE = 0u;
+            first = false;
+            grid.sync();
+            if (nP == 0u) break;
+        }
+        done += n;
+    }
+    if (!a.finalize) return;
+    grid.sync();
+    // ---- H8 finalize: dose = energy / mass / histories, and the total deposited energy
+    double s = 0.0;
+    for (size_t i = blockIdx.x * static_cast<size_t>(blockDim.x) + threadIdx.x; i < a.nvox;
+         i += static_cast<size_t>(gridDim.x) * blockDim.x) {
+        const double e = P.edep[i];
+        s += e;
+        if (a.dose) a.dose[i] = static_cast<float>(e / static_cast<double>(P.geo.phantom[i].x) * a.inv_h3_n);
+    }
+    s = wsum(s);
+    __shared__ double part[kPThreads / 32];
+    if ((threadIdx.x & 31) == 0) part[threadIdx.x >> 5] = s;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double t = 0.0;
+        for (int k = 0; k < kPThreads / 32; ++k) t += part[k];
+        atomicAdd(&P.cnt->e_dep_total, t);
+    }
+}
+
+} // namespace gpumcd

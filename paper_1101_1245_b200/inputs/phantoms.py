@@ -51,7 +51,7 @@ def ct_like(nx: int, ny: int, nz: int, voxel_cm: float, seed: int = 5, sigma_cm:
     ky = np.fft.fftfreq(ny, d=voxel_cm)[None, :, None]
     kx = np.fft.rfftfreq(nx, d=voxel_cm)[None, None, :]
     filt = np.exp(-2.0 * (np.pi * sigma_cm) ** 2 * (kx**2 + ky**2 + kz**2))
-    g = np.fft.irfftn(np.fft.rfftn(g) * filt, s=g.shape)
+    g = np.fft.irfftn(np.fft.rfftn(g, axes=(0, 1, 2)) * filt, s=g.shape, axes=(0, 1, 2))
     edges = np.quantile(g, np.cumsum(fractions)[:-1])
     mat = np.digitize(g, edges).astype(np.uint8)
     u = rng.uniform(-noise, noise, size=g.shape)
