@@ -47,26 +47,21 @@ __global__ void k_pack_phantom(const float *__restrict__ density, const uint8_t 
 __global__ void k_source(Params P, SourceDev S, Queue q, unsigned long long hist0, unsigned n)
 {
     const unsigned i = blockIdx.x * blockDim.x + threadIdx.x;
-    double e_inc = 0.0, e_cut = 0.0;
+    const Acc acc(P);
+    double e_inc = 0.0;
     if (i < n) {
         Particle p = make_primary(P, S, hist0 + i);
         e_inc = static_cast<double>(p.E);
         if (S.particle == 1 && !electron_tracked(P, p.E)) {
             // an electron below the cutoff (or photon_only): deposited where it is born
             deposit(P, voxel_index(P.geo, p), p.E);
-            e_cut = e_inc;
+            acc.cut(p.E);
             p.E = -1.0f; // marks an empty record
         }
-        q.A[i] = make_float4(p.fx, p.fy, p.fz, p.E);
-        q.B[i] = make_float4(p.u, p.v, p.w, __uint_as_float(pack_voxel(p.ix, p.iy, p.iz)));
-        q.C[i] = make_uint4(p.hist, p.track, p.ctr, 0u);
+        store_rec(q.A, q.B, q.C, i, p, 0u);
     }
     e_inc = wsum(e_inc);
-    e_cut = wsum(e_cut);
-    if ((threadIdx.x & 31) == 0) {
-        if (e_inc != 0.0) atomicAdd(&P.cnt->e_incident, e_inc);
-        if (e_cut != 0.0) atomicAdd(&P.cnt->e_dep_cutoff, e_cut);
-    }
+    if ((threadIdx.x & 31) == 0 && e_inc != 0.0) acc.inc(e_inc);
     if (i == 0) *q.count = n;
 }
 
@@ -80,7 +75,8 @@ __global__ void __launch_bounds__(kBlock) k_photon_pass(Params P, Queue in, unsi
     const unsigned i = blockIdx.x * blockDim.x + threadIdx.x;
     Local L;
     if (i < n_in) {
-        const Particle p = pop(in, i);
+        uint32_t extra;
+        const Particle p = load_rec(in.A, in.B, in.C, i, extra);
         if (p.E >= 0.0f) photon_run<TRACE>(P, p, L, qE, qG);
     }
     flush(P, L);
@@ -91,7 +87,8 @@ __global__ void __launch_bounds__(kBlock) k_electron_pass(Params P, Queue in, un
     const unsigned i = blockIdx.x * blockDim.x + threadIdx.x;
     Local L;
     if (i < n_in) {
-        const Particle p = pop(in, i);
+        uint32_t extra;
+        const Particle p = load_rec(in.A, in.B, in.C, i, extra);
         if (p.E >= 0.0f) electron_run(P, p, L, qE, qG);
     }
     flush(P, L);
@@ -653,11 +650,13 @@ extern "C" int gpumcd_get_counters(gpumcd_ctx *ctx, gpumcd_counters *out)
     out->hard_fict = d.hard_fict; out->pushes_e = d.pushes_e; out->pushes_g = d.pushes_g;
     out->bank_high_water = ctx->high_water;
     out->overflow_count = d.overflow;
-    out->e_incident = d.e_incident;
-    out->e_dep_cutoff = d.e_dep_cutoff;
-    out->e_dep_continuous = d.e_dep_total - d.e_dep_cutoff;
-    out->e_escaped = d.e_escaped;
-    out->e_pair_rest = d.e_pair_rest;
+    for (int k = 0; k < kEnergySlots; ++k) {
+        out->e_incident += d.slot[k].e_inc;
+        out->e_dep_cutoff += d.slot[k].e_cut;
+        out->e_escaped += d.slot[k].e_esc;
+        out->e_pair_rest += d.slot[k].e_pair;
+    }
+    out->e_dep_continuous = d.e_dep_total - out->e_dep_cutoff;
     if (d.overflow) { set_error(ctx, "particle queue overflow: the result is invalid"); return GPUMCD_ERR_BANK_OVERFLOW; }
     return GPUMCD_OK;
 }

@@ -24,7 +24,10 @@ namespace gpumcd {
 
 namespace cg = cooperative_groups;
 
-constexpr int kPThreads = 512;    // threads per persistent CTA (one CTA per SM)
+#ifndef GPUMCD_PTHREADS
+#define GPUMCD_PTHREADS 512
+#endif
+constexpr int kPThreads = GPUMCD_PTHREADS; // threads per persistent CTA (one CTA per SM)
 constexpr unsigned kHardCap = 64; // per-warp buffer of pending hard events
 constexpr unsigned kFull = 0xffffffffu;
 
@@ -108,28 +111,6 @@ __device__ __forceinline__ void stage_tables(float *dst, const float *src, unsig
     }
 }
 
-// ---- records in arbitrary arrays --------------------------------------------------------------
-__device__ __forceinline__ void store_rec(float4 *A, float4 *B, uint4 *C, size_t i, const Particle &c, uint32_t extra)
-{
-    A[i] = make_float4(c.fx, c.fy, c.fz, c.E);
-    B[i] = make_float4(c.u, c.v, c.w, __uint_as_float(pack_voxel(c.ix, c.iy, c.iz)));
-    C[i] = make_uint4(c.hist, c.track, c.ctr, extra);
-}
-__device__ __forceinline__ Particle load_rec(const float4 *A, const float4 *B, const uint4 *C, size_t i, uint32_t &extra)
-{
-    const float4 a = A[i];
-    const float4 b = B[i];
-    const uint4 c = C[i];
-    Particle p;
-    p.fx = a.x; p.fy = a.y; p.fz = a.z; p.E = a.w;
-    p.u = b.x; p.v = b.y; p.w = b.z;
-    const uint32_t vox = __float_as_uint(b.w);
-    p.ix = vox & 1023u; p.iy = (vox >> 10) & 1023u; p.iz = vox >> 20;
-    p.hist = c.x; p.track = c.y; p.ctr = c.z;
-    extra = c.w;
-    return p;
-}
-
 struct PersistArgs {
     Params P;
     SourceDev S;
@@ -153,18 +134,20 @@ struct PersistArgs {
 // ---------------------------------------------------------------------------------------------
 // Photon phase: every warp steps 32 photons; finished lanes are refilled from the input.
 // SRC: the input is the source itself (primaries generated on the fly), else queue `in`.
+// Event counts are warp-level (ballot + popc into warp-uniform counters): no per-lane registers.
 // ---------------------------------------------------------------------------------------------
 template <bool TRACE, bool SRC>
 __device__ void photon_phase(const Params &P, const float *__restrict__ TB, const SourceDev &S,
                              unsigned long long hist_base, const Queue &in, unsigned n_in, unsigned *head,
                              const Queue &qE, const Queue &qG)
 {
-    Local L; // flushed at the end of the phase, so its registers are free in the other phase
     const int lane = threadIdx.x & 31;
     const unsigned lt = (1u << lane) - 1u;
+    const Acc acc(P);
     Particle p;
     Trace tr;
     bool alive = false, exhausted = (n_in == 0);
+    unsigned n_flight = 0, n_compton = 0, n_photo = 0, n_pair = 0, n_fict = 0;
     for (;;) {
         const unsigned dead = __ballot_sync(kFull, !alive);
         const int k = __popc(dead);
@@ -173,31 +156,48 @@ __device__ void photon_phase(const Params &P, const float *__restrict__ TB, cons
             if (lane == 0) base = atomicAdd(head, static_cast<unsigned>(k));
             base = __shfl_sync(kFull, base, 0);
             const unsigned idx = base + __popc(dead & lt);
+            double e_new = 0.0;
             if (!alive && idx < n_in) {
                 uint32_t extra;
                 if (SRC) {
                     p = make_primary(P, S, hist_base + idx);
-                    L.e_inc += static_cast<double>(p.E);
+                    e_new = static_cast<double>(p.E);
                 } else {
                     p = load_rec(in.A, in.B, in.C, idx, extra);
                 }
                 alive = true;
                 tr = Trace{};
             }
+            if (SRC) {
+                e_new = wsum(e_new);
+                if (lane == 0 && e_new != 0.0) acc.inc(e_new);
+            }
             if (base + k >= n_in) exhausted = true;
         }
-        if (__ballot_sync(kFull, alive) == 0u) {
+        const unsigned am = __ballot_sync(kFull, alive);
+        if (am == 0u) {
             if (exhausted) break;
             continue;
         }
+        int ev = -1;
         if (alive) {
-            if (!photon_step<TRACE>(P, TB, p, L, qE, qG, tr)) {
+            ev = photon_step<TRACE>(P, TB, p, acc, qE, qG, tr);
+            if (!photon_alive(ev)) {
                 write_trace<TRACE>(P, p, tr);
                 alive = false;
             }
         }
+        n_flight += __popc(am);
+        n_compton += __popc(__ballot_sync(kFull, ev == PH_COMPTON || ev == PH_ABSORBED));
+        n_photo += __popc(__ballot_sync(kFull, ev == PH_PHOTO));
+        n_pair += __popc(__ballot_sync(kFull, ev == PH_PAIR));
+        n_fict += __popc(__ballot_sync(kFull, ev == PH_FICT));
     }
-    flush(P, L);
+    if (lane == 0) {
+        DevCounters *c = P.cnt;
+        bump(&c->photon_flights, n_flight); bump(&c->photon_compton, n_compton); bump(&c->photon_photo, n_photo);
+        bump(&c->photon_pair, n_pair); bump(&c->photon_fict, n_fict);
+    }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -208,16 +208,16 @@ __device__ void electron_phase(const Params &P, const float *__restrict__ TB, co
                                unsigned long long hist_base, const Queue &in, unsigned n_in, unsigned *head,
                                const Queue &qG, float4 *pA, float4 *pB, uint4 *pC, unsigned ready_cap)
 {
-    Local L;
     const int lane = threadIdx.x & 31;
     const unsigned lt = (1u << lane) - 1u;
-    // private records of this warp: [0, ready_cap) ready stack, [ready_cap, ready_cap + kHardCap) hard buffer
-    float4 *hA = pA + ready_cap, *hB = pB + ready_cap;
-    uint4 *hC = pC + ready_cap;
+    const Acc acc(P);
+    // private records of this warp: [0, ready_cap) ready stack (extra word = ln T),
+    // [ready_cap, ready_cap + kHardCap) pending hard events (extra word = majorant M)
     Particle p;
     float lnT = 0.f, M = 0.f;
     bool alive = false, exhausted = (n_in == 0);
     unsigned n_ready = 0, n_hard = 0;
+    unsigned n_step = 0, n_moller = 0, n_brems = 0, n_hfict = 0;
     for (;;) {
         // ---- refill dead lanes: private stack first, then the phase input
         const unsigned dead = __ballot_sync(kFull, !alive);
@@ -227,32 +227,37 @@ __device__ void electron_phase(const Params &P, const float *__restrict__ TB, co
             if (!alive && rank < take) {
                 uint32_t extra;
                 p = load_rec(pA, pB, pC, n_ready - 1u - rank, extra);
-                lnT = logf(p.E);
+                lnT = __uint_as_float(extra);
                 alive = true;
             }
             n_ready -= take;
             const unsigned want = k - take;
-            if (want > 0 && !exhausted && (want >= 8 || take + want == 32u)) {
+            if (want > 0 && !exhausted && (want >= 8 || k == 32u)) {
                 unsigned base = 0;
                 if (lane == 0) base = atomicAdd(head, want);
                 base = __shfl_sync(kFull, base, 0);
                 const unsigned idx = base + rank - take;
+                double e_new = 0.0;
                 if (!alive && rank >= take && idx < n_in) {
                     uint32_t extra;
                     if (SRC) {
                         p = make_primary(P, S, hist_base + idx);
-                        L.e_inc += static_cast<double>(p.E);
+                        e_new = static_cast<double>(p.E);
                         if (electron_tracked(P, p.E)) {
                             alive = true;
                         } else { // below the cutoff (or photon_only): deposited where it is born
                             deposit(P, voxel_index(P.geo, p), p.E);
-                            L.e_cut += static_cast<double>(p.E);
+                            acc.cut(p.E);
                         }
                     } else {
                         p = load_rec(in.A, in.B, in.C, idx, extra);
                         alive = true;
                     }
-                    lnT = logf(p.E);
+                    lnT = flog(p.E);
+                }
+                if (SRC) {
+                    e_new = wsum(e_new);
+                    if (lane == 0 && e_new != 0.0) acc.inc(e_new);
                 }
                 if (base + want >= n_in) exhausted = true;
             }
@@ -262,42 +267,46 @@ __device__ void electron_phase(const Params &P, const float *__restrict__ TB, co
         if (n_hard >= 32u || (n_hard > 0u && am == 0u && n_ready == 0u && exhausted)) {
             const unsigned nb = min(32u, n_hard);
             Particle q, c;
-            int st = ST_DEAD, ct = 0;
+            float qlnT = 0.f;
+            int st = ST_DEAD, kind = -1;
             if (static_cast<unsigned>(lane) < nb) {
                 uint32_t mbits;
-                q = load_rec(hA, hB, hC, n_hard - 1u - lane, mbits);
-                float qlnT = logf(q.E);
-                st = electron_hard(P, TB, q, qlnT, __uint_as_float(mbits), L, c, ct);
+                q = load_rec(pA, pB, pC, ready_cap + n_hard - 1u - lane, mbits);
+                qlnT = flog(q.E);
+                st = electron_hard(P, TB, q, qlnT, __uint_as_float(mbits), acc, c, kind);
             }
             n_hard -= nb;
             // bremsstrahlung photons -> global photon queue of the next photon phase
-            const unsigned gm = __ballot_sync(kFull, ct == 2);
+            const unsigned gm = __ballot_sync(kFull, kind == HK_BREMS);
             if (gm) {
                 unsigned base = 0;
                 if (lane == 0) base = atomicAdd(qG.count, static_cast<unsigned>(__popc(gm)));
                 base = __shfl_sync(kFull, base, 0);
-                if (ct == 2) {
+                if (kind == HK_BREMS) {
                     const unsigned slot = base + __popc(gm & lt);
                     if (slot < qG.cap) store_rec(qG.A, qG.B, qG.C, slot, c, 0u);
                     else atomicAdd(&P.cnt->overflow, 1ull);
                 }
             }
             // knock-on electrons and the surviving primaries -> this warp's ready stack
-            const unsigned em = __ballot_sync(kFull, ct == 1);
-            if (ct == 1) {
+            const unsigned em = __ballot_sync(kFull, kind == HK_MOLLER);
+            if (kind == HK_MOLLER) {
                 const unsigned slot = n_ready + __popc(em & lt);
-                if (slot < ready_cap) store_rec(pA, pB, pC, slot, c, 0u);
+                if (slot < ready_cap) store_rec(pA, pB, pC, slot, c, __float_as_uint(flog(c.E)));
                 else atomicAdd(&P.cnt->overflow, 1ull);
             }
             n_ready = min(n_ready + __popc(em), ready_cap);
-            const bool cont = (static_cast<unsigned>(lane) < nb) && st == ST_ALIVE;
+            const bool cont = (kind >= 0) && st == ST_ALIVE;
             const unsigned cm = __ballot_sync(kFull, cont);
             if (cont) {
                 const unsigned slot = n_ready + __popc(cm & lt);
-                if (slot < ready_cap) store_rec(pA, pB, pC, slot, q, 0u);
+                if (slot < ready_cap) store_rec(pA, pB, pC, slot, q, __float_as_uint(qlnT));
                 else atomicAdd(&P.cnt->overflow, 1ull);
             }
             n_ready = min(n_ready + __popc(cm), ready_cap);
+            n_moller += __popc(em);
+            n_brems += __popc(gm);
+            n_hfict += __popc(__ballot_sync(kFull, kind == HK_FICT));
             __syncwarp();
             continue;
         }
@@ -307,18 +316,23 @@ __device__ void electron_phase(const Params &P, const float *__restrict__ TB, co
         }
         // ---- one condensed-history step for every live lane
         int st = ST_ALIVE;
-        if (alive) st = electron_step(P, TB, p, lnT, M, L);
+        if (alive) st = electron_step(P, TB, p, lnT, M, acc);
+        n_step += __popc(am);
         const bool hard = alive && st == ST_HARD;
         const unsigned hm = __ballot_sync(kFull, hard);
         if (hard) {
-            store_rec(hA, hB, hC, n_hard + __popc(hm & lt), p, __float_as_uint(M));
+            store_rec(pA, pB, pC, ready_cap + n_hard + __popc(hm & lt), p, __float_as_uint(M));
             alive = false;
         }
         n_hard += __popc(hm);
         if (st == ST_DEAD) alive = false;
         __syncwarp();
     }
-    flush(P, L);
+    if (lane == 0) {
+        DevCounters *c = P.cnt;
+        bump(&c->ch_steps, n_step); bump(&c->hard_moller, n_moller); bump(&c->hard_brems, n_brems);
+        bump(&c->hard_fict, n_hfict); bump(&c->pushes_e, n_moller); bump(&c->pushes_g, n_brems);
+    }
 }
 
 // ---------------------------------------------------------------------------------------------

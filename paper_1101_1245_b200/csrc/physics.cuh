@@ -37,7 +37,45 @@ __device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_
 // U(w) = ((w >> 9) + 1/2) 2^-23 in (0,1); exact in fp32 (Eq. 1 needs zeta in (0,1], L53).
 __device__ __forceinline__ float u01(uint32_t w)
 {
-    return (static_cast<float>(w >> 9) + 0.5f) * (1.0f / 8388608.0f);
+    return fmaf(__uint2float_rz(w >> 9), 1.0f / 8388608.0f, 1.0f / 16777216.0f);
+}
+
+// ---------------------------------------------------------------------------------------------
+// Math policy.  The transport kernels are issue-bound, so the transcendental and division
+// sequences matter.  With GPUMCD_FAST_MATH (default) the step code uses the SFU forms
+// (MUFU.LG2 / MUFU.RCP / MUFU.SIN,COS): absolute errors of a few 1e-7, the same size as fp32
+// rounding of the quantities they feed.  -DGPUMCD_FAST_MATH=0 selects the IEEE library forms.
+// ---------------------------------------------------------------------------------------------
+#ifndef GPUMCD_FAST_MATH
+#define GPUMCD_FAST_MATH 1
+#endif
+__device__ __forceinline__ float flog(float x)
+{
+#if GPUMCD_FAST_MATH
+    return __logf(x);
+#else
+    return logf(x);
+#endif
+}
+__device__ __forceinline__ float fdiv(float a, float b)
+{
+#if GPUMCD_FAST_MATH
+    return __fdividef(a, b);
+#else
+    return a / b;
+#endif
+}
+// sin and cos of 2*pi*u, u in (0,1)
+__device__ __forceinline__ void sincos2pi(float u, float &s, float &c)
+{
+#if GPUMCD_FAST_MATH
+    // keep the SFU argument inside (-pi, pi), where its absolute error is 2^-21.4: u - 1/2 is exact
+    __sincosf(kTwoPi * (u - 0.5f), &s, &c);
+    s = -s;
+    c = -c;
+#else
+    sincospif(2.0f * u, &s, &c);
+#endif
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -97,12 +135,10 @@ __device__ __forceinline__ void advance(Particle &p, float t)
     p.fz -= cz;
 }
 
-// Rotate direction d by polar angle (cost, sint) and azimuth 2*pi*uphi about itself (R-P8).
-__device__ __forceinline__ void rotate(float u, float v, float w, float cost, float sint, float uphi,
-                                       float phase, float &ou, float &ov, float &ow)
+// Rotate direction d by polar angle (cost, sint) and azimuth (cp, sp) about itself (R-P8).
+__device__ __forceinline__ void rotate(float u, float v, float w, float cost, float sint, float cp, float sp,
+                                       float &ou, float &ov, float &ow)
 {
-    float sp, cp;
-    sincospif(2.0f * uphi + phase, &sp, &cp); // phase = 1 adds pi (opposite azimuth)
     const float r2 = fmaf(u, u, v * v);
     float a, b, c;
     if (r2 < 1e-10f) {
