@@ -702,3 +702,12 @@ extern "C" const char *gpumcd_last_error(gpumcd_ctx *ctx)
 }
 
 extern "C" void gpumcd_destroy(gpumcd_ctx *ctx) { destroy_impl(ctx); }
+
+#ifdef GPUMCD_TIMELINE
+// development aid (only with -DGPUMCD_TIMELINE): copy the phase timeline of the last persistent launch
+extern "C" int gpumcd_debug_timeline(void *host_out, size_t bytes)
+{
+    if (bytes < sizeof(Timeline)) return static_cast<int>(sizeof(Timeline));
+    return cudaMemcpyFromSymbol(host_out, g_timeline, sizeof(Timeline)) == cudaSuccess ? 0 : -2;
+}
+#endif

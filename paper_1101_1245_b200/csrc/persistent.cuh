@@ -30,6 +30,7 @@ namespace cg = cooperative_groups;
 constexpr int kPThreads = GPUMCD_PTHREADS; // threads per persistent CTA (one CTA per SM)
 constexpr unsigned kHardCap = 64; // per-warp buffer of pending hard events
 constexpr unsigned kFull = 0xffffffffu;
+constexpr unsigned kChunk = 32;   // inputs a warp claims per atomic on the phase's head counter
 
 struct SourceDev {
     int particle, shape;
@@ -138,8 +139,8 @@ struct PersistArgs {
 // ---------------------------------------------------------------------------------------------
 template <bool TRACE, bool SRC>
 __device__ void photon_phase(const Params &P, const float *__restrict__ TB, const SourceDev &S,
-                             unsigned long long hist_base, const Queue &in, unsigned n_in, unsigned *head,
-                             const Queue &qE, const Queue &qG)
+                             unsigned long long hist_base, const Queue &in, unsigned n_queue, unsigned n_in,
+                             unsigned *head, const Queue &qE, const Queue &qG)
 {
     const int lane = threadIdx.x & 31;
     const unsigned lt = (1u << lane) - 1u;
@@ -148,19 +149,26 @@ __device__ void photon_phase(const Params &P, const float *__restrict__ TB, cons
     Trace tr;
     bool alive = false, exhausted = (n_in == 0);
     unsigned n_flight = 0, n_compton = 0, n_photo = 0, n_pair = 0, n_fict = 0;
+    unsigned w_next = 0, w_end = 0; // this warp's chunk of the input, [w_next, w_end)
     for (;;) {
         const unsigned dead = __ballot_sync(kFull, !alive);
-        const int k = __popc(dead);
-        if (!exhausted && (k >= 8 || dead == kFull)) {
-            unsigned base = 0;
-            if (lane == 0) base = atomicAdd(head, static_cast<unsigned>(k));
-            base = __shfl_sync(kFull, base, 0);
-            const unsigned idx = base + __popc(dead & lt);
+        if (dead && !(exhausted && w_next == w_end)) {
+            if (w_next == w_end) { // take the next chunk of kChunk inputs: one atomic per chunk
+                unsigned base = 0;
+                if (lane == 0) base = atomicAdd(head, kChunk);
+                base = __shfl_sync(kFull, base, 0);
+                w_next = min(base, n_in);
+                w_end = min(base + kChunk, n_in);
+                if (base + kChunk >= n_in) exhausted = true;
+            }
+            const unsigned take = min(static_cast<unsigned>(__popc(dead)), w_end - w_next);
+            const unsigned rank = __popc(dead & lt);
             double e_new = 0.0;
-            if (!alive && idx < n_in) {
+            if (!alive && rank < take) {
+                const unsigned idx = w_next + rank;
                 uint32_t extra;
-                if (SRC) {
-                    p = make_primary(P, S, hist_base + idx);
+                if (SRC && idx >= n_queue) {
+                    p = make_primary(P, S, hist_base + (idx - n_queue));
                     e_new = static_cast<double>(p.E);
                 } else {
                     p = load_rec(in.A, in.B, in.C, idx, extra);
@@ -168,15 +176,15 @@ __device__ void photon_phase(const Params &P, const float *__restrict__ TB, cons
                 alive = true;
                 tr = Trace{};
             }
+            w_next += take;
             if (SRC) {
                 e_new = wsum(e_new);
                 if (lane == 0 && e_new != 0.0) acc.inc(e_new);
             }
-            if (base + k >= n_in) exhausted = true;
         }
         const unsigned am = __ballot_sync(kFull, alive);
         if (am == 0u) {
-            if (exhausted) break;
+            if (exhausted && w_next == w_end) break;
             continue;
         }
         int ev = -1;
@@ -205,8 +213,9 @@ __device__ void photon_phase(const Params &P, const float *__restrict__ TB, cons
 // ---------------------------------------------------------------------------------------------
 template <bool SRC>
 __device__ void electron_phase(const Params &P, const float *__restrict__ TB, const SourceDev &S,
-                               unsigned long long hist_base, const Queue &in, unsigned n_in, unsigned *head,
-                               const Queue &qG, float4 *pA, float4 *pB, uint4 *pC, unsigned ready_cap)
+                               unsigned long long hist_base, const Queue &in, unsigned n_queue, unsigned n_in,
+                               unsigned *head, const Queue &qG, float4 *pA, float4 *pB, uint4 *pC,
+                               unsigned ready_cap)
 {
     const int lane = threadIdx.x & 31;
     const unsigned lt = (1u << lane) - 1u;
@@ -218,6 +227,7 @@ __device__ void electron_phase(const Params &P, const float *__restrict__ TB, co
     bool alive = false, exhausted = (n_in == 0);
     unsigned n_ready = 0, n_hard = 0;
     unsigned n_step = 0, n_moller = 0, n_brems = 0, n_hfict = 0;
+    unsigned w_next = 0, w_end = 0; // this warp's chunk of the input, [w_next, w_end)
     for (;;) {
         // ---- refill dead lanes: private stack first, then the phase input
         const unsigned dead = __ballot_sync(kFull, !alive);
@@ -231,17 +241,22 @@ __device__ void electron_phase(const Params &P, const float *__restrict__ TB, co
                 alive = true;
             }
             n_ready -= take;
-            const unsigned want = k - take;
-            if (want > 0 && !exhausted && (want >= 8 || k == 32u)) {
-                unsigned base = 0;
-                if (lane == 0) base = atomicAdd(head, want);
-                base = __shfl_sync(kFull, base, 0);
-                const unsigned idx = base + rank - take;
+            if (k > take && !(exhausted && w_next == w_end)) {
+                if (w_next == w_end) { // next chunk of the input: one atomic per kChunk particles
+                    unsigned base = 0;
+                    if (lane == 0) base = atomicAdd(head, kChunk);
+                    base = __shfl_sync(kFull, base, 0);
+                    w_next = min(base, n_in);
+                    w_end = min(base + kChunk, n_in);
+                    if (base + kChunk >= n_in) exhausted = true;
+                }
+                const unsigned take2 = min(k - take, w_end - w_next);
                 double e_new = 0.0;
-                if (!alive && rank >= take && idx < n_in) {
+                if (!alive && rank >= take && rank - take < take2) {
+                    const unsigned idx = w_next + rank - take;
                     uint32_t extra;
-                    if (SRC) {
-                        p = make_primary(P, S, hist_base + idx);
+                    if (SRC && idx >= n_queue) {
+                        p = make_primary(P, S, hist_base + (idx - n_queue));
                         e_new = static_cast<double>(p.E);
                         if (electron_tracked(P, p.E)) {
                             alive = true;
@@ -255,16 +270,16 @@ __device__ void electron_phase(const Params &P, const float *__restrict__ TB, co
                     }
                     lnT = flog(p.E);
                 }
+                w_next += take2;
                 if (SRC) {
                     e_new = wsum(e_new);
                     if (lane == 0 && e_new != 0.0) acc.inc(e_new);
                 }
-                if (base + want >= n_in) exhausted = true;
             }
         }
         const unsigned am = __ballot_sync(kFull, alive);
         // ---- hard events, 32 at a time (or whatever is left when nothing else can run)
-        if (n_hard >= 32u || (n_hard > 0u && am == 0u && n_ready == 0u && exhausted)) {
+        if (n_hard >= 32u || (n_hard > 0u && am == 0u && n_ready == 0u && exhausted && w_next == w_end)) {
             const unsigned nb = min(32u, n_hard);
             Particle q, c;
             float qlnT = 0.f;
@@ -311,7 +326,7 @@ __device__ void electron_phase(const Params &P, const float *__restrict__ TB, co
             continue;
         }
         if (am == 0u) {
-            if (exhausted && n_ready == 0u) break;
+            if (exhausted && w_next == w_end && n_ready == 0u) break;
             continue;
         }
         // ---- one condensed-history step for every live lane
@@ -336,6 +351,34 @@ __device__ void electron_phase(const Params &P, const float *__restrict__ TB, co
 }
 
 // ---------------------------------------------------------------------------------------------
+// Optional phase timeline (compile with -DGPUMCD_TIMELINE; development aid, not in the default build):
+// per phase the input size, start time, the time each CTA finished and the time the barrier opened.
+// ---------------------------------------------------------------------------------------------
+#ifdef GPUMCD_TIMELINE
+constexpr int kTlPhases = 256, kTlBlocks = 160;
+struct Timeline {
+    unsigned n_phase;
+    unsigned type[kTlPhases], n_in[kTlPhases];
+    unsigned long long t0[kTlPhases], t1[kTlPhases];
+    unsigned long long done[kTlPhases][kTlBlocks];
+};
+__device__ Timeline g_timeline;
+__device__ __forceinline__ unsigned long long gtime()
+{
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
+    return t;
+}
+#define TL_BEGIN(ty, n) do { if (leader && tl < kTlPhases) { g_timeline.type[tl] = (ty); g_timeline.n_in[tl] = (n); g_timeline.t0[tl] = gtime(); } } while (0)
+#define TL_DONE() do { __syncthreads(); if (threadIdx.x == 0 && tl < kTlPhases && blockIdx.x < kTlBlocks) g_timeline.done[tl][blockIdx.x] = gtime(); } while (0)
+#define TL_END() do { if (leader && tl < kTlPhases) { g_timeline.t1[tl] = gtime(); g_timeline.n_phase = tl + 1; } ++tl; } while (0)
+#else
+#define TL_BEGIN(ty, n) do {} while (0)
+#define TL_DONE() do {} while (0)
+#define TL_END() do {} while (0)
+#endif
+
+// ---------------------------------------------------------------------------------------------
 // The persistent kernel
 // ---------------------------------------------------------------------------------------------
 __device__ __forceinline__ unsigned ld_volatile(const unsigned *p) { return *reinterpret_cast<const volatile unsigned *>(p); }
@@ -358,44 +401,49 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(const PersistArgs a
     float4 *pA = a.privA + gwarp * stride, *pB = a.privB + gwarp * stride;
     uint4 *pC = a.privC + gwarp * stride;
     const bool leader = (blockIdx.x == 0 && threadIdx.x == 0);
+#ifdef GPUMCD_TIMELINE
+    unsigned tl = 0;
+#endif
 
+    // Iterations alternate a photon phase and an electron phase.  Each iteration also injects the
+    // next wave of primaries into the phase of the source's type, so the few particles left over
+    // from a wave ride along with the bulk of the next one instead of costing phases of their own;
+    // only the very end of the run has a tail.  Queue slots [0, n_queue) are read from the queue,
+    // indices beyond that are primaries generated on the fly.
     unsigned long long done = 0;
-    while (done < a.n_hist) {
-        const unsigned n = static_cast<unsigned>(min(static_cast<unsigned long long>(a.wave), a.n_hist - done));
+    int cur = 0;
+    unsigned nP = 0, nE = 0; // queued photons in qP[cur] / electrons in qE
+    for (;;) {
+        const unsigned n_src = static_cast<unsigned>(min(static_cast<unsigned long long>(a.wave), a.n_hist - done));
         const unsigned long long hist_base = a.hist0 + done;
-        // all queue counters and heads are zero here
-        int cur = 0;
-        unsigned nP = (a.S.particle == 0) ? n : 0u, nE = (a.S.particle == 1) ? n : 0u;
-        bool first = true;
-        for (;;) {
-            // ---- photon phase: reads qP[cur] (or the source), fills qE and qP[cur^1]
-            if (nP) {
-                if (first && a.S.particle == 0)
-                    photon_phase<TRACE, true>(P, TB, a.S, hist_base, a.qP[cur], nP, a.heads + 3, a.qE, a.qP[cur ^ 1]);
-                else
-                    photon_phase<TRACE, false>(P, TB, a.S, hist_base, a.qP[cur], nP, a.heads + cur, a.qE, a.qP[cur ^ 1]);
-            }
-            grid.sync();
-            if (leader) { *a.qP[cur].count = 0u; a.heads[cur] = 0u; a.heads[3] = 0u; }
-            if (!(first && a.S.particle == 1)) nE = min(ld_volatile(a.qE.count), a.qE.cap);
-            grid.sync();
-            // ---- electron phase: reads qE (or the source), fills qP[cur^1]; knock-ons stay in the warp
-            if (nE) {
-                if (first && a.S.particle == 1)
-                    electron_phase<true>(P, TB, a.S, hist_base, a.qE, nE, a.heads + 3, a.qP[cur ^ 1], pA, pB, pC, a.priv_ready);
-                else
-                    electron_phase<false>(P, TB, a.S, hist_base, a.qE, nE, a.heads + 2, a.qP[cur ^ 1], pA, pB, pC, a.priv_ready);
-            }
-            grid.sync();
-            if (leader) { *a.qE.count = 0u; a.heads[2] = 0u; a.heads[3] = 0u; }
-            cur ^= 1;
-            nP = min(ld_volatile(a.qP[cur].count), a.qP[cur].cap);
-            nE = 0u;
-            first = false;
-            grid.sync();
-            if (nP == 0u) break;
+        const unsigned srcP = (a.S.particle == 0) ? n_src : 0u, srcE = (a.S.particle == 1) ? n_src : 0u;
+        // ---- photon phase: reads qP[cur] and the source, fills qE and qP[cur^1]
+        TL_BEGIN(0u, nP + srcP);
+        if (nP + srcP) {
+            if (srcP) photon_phase<TRACE, true>(P, TB, a.S, hist_base, a.qP[cur], nP, nP + srcP, a.heads + cur, a.qE, a.qP[cur ^ 1]);
+            else photon_phase<TRACE, false>(P, TB, a.S, hist_base, a.qP[cur], nP, nP, a.heads + cur, a.qE, a.qP[cur ^ 1]);
         }
-        done += n;
+        TL_DONE();
+        grid.sync();
+        TL_END();
+        if (leader) { *a.qP[cur].count = 0u; a.heads[cur] = 0u; }
+        nE = min(ld_volatile(a.qE.count), a.qE.cap);
+        grid.sync();
+        // ---- electron phase: reads qE and the source, fills qP[cur^1]; knock-ons stay in the warp
+        TL_BEGIN(1u, nE + srcE);
+        if (nE + srcE) {
+            if (srcE) electron_phase<true>(P, TB, a.S, hist_base, a.qE, nE, nE + srcE, a.heads + 2, a.qP[cur ^ 1], pA, pB, pC, a.priv_ready);
+            else electron_phase<false>(P, TB, a.S, hist_base, a.qE, nE, nE, a.heads + 2, a.qP[cur ^ 1], pA, pB, pC, a.priv_ready);
+        }
+        TL_DONE();
+        grid.sync();
+        TL_END();
+        if (leader) { *a.qE.count = 0u; a.heads[2] = 0u; }
+        cur ^= 1;
+        nP = min(ld_volatile(a.qP[cur].count), a.qP[cur].cap);
+        done += n_src;
+        grid.sync();
+        if (nP == 0u && done >= a.n_hist) break;
     }
     if (!a.finalize) return;
     grid.sync();

@@ -400,40 +400,65 @@ __device__ __forceinline__ int electron_hard(const Params &P, const float *__res
     const float T1 = p.E;
     kind = HK_FICT;
     if (r >= sM + sB) return ST_ALIVE;
-    if (r < sM) {
-        // Moller (L88-90)
-        kind = HK_MOLLER;
-        float eps, uphi, sp, cp;
-        sample_moller(P.rng, p, T1, tb.e_cut, eps, uphi);
-        sincos2pi(uphi, sp, cp);
-        const float W = eps * T1;
+    // One rejection loop serves both samplers (one Philox block per trial, as everywhere): the lanes
+    // of a sorted batch stay together through the expensive part, whatever their event kind.
+    //   Moller (L90): eps = W/T in [K_cut/T, 1/2] from 1/eps^2, g = 1 + g2 eps^2 + r (r - g3)
+    //   brems  (L92): k in [k_c, T] from 1/k, g = 4/3 (1 - y) + y^2, y = k/(T + m)
+    const bool mol = r < sM;
+    kind = mol ? HK_MOLLER : HK_BREMS;
+    const float tau = T1 * (1.0f / kMe);
+    const float qq = tau / (tau + 1.0f);
+    const float g2 = qq * qq;
+    const float g3 = (2.0f * tau + 1.0f) / ((tau + 1.0f) * (tau + 1.0f));
+    const float gmax = mol ? 1.0f + 0.25f * g2 + (1.0f - g3) : (4.0f / 3.0f);
+    const float emin = tb.e_cut / T1;
+    const float lr = logf(T1 / tb.p_cut);
+    const float iEt = 1.0f / (T1 + kMe);
+    float x, uphi;
+    for (;;) {
+        const uint4 v = draw(P.rng, p);
+        const float u0 = u01(v.x);
+        float gg;
+        if (mol) {
+            x = emin / (1.0f - u0 * (1.0f - 2.0f * emin));
+            const float rr = x / (1.0f - x);
+            gg = 1.0f + g2 * x * x + rr * (rr - g3);
+        } else {
+            x = tb.p_cut * expf(u0 * lr);
+            const float y = x * iEt;
+            gg = fmaf(y, y, (4.0f / 3.0f) * (1.0f - y));
+        }
+        if (u01(v.y) * gmax <= gg) {
+            uphi = u01(v.z);
+            break;
+        }
+    }
+    float sp, cp;
+    sincos2pi(uphi, sp, cp);
+    child = p;
+    child.track = lineage(P.rng, p).x;
+    child.ctr = 0u;
+    if (mol) {
+        // Moller kinematics (L88-90): scattered and knock-on electrons at opposite azimuths
+        const float W = x * T1;
         const float Tp = T1 - W;
         const float den_p = 1.0f / (T1 * (Tp + 2.0f * kMe));
         const float den_d = 1.0f / (T1 * (W + 2.0f * kMe));
         const float cpo = sqrtf(Tp * (T1 + 2.0f * kMe) * den_p), spo = sqrtf(2.0f * kMe * W * den_p);
         const float cdo = sqrtf(W * (T1 + 2.0f * kMe) * den_d), sdo = sqrtf(2.0f * kMe * Tp * den_d);
-        child = p;
-        rotate(p.u, p.v, p.w, cdo, sdo, -cp, -sp, child.u, child.v, child.w); // knock-on at the opposite azimuth
+        rotate(p.u, p.v, p.w, cdo, sdo, -cp, -sp, child.u, child.v, child.w);
         child.E = W;
-        child.track = lineage(P.rng, p).x;
-        child.ctr = 0u;
         rotate(p.u, p.v, p.w, cpo, spo, cp, sp, p.u, p.v, p.w);
         p.E = Tp;
         lnT = flog(Tp);
         return ST_ALIVE;
     }
     // bremsstrahlung (L92): electron direction unchanged, photon at theta = m/E
-    kind = HK_BREMS;
-    float k, uphi, sp, cp, st, ct;
-    sample_brems(P.rng, p, T1, tb.p_cut, k, uphi);
-    sincos2pi(uphi, sp, cp);
-    sincosf(kMe / (T1 + kMe), &st, &ct);
-    child = p;
+    float st, ct;
+    sincosf(kMe * iEt, &st, &ct);
     rotate(p.u, p.v, p.w, ct, st, cp, sp, child.u, child.v, child.w);
-    child.E = k;
-    child.track = lineage(P.rng, p).x;
-    child.ctr = 0u;
-    p.E = T1 - k;
+    child.E = x;
+    p.E = T1 - x;
     if (p.E < tb.e_cut) {
         deposit(P, lin1, p.E);
         acc.cut(p.E);
