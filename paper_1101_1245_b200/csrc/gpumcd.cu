@@ -123,6 +123,8 @@ __global__ void k_finalize(const double *__restrict__ edep, const float2 *__rest
 // =============================================================================================
 using namespace gpumcd;
 
+constexpr int kMaxQueues = 6;
+
 struct gpumcd_ctx {
     int nx = 0, ny = 0, nz = 0;
     size_t nvox = 0;
@@ -134,15 +136,18 @@ struct gpumcd_ctx {
     float *table_blob = nullptr;
     double *edep = nullptr;
     DevCounters *cnt = nullptr;
-    unsigned *qcount = nullptr; // 4 counters: PA, PB, EA, EB
-    float4 *qA[4] = {nullptr, nullptr, nullptr, nullptr};
-    float4 *qB[4] = {nullptr, nullptr, nullptr, nullptr};
-    uint4 *qC[4] = {nullptr, nullptr, nullptr, nullptr};
+    // particle queues: scheduler 0 uses 0..3 (PA, PB, EA, EB); scheduler 1 uses 0..2 as its three
+    // photon queues and 3..5 as its three electron queues
+    int n_queues = 4;
+    unsigned *qcount = nullptr; // kMaxQueues push counters
+    float4 *qA[kMaxQueues] = {};
+    float4 *qB[kMaxQueues] = {};
+    uint4 *qC[kMaxQueues] = {};
     unsigned qcap = 0;
     double *spec_cdf = nullptr;
     float *spec_edges = nullptr;
     // scheduler 1 (persistent kernel)
-    unsigned *heads = nullptr;      // 4 pop heads
+    unsigned *heads = nullptr;      // kMaxQueues pop heads
     float4 *privA = nullptr, *privB = nullptr;
     uint4 *privC = nullptr;
     unsigned priv_ready = 0;        // ready-stack capacity per warp
@@ -230,7 +235,7 @@ static void destroy_impl(gpumcd_ctx *c)
     cudaFree(c->edep);
     cudaFree(c->cnt);
     cudaFree(c->qcount);
-    for (int k = 0; k < 4; ++k) { cudaFree(c->qA[k]); cudaFree(c->qB[k]); cudaFree(c->qC[k]); }
+    for (int k = 0; k < kMaxQueues; ++k) { cudaFree(c->qA[k]); cudaFree(c->qB[k]); cudaFree(c->qC[k]); }
     cudaFree(c->spec_cdf);
     cudaFree(c->spec_edges);
     cudaFree(c->heads);
@@ -352,9 +357,10 @@ static int create_impl(gpumcd_ctx **out, const float *density, const uint8_t *ma
     // ---- tally, counters, queues ----
     CK(cudaMalloc(&ctx->edep, nvox * sizeof(double)));
     CK(cudaMalloc(&ctx->cnt, sizeof(DevCounters)));
-    CK(cudaMalloc(&ctx->qcount, 4 * sizeof(unsigned)));
+    CK(cudaMalloc(&ctx->qcount, kMaxQueues * sizeof(unsigned)));
+    ctx->n_queues = opt.scheduler == 1 ? 6 : 4;
     ctx->qcap = opt.wave_size * opt.bank_factor;
-    for (int k = 0; k < 4; ++k) {
+    for (int k = 0; k < ctx->n_queues; ++k) {
         CK(cudaMalloc(&ctx->qA[k], static_cast<size_t>(ctx->qcap) * sizeof(float4)));
         CK(cudaMalloc(&ctx->qB[k], static_cast<size_t>(ctx->qcap) * sizeof(float4)));
         CK(cudaMalloc(&ctx->qC[k], static_cast<size_t>(ctx->qcap) * sizeof(uint4)));
@@ -367,7 +373,9 @@ static int create_impl(gpumcd_ctx **out, const float *density, const uint8_t *ma
         CK(cudaDeviceGetAttribute(&max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
         if (!coop) { set_error(ctx, "device does not support cooperative launches (scheduler 1)"); return GPUMCD_ERR_CUDA; }
         const size_t table_bytes = static_cast<size_t>(ctx->table_floats) * sizeof(float);
-        ctx->smem_tables = table_bytes + 2048 <= static_cast<size_t>(max_smem);
+        cudaFuncAttributes fa{};
+        CK(cudaFuncGetAttributes(&fa, k_persistent<false, true>));
+        ctx->smem_tables = table_bytes + fa.sharedSizeBytes + 1024 <= static_cast<size_t>(max_smem);
         const size_t dyn = ctx->smem_tables ? table_bytes : 0;
         if (ctx->smem_tables) {
             CK(cudaFuncSetAttribute(k_persistent<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(dyn)));
@@ -386,7 +394,7 @@ static int create_impl(gpumcd_ctx **out, const float *density, const uint8_t *ma
         CK(cudaMalloc(&ctx->privA, recs * sizeof(float4)));
         CK(cudaMalloc(&ctx->privB, recs * sizeof(float4)));
         CK(cudaMalloc(&ctx->privC, recs * sizeof(uint4)));
-        CK(cudaMalloc(&ctx->heads, 4 * sizeof(unsigned)));
+        CK(cudaMalloc(&ctx->heads, kMaxQueues * sizeof(unsigned)));
     }
     CK(cudaDeviceSynchronize());
     guard.ok = true;
@@ -540,8 +548,8 @@ static int run_waves_host_loop(gpumcd_ctx *ctx, uint64_t n_hist, uint64_t seed, 
 static int run_persistent(gpumcd_ctx *ctx, uint64_t n_hist, uint64_t seed, float *dose_dev, unsigned long long *trace,
                           cudaStream_t st)
 {
-    CK(cudaMemsetAsync(ctx->qcount, 0, 4 * sizeof(unsigned), st));
-    CK(cudaMemsetAsync(ctx->heads, 0, 4 * sizeof(unsigned), st));
+    CK(cudaMemsetAsync(ctx->qcount, 0, kMaxQueues * sizeof(unsigned), st));
+    CK(cudaMemsetAsync(ctx->heads, 0, kMaxQueues * sizeof(unsigned), st));
     const double h3 = static_cast<double>(ctx->h) * ctx->h * ctx->h;
     uint64_t h0 = ctx->hist_offset;
     const uint64_t h_end = ctx->hist_offset + n_hist;
@@ -550,9 +558,7 @@ static int run_persistent(gpumcd_ctx *ctx, uint64_t n_hist, uint64_t seed, float
         PersistArgs a{};
         a.P = make_params(ctx, seed, static_cast<uint32_t>(h0 >> 32), trace != nullptr, trace);
         a.S = ctx->src;
-        a.qP[0] = make_queue(ctx, 0);
-        a.qP[1] = make_queue(ctx, 1);
-        a.qE = make_queue(ctx, 2);
+        for (int k = 0; k < 3; ++k) { a.qP[k] = make_queue(ctx, k); a.qE[k] = make_queue(ctx, 3 + k); }
         a.heads = ctx->heads;
         a.privA = ctx->privA; a.privB = ctx->privB; a.privC = ctx->privC;
         a.priv_ready = ctx->priv_ready;

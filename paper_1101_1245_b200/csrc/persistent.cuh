@@ -115,9 +115,9 @@ __device__ __forceinline__ void stage_tables(float *dst, const float *src, unsig
 struct PersistArgs {
     Params P;
     SourceDev S;
-    Queue qP[2];       // photon queues, alternating by phase
-    Queue qE;          // electron queue (filled by photon phases, drained by electron phases)
-    unsigned *heads;   // pop heads: [0],[1] photon queues, [2] electron queue, [3] source
+    Queue qP[3];       // photon queues, rotating: read [i%3], written [(i+1)%3], reset [(i+2)%3]
+    Queue qE[3];       // electron queues, same rotation
+    unsigned *heads;   // pop heads: [0..2] photon queues, [3..5] electron queues
     float4 *privA;     // per-warp private records: ready stack [priv_ready] then hard buffer [kHardCap]
     float4 *privB;
     uint4 *privC;
@@ -369,11 +369,11 @@ __device__ __forceinline__ unsigned long long gtime()
     asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
     return t;
 }
-#define TL_BEGIN(ty, n) do { if (leader && tl < kTlPhases) { g_timeline.type[tl] = (ty); g_timeline.n_in[tl] = (n); g_timeline.t0[tl] = gtime(); } } while (0)
+#define TL_BEGIN(np, ne) do { if (leader && tl < kTlPhases) { g_timeline.type[tl] = (np); g_timeline.n_in[tl] = (ne); g_timeline.t0[tl] = gtime(); } } while (0)
 #define TL_DONE() do { __syncthreads(); if (threadIdx.x == 0 && tl < kTlPhases && blockIdx.x < kTlBlocks) g_timeline.done[tl][blockIdx.x] = gtime(); } while (0)
 #define TL_END() do { if (leader && tl < kTlPhases) { g_timeline.t1[tl] = gtime(); g_timeline.n_phase = tl + 1; } ++tl; } while (0)
 #else
-#define TL_BEGIN(ty, n) do {} while (0)
+#define TL_BEGIN(np, ne) do {} while (0)
 #define TL_DONE() do {} while (0)
 #define TL_END() do {} while (0)
 #endif
@@ -405,45 +405,52 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(const PersistArgs a
     unsigned tl = 0;
 #endif
 
-    // Iterations alternate a photon phase and an electron phase.  Each iteration also injects the
-    // next wave of primaries into the phase of the source's type, so the few particles left over
-    // from a wave ride along with the bulk of the next one instead of costing phases of their own;
-    // only the very end of the run has a tail.  Queue slots [0, n_queue) are read from the queue,
-    // indices beyond that are primaries generated on the fly.
+    // One iteration = one photon phase and one electron phase that do NOT depend on each other:
+    // iteration i reads photon queue X[i%3] and electron queue Y[i%3] and writes X[(i+1)%3] /
+    // Y[(i+1)%3]; the third pair was read in iteration i-1 and is reset now, to be written in i+1.
+    // So one grid barrier per iteration suffices, a warp that runs out of one type's input moves on
+    // to the other type without waiting, and odd / even warps start with different types, which
+    // keeps latency-bound photon warps and issue-bound electron warps on every SM at the same time.
+    // Each iteration also injects the next wave of primaries, so what is left over from a wave
+    // rides along with the bulk of the next one; only the very end of the run has a tail.
     unsigned long long done = 0;
-    int cur = 0;
-    unsigned nP = 0, nE = 0; // queued photons in qP[cur] / electrons in qE
+    unsigned it = 0;
+    unsigned nP = 0, nE = 0; // queued photons in X[it%3] / electrons in Y[it%3]
+    const bool e_first = ((threadIdx.x >> 5) & 1) != 0;
     for (;;) {
+        const unsigned r = it % 3u, w = (it + 1u) % 3u, z = (it + 2u) % 3u;
         const unsigned n_src = static_cast<unsigned>(min(static_cast<unsigned long long>(a.wave), a.n_hist - done));
         const unsigned long long hist_base = a.hist0 + done;
         const unsigned srcP = (a.S.particle == 0) ? n_src : 0u, srcE = (a.S.particle == 1) ? n_src : 0u;
-        // ---- photon phase: reads qP[cur] and the source, fills qE and qP[cur^1]
-        TL_BEGIN(0u, nP + srcP);
-        if (nP + srcP) {
-            if (srcP) photon_phase<TRACE, true>(P, TB, a.S, hist_base, a.qP[cur], nP, nP + srcP, a.heads + cur, a.qE, a.qP[cur ^ 1]);
-            else photon_phase<TRACE, false>(P, TB, a.S, hist_base, a.qP[cur], nP, nP, a.heads + cur, a.qE, a.qP[cur ^ 1]);
+        if (leader) {
+            *a.qP[z].count = 0u; a.heads[z] = 0u;
+            *a.qE[z].count = 0u; a.heads[3 + z] = 0u;
+        }
+        TL_BEGIN(nP + srcP, nE + srcE);
+#pragma unroll 1
+        for (int t = 0; t < 2; ++t) {
+            if ((t == 0) != e_first) {
+                // photons: read X[r] and the source, electrons -> Y[w], annihilation photons -> X[w]
+                if (nP + srcP) {
+                    if (srcP) photon_phase<TRACE, true>(P, TB, a.S, hist_base, a.qP[r], nP, nP + srcP, a.heads + r, a.qE[w], a.qP[w]);
+                    else photon_phase<TRACE, false>(P, TB, a.S, hist_base, a.qP[r], nP, nP, a.heads + r, a.qE[w], a.qP[w]);
+                }
+            } else {
+                // electrons: read Y[r] and the source, bremsstrahlung photons -> X[w], knock-ons stay in the warp
+                if (nE + srcE) {
+                    if (srcE) electron_phase<true>(P, TB, a.S, hist_base, a.qE[r], nE, nE + srcE, a.heads + 3 + r, a.qP[w], pA, pB, pC, a.priv_ready);
+                    else electron_phase<false>(P, TB, a.S, hist_base, a.qE[r], nE, nE, a.heads + 3 + r, a.qP[w], pA, pB, pC, a.priv_ready);
+                }
+            }
         }
         TL_DONE();
         grid.sync();
         TL_END();
-        if (leader) { *a.qP[cur].count = 0u; a.heads[cur] = 0u; }
-        nE = min(ld_volatile(a.qE.count), a.qE.cap);
-        grid.sync();
-        // ---- electron phase: reads qE and the source, fills qP[cur^1]; knock-ons stay in the warp
-        TL_BEGIN(1u, nE + srcE);
-        if (nE + srcE) {
-            if (srcE) electron_phase<true>(P, TB, a.S, hist_base, a.qE, nE, nE + srcE, a.heads + 2, a.qP[cur ^ 1], pA, pB, pC, a.priv_ready);
-            else electron_phase<false>(P, TB, a.S, hist_base, a.qE, nE, nE, a.heads + 2, a.qP[cur ^ 1], pA, pB, pC, a.priv_ready);
-        }
-        TL_DONE();
-        grid.sync();
-        TL_END();
-        if (leader) { *a.qE.count = 0u; a.heads[2] = 0u; }
-        cur ^= 1;
-        nP = min(ld_volatile(a.qP[cur].count), a.qP[cur].cap);
+        nP = min(ld_volatile(a.qP[w].count), a.qP[w].cap);
+        nE = min(ld_volatile(a.qE[w].count), a.qE[w].cap);
         done += n_src;
-        grid.sync();
-        if (nP == 0u && done >= a.n_hist) break;
+        ++it;
+        if (nP == 0u && nE == 0u && done >= a.n_hist) break;
     }
     if (!a.finalize) return;
     grid.sync();
