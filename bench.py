@@ -44,15 +44,49 @@ def measured_peaks():
 
 
 class ClockSampler:
-    """Samples nvidia-smi clocks / throttle reasons every 200 ms while the timed region runs."""
+    """Samples SM clock and throttle reasons while the timed region runs (NVML every 20 ms; falls back to
+    `nvidia-smi -lms 200` when the NVML binding is unavailable)."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
          "clocks_event_reasons.sw_power_cap")
 
     def __init__(self, index: int):
-        self.index, self.rows, self.proc = index, [], None
+        self.index, self.rows, self.proc, self.thread = index, [], None, None
+        self.sm, self.smax, self.reasons, self._stop = [], [], set(), threading.Event()
+
+    def _nvml_loop(self, nv, h):
+        names = {"hw_slowdown": nv.nvmlClocksThrottleReasonHwSlowdown,
+                 "hw_thermal_slowdown": nv.nvmlClocksThrottleReasonHwThermalSlowdown,
+                 "sw_thermal_slowdown": nv.nvmlClocksThrottleReasonSwThermalSlowdown,
+                 "sw_power_cap": nv.nvmlClocksThrottleReasonSwPowerCap}
+        smax = float(nv.nvmlDeviceGetMaxClockInfo(h, nv.NVML_CLOCK_SM))
+        while not self._stop.is_set():
+            try:
+                self.sm.append(float(nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM)))
+                self.smax.append(smax)
+                mask = nv.nvmlDeviceGetCurrentClocksThrottleReasons(h)
+                for n, bit in names.items():
+                    if mask & bit:
+                        self.reasons.add(n)
+            except Exception:
+                pass
+            self._stop.wait(0.02)
 
     def start(self):
+        try:
+            import pynvml as nv
+            nv.nvmlInit()
+            # NVML enumerates physical devices: map the CUDA ordinal through CUDA_VISIBLE_DEVICES when it lists indices
+            vis = os.environ.get("CUDA_VISIBLE_DEVICES", "")
+            idx = self.index
+            if vis and all(x.strip().isdigit() for x in vis.split(",")):
+                idx = int(vis.split(",")[self.index])
+            h = nv.nvmlDeviceGetHandleByIndex(idx)
+            self.thread = threading.Thread(target=self._nvml_loop, args=(nv, h), daemon=True)
+            self.thread.start()
+            return
+        except Exception:
+            self.thread = None
         try:
             self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
                                           "--format=csv,noheader,nounits", "-lms", "200"],
@@ -66,13 +100,16 @@ class ClockSampler:
             self.rows.append([x.strip() for x in line.split(",")])
 
     def stop(self):
+        self._stop.set()
+        if self.thread:
+            self.thread.join(timeout=1)
         if self.proc:
             self.proc.terminate()
             try:
                 self.proc.wait(timeout=2)
             except subprocess.TimeoutExpired:
                 self.proc.kill()
-        sm, smax, reasons = [], [], set()
+        sm, smax, reasons = list(self.sm), list(self.smax), set(self.reasons)
         for r in self.rows:
             try:
                 sm.append(float(r[0]))
@@ -137,12 +174,13 @@ def reference_arm(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=2)
     ap.add_argument("--histories", type=int, default=0, help="override histories per step (0 = the config's)")
     ap.add_argument("--scheduler", type=int, default=-1)
+    ap.add_argument("--wave", type=int, default=0, help="override wave_size (0 = library default)")
     ap.add_argument("--ref-histories", type=int, default=50_000)
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -157,6 +195,7 @@ def main():
     import paper_1101_1245_b200 as g
     from paper_1101_1245_b200 import build as cuda_build
     from paper_1101_1245_b200.inputs import make_config
+    from paper_1101_1245_b200.sharding import combine_dose
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -183,6 +222,8 @@ def main():
     opts = {}
     if args.scheduler >= 0:
         opts["scheduler"] = args.scheduler
+    if args.wave > 0:
+        opts["wave_size"] = args.wave
     opt = g.gpumcd_default_options(**opts)
     ctx = g.gpumcd_create(rho, mat, w.voxel_cm, w.tables, opt)
     g.gpumcd_set_source(ctx, w.source)
@@ -193,7 +234,7 @@ def main():
     def step(seed):
         g.gpumcd_run(ctx, n, seed, dose)
         if dist:
-            dist.all_reduce(dose)                     # "the resulting dose arrays are summed" (L188)
+            combine_dose(dose, n, world * n, dist)    # "the resulting dose arrays are summed" (L188)
 
     for k in range(args.warmup):
         step(w.seed + k)
@@ -251,33 +292,40 @@ def main():
                 "kernel_share_of_step": ms_e / t_ms if t_ms else None,
                 "alg_inst_per_ch_step": ALG_INST_PER_CH_STEP}
 
-    # ---- end to end through the host entry points (volumes and dose in host memory)
+    # ---- end to end through the host entry points: every step copies that step's inputs (the phantom volumes,
+    # from pinned host memory) to the device and the resulting dose grid back to the host
     e2e = None
     if not args.no_e2e:
         rho_h = torch.from_numpy(w.density).pin_memory()
         mat_h = torch.from_numpy(w.material).pin_memory()
         dose_h = torch.empty(rho.shape, dtype=torch.float32).pin_memory()
-        reps, tot = 0, 0.0
-        for k in range(1 + min(args.steps, 3)):
-            torch.cuda.synchronize()
-            t0 = time.perf_counter()
-            with g.gpumcd_create_host(rho_h.numpy(), mat_h.numpy(), w.voxel_cm, w.tables, opt) as c2:
-                g.gpumcd_set_source(c2, w.source)
-                g.gpumcd_set_history_offset(c2, rank * n)
-                g.gpumcd_run_host(c2, n, w.seed + 200 + k, dose_h.numpy())
-            torch.cuda.synchronize()
-            if k > 0:
-                tot += time.perf_counter() - t0
-                reps += 1
-        e2e_t = tot / reps
+        rho_np, mat_np, dose_np = rho_h.numpy(), mat_h.numpy(), dose_h.numpy()
+
+        def e2e_step(seed):
+            g.gpumcd_set_phantom_host(ctx, rho_np, mat_np)
+            g.gpumcd_set_source(ctx, w.source)
+            g.gpumcd_run_host(ctx, n, seed, dose_np)          # returns after the device-to-host copy
+
+        g.gpumcd_set_profiling(ctx, False)
+        for k in range(args.warmup):
+            e2e_step(w.seed + 300 + k)
+        if dist:
+            dist.barrier()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for k in range(args.steps):
+            e2e_step(w.seed + 400 + k)
+        torch.cuda.synchronize()
+        e2e_t = (time.perf_counter() - t0) / args.steps
         if dist:
             tt = torch.tensor([e2e_t], dtype=torch.float64, device=dev)
             dist.all_reduce(tt, op=dist.ReduceOp.MAX)
             e2e_t = float(tt.item())
-        tab_bytes = 4 * (w.tables.photon.size + w.tables.electron.size + w.tables.ms_a.size)
-        e2e = {"value": world * n / e2e_t, "unit": "histories/s", "h2d_bytes_per_step": int(rho.numel() * 5 + tab_bytes),
-               "d2h_bytes_per_step": int(rho.numel() * 4), "ms_per_step": e2e_t * 1e3,
-               "what": "gpumcd_create_host + set_source + run_host + destroy, wall clock"}
+        blob_bytes = 4 * (w.tables.photon.size + w.tables.electron.size + w.tables.ms_a.size + 2 * w.tables.n_energy)
+        e2e = {"value": world * n / e2e_t, "unit": "histories/s",
+               "h2d_bytes_per_step": int(rho.numel() * 5 + blob_bytes), "d2h_bytes_per_step": int(rho.numel() * 4),
+               "ms_per_step": e2e_t * 1e3,
+               "what": "gpumcd_set_phantom_host + gpumcd_set_source + gpumcd_run_host per step, wall clock, pinned host buffers"}
 
     g.gpumcd_destroy(ctx)
 

@@ -77,14 +77,17 @@ typedef struct {
                               photons; 0: it is deposited at the vertex (L74 is silent)            */
     int32_t photon_only;   /* 1: every electron is deposited where it is born; default 0           */
     float majorant_scale;  /* >= 1, inflates the Woodcock majorants (Eq. 3; test hook); default 1  */
-    uint32_t wave_size;    /* primaries generated per wave; default 2^20                           */
-    uint32_t bank_factor;  /* queue capacity = bank_factor * wave_size records (the paper's d, L166);
-                              default 8                                                            */
-    int32_t scheduler;     /* 1 (default): one persistent cooperative kernel per run, lanes refilled,
-                              hard events sorted, no host round trips;
+    uint32_t wave_size;    /* scheduler 0: primaries generated per wave; default 2^20              */
+    uint32_t bank_factor;  /* scheduler 0: queue capacity = bank_factor * wave_size records (the
+                              paper's d, L166); default 8                                          */
+    int32_t scheduler;     /* 1 (default): one persistent kernel per run; every warp keeps its own
+                              type-sorted stacks of secondaries, refills its lanes and sorts events,
+                              no host round trips;
                               0: the paper's scheme (L166): one launch per pass, one thread per
                               particle, the host reads the queue counts between passes            */
-    int32_t reserved;
+    uint32_t warp_stack;   /* scheduler 1: capacity of a warp's electron stack and of its photon
+                              stack, records; default 1024 (smaller values only make sense in
+                              tests of the overflow report; at least 192)                          */
 } gpumcd_options;
 
 typedef struct {
@@ -103,7 +106,7 @@ typedef struct {
     uint64_t photon_flights, photon_compton, photon_photo, photon_pair, photon_fict;
     uint64_t ch_steps, hard_moller, hard_brems, hard_fict;
     uint64_t pushes_e, pushes_g;
-    uint64_t bank_high_water; /* largest queue occupancy seen, records */
+    uint64_t bank_high_water; /* largest queue (scheduler 0) or warp stack (scheduler 1) occupancy seen, records */
     uint64_t overflow_count;  /* records dropped because a queue was full; must be 0 */
     double e_incident, e_dep_continuous, e_dep_cutoff, e_escaped, e_pair_rest; /* MeV */
 } gpumcd_counters;
@@ -123,6 +126,16 @@ int gpumcd_create(gpumcd_ctx **out, const float *density_dev, const uint8_t *mat
 int gpumcd_create_host(gpumcd_ctx **out, const float *density_host, const uint8_t *material_host,
                        int nx, int ny, int nz, float voxel_cm, const gpumcd_tables *tables,
                        const gpumcd_options *opt);
+
+/* Replace the phantom of an existing context by another one of the same dimensions (the
+ * per-patient inputs of the method): the volumes are copied (gpumcd_set_phantom:
+ * DEVICE pointers; gpumcd_set_phantom_host: HOST pointers, the host-to-device copy is part of the
+ * call and is fastest from pinned memory), validated, and the majorants mu_max(E), M_e(E) are
+ * rebuilt.  Waits for the context's last run; synchronous.  Tables, options, source and queues
+ * are kept.  On GPUMCD_ERR_INVALID_ARG (bad voxel) the context must be given a valid phantom
+ * before the next run. */
+int gpumcd_set_phantom(gpumcd_ctx *ctx, const float *density_dev, const uint8_t *material_dev);
+int gpumcd_set_phantom_host(gpumcd_ctx *ctx, const float *density_host, const uint8_t *material_host);
 
 /* Select the source (PAPER.md L166 initParticle): particle type, energy or spectrum, geometry. */
 int gpumcd_set_source(gpumcd_ctx *ctx, const gpumcd_source *src);

@@ -23,7 +23,8 @@ GPUMCD_ERR_BANK_OVERFLOW = -4
 GPUMCD_ERR_NO_SOURCE = -5
 GPUMCD_ERR_TABLE_RANGE = -6
 
-EXPORTS = ("gpumcd_default_options", "gpumcd_create", "gpumcd_create_host", "gpumcd_set_source", "gpumcd_run",
+EXPORTS = ("gpumcd_default_options", "gpumcd_create", "gpumcd_create_host", "gpumcd_set_phantom",
+           "gpumcd_set_phantom_host", "gpumcd_set_source", "gpumcd_run",
            "gpumcd_run_host", "gpumcd_run_trace", "gpumcd_get_counters", "gpumcd_get_energy_tally",
            "gpumcd_set_history_offset", "gpumcd_set_profiling", "gpumcd_get_profile",
            "gpumcd_last_error", "gpumcd_destroy")
@@ -39,7 +40,7 @@ class gpumcd_options(C.Structure):
     _fields_ = [("es_max_cm", C.c_float), ("f_eloss_max", C.c_float), ("boundary_nudge", C.c_float),
                 ("pair_mode", C.c_int32), ("photon_only", C.c_int32), ("majorant_scale", C.c_float),
                 ("wave_size", C.c_uint32), ("bank_factor", C.c_uint32), ("scheduler", C.c_int32),
-                ("reserved", C.c_int32)]
+                ("warp_stack", C.c_uint32)]
 
 
 class gpumcd_source(C.Structure):
@@ -90,6 +91,8 @@ def load_library():
         lib.gpumcd_create.argtypes = [C.POINTER(vp), vp, vp, C.c_int, C.c_int, C.c_int, C.c_float,
                                       C.POINTER(gpumcd_tables), C.POINTER(gpumcd_options)]
         lib.gpumcd_create_host.argtypes = lib.gpumcd_create.argtypes
+        lib.gpumcd_set_phantom.argtypes = [vp, vp, vp]
+        lib.gpumcd_set_phantom_host.argtypes = [vp, vp, vp]
         lib.gpumcd_set_source.argtypes = [vp, C.POINTER(gpumcd_source)]
         lib.gpumcd_run.argtypes = [vp, C.c_uint64, C.c_uint64, vp, vp]
         lib.gpumcd_run_host.argtypes = [vp, C.c_uint64, C.c_uint64, vp, vp]
@@ -191,6 +194,23 @@ def gpumcd_create_host(density: np.ndarray, material: np.ndarray, voxel_cm, tabl
     assert density.shape == material.shape and density.ndim == 3
     return _create(load_library().gpumcd_create_host, _hptr(density), _hptr(material), density.shape, voxel_cm,
                    tables, options)
+
+
+def gpumcd_set_phantom(ctx: Context, density_dev, material_dev) -> None:
+    """New phantom of the same shape from CUDA tensors (float32 / uint8, [nz,ny,nx])."""
+    assert density_dev.is_cuda and material_dev.is_cuda and density_dev.is_contiguous() and material_dev.is_contiguous()
+    assert tuple(density_dev.shape) == ctx.shape == tuple(material_dev.shape)
+    assert density_dev.element_size() == 4 and material_dev.element_size() == 1
+    ctx._check(load_library().gpumcd_set_phantom(ctx._h, C.c_void_p(density_dev.data_ptr()),
+                                                 C.c_void_p(material_dev.data_ptr())))
+
+
+def gpumcd_set_phantom_host(ctx: Context, density: np.ndarray, material: np.ndarray) -> None:
+    """New phantom of the same shape from host arrays (float32 / uint8, [nz,ny,nx]; pinned memory copies fastest)."""
+    assert density.dtype == np.float32 and material.dtype == np.uint8
+    assert density.flags.c_contiguous and material.flags.c_contiguous
+    assert density.shape == ctx.shape == material.shape
+    ctx._check(load_library().gpumcd_set_phantom_host(ctx._h, _hptr(density), _hptr(material)))
 
 
 def gpumcd_set_source(ctx: Context, source) -> None:

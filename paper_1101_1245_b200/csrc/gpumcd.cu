@@ -123,7 +123,7 @@ __global__ void k_finalize(const double *__restrict__ edep, const float2 *__rest
 // =============================================================================================
 using namespace gpumcd;
 
-constexpr int kMaxQueues = 6;
+constexpr int kMaxQueues = 4;
 
 struct gpumcd_ctx {
     int nx = 0, ny = 0, nz = 0;
@@ -133,11 +133,16 @@ struct gpumcd_ctx {
     gpumcd_options opt{};
     // device memory
     float2 *phantom = nullptr;
+    float *stage_density = nullptr;   // device staging of host volumes (gpumcd_create_host / set_phantom_host)
+    uint8_t *stage_material = nullptr;
+    unsigned *scratch = nullptr;      // 8 rho_max bit patterns + 1 bad-voxel count
+    float *dose_stage = nullptr;      // device dose of gpumcd_run_host
     float *table_blob = nullptr;
+    std::vector<float> blob_host;     // host copy of the table blob (majorants are rebuilt per phantom)
+    int n_mat = 0, n_E = 0;
     double *edep = nullptr;
     DevCounters *cnt = nullptr;
-    // particle queues: scheduler 0 uses 0..3 (PA, PB, EA, EB); scheduler 1 uses 0..2 as its three
-    // photon queues and 3..5 as its three electron queues
+    // global particle queues of scheduler 0: PA, PB, EA, EB (scheduler 1 has per-warp stacks instead)
     int n_queues = 4;
     unsigned *qcount = nullptr; // kMaxQueues push counters
     float4 *qA[kMaxQueues] = {};
@@ -147,10 +152,11 @@ struct gpumcd_ctx {
     double *spec_cdf = nullptr;
     float *spec_edges = nullptr;
     // scheduler 1 (persistent kernel)
-    unsigned *heads = nullptr;      // kMaxQueues pop heads
-    float4 *privA = nullptr, *privB = nullptr;
-    uint4 *privC = nullptr;
-    unsigned priv_ready = 0;        // ready-stack capacity per warp
+    unsigned *head = nullptr;       // next primary to be claimed
+    float4 *stkA = nullptr, *stkB = nullptr; // per-warp stacks (persistent.cuh)
+    uint4 *stkC = nullptr;
+    unsigned cap_r = 0;             // ready-stack capacity per warp
+    unsigned stride = 0;            // records per warp
     int p_grid = 0;                 // CTAs of the persistent kernel (one per SM)
     bool smem_tables = false;
     unsigned table_floats = 0;
@@ -223,7 +229,7 @@ extern "C" int gpumcd_default_options(gpumcd_options *opt)
     opt->wave_size = 1u << 20;
     opt->bank_factor = 8;
     opt->scheduler = 1;
-    opt->reserved = 0;
+    opt->warp_stack = 1024;
     return GPUMCD_OK;
 }
 
@@ -231,6 +237,10 @@ static void destroy_impl(gpumcd_ctx *c)
 {
     if (!c) return;
     cudaFree(c->phantom);
+    cudaFree(c->stage_density);
+    cudaFree(c->stage_material);
+    cudaFree(c->scratch);
+    cudaFree(c->dose_stage);
     cudaFree(c->table_blob);
     cudaFree(c->edep);
     cudaFree(c->cnt);
@@ -238,10 +248,61 @@ static void destroy_impl(gpumcd_ctx *c)
     for (int k = 0; k < kMaxQueues; ++k) { cudaFree(c->qA[k]); cudaFree(c->qB[k]); cudaFree(c->qC[k]); }
     cudaFree(c->spec_cdf);
     cudaFree(c->spec_edges);
-    cudaFree(c->heads);
-    cudaFree(c->privA); cudaFree(c->privB); cudaFree(c->privC);
+    cudaFree(c->head);
+    cudaFree(c->stkA); cudaFree(c->stkB); cudaFree(c->stkC);
     for (auto &e : c->events) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
     delete c;
+}
+
+// Phantom -> device: pack {density, material}, validate, reduce rho_max per material, rebuild the
+// Woodcock majorants (H10) and upload the table blob.  Synchronous.
+//   mu_max(E_i) = max_m rho_max[m] mu_m(E_i) (Eq. 3);  M_e = running max in E of
+//   max_m rho_max[m] (Sigma_Moller + Sigma_brems) (L110-113 made rigorous).
+static int load_phantom(gpumcd_ctx *ctx, const float *density, const uint8_t *material, bool on_host)
+{
+    const size_t nvox = ctx->nvox;
+    const float *d_density = density;
+    const uint8_t *d_material = material;
+    if (on_host) {
+        if (!ctx->stage_density) {
+            CK(cudaMalloc(&ctx->stage_density, nvox * sizeof(float)));
+            CK(cudaMalloc(&ctx->stage_material, nvox));
+        }
+        CK(cudaMemcpyAsync(ctx->stage_density, density, nvox * sizeof(float), cudaMemcpyHostToDevice, nullptr));
+        CK(cudaMemcpyAsync(ctx->stage_material, material, nvox, cudaMemcpyHostToDevice, nullptr));
+        d_density = ctx->stage_density;
+        d_material = ctx->stage_material;
+    }
+    CK(cudaMemsetAsync(ctx->scratch, 0, 9 * sizeof(unsigned), nullptr));
+    const int grid = static_cast<int>(std::min<size_t>((nvox + kBlock - 1) / kBlock, 148 * 8));
+    k_pack_phantom<<<grid, kBlock>>>(d_density, d_material, nvox, ctx->n_mat, ctx->phantom, ctx->scratch, ctx->scratch + 8);
+    CK(cudaGetLastError());
+    unsigned h_scratch[9];
+    CK(cudaMemcpy(h_scratch, ctx->scratch, sizeof h_scratch, cudaMemcpyDeviceToHost));
+    if (h_scratch[8] != 0) {
+        set_error(ctx, "phantom has a material id >= n_materials or a density that is not a positive finite number");
+        return GPUMCD_ERR_INVALID_ARG;
+    }
+    double rho_max[8];
+    for (int m = 0; m < 8; ++m) { float f; memcpy(&f, &h_scratch[m], 4); rho_max[m] = f; }
+    const int nE = ctx->n_E, nM = ctx->n_mat;
+    const float *ph = ctx->blob_host.data(), *el = ph + ctx->tab.off_el;
+    float *mu_max = ctx->blob_host.data() + ctx->tab.off_mu, *m_e = ctx->blob_host.data() + ctx->tab.off_me;
+    double run = 0.0;
+    for (int i = 0; i < nE; ++i) {
+        double mu = 0.0, se = 0.0;
+        for (int m = 0; m < nM; ++m) {
+            const float *p = ph + static_cast<size_t>(m) * 3 * nE;
+            const float *e = el + static_cast<size_t>(m) * 4 * nE;
+            mu = std::max(mu, rho_max[m] * (static_cast<double>(p[i]) + p[nE + i] + p[2 * nE + i]));
+            se = std::max(se, rho_max[m] * (static_cast<double>(e[nE + i]) + e[2 * nE + i]));
+        }
+        run = std::max(run, se);
+        mu_max[i] = static_cast<float>(mu * ctx->opt.majorant_scale);
+        m_e[i] = static_cast<float>(run * ctx->opt.majorant_scale);
+    }
+    CK(cudaMemcpy(ctx->table_blob, ctx->blob_host.data(), ctx->blob_host.size() * sizeof(float), cudaMemcpyHostToDevice));
+    return GPUMCD_OK;
 }
 
 static int create_impl(gpumcd_ctx **out, const float *density, const uint8_t *material, bool on_host, int nx,
@@ -265,7 +326,7 @@ static int create_impl(gpumcd_ctx **out, const float *density, const uint8_t *ma
     gpumcd_default_options(&opt);
     if (opt_in) opt = *opt_in;
     if (!(opt.es_max_cm > 0.f) || !(opt.f_eloss_max > 0.f) || opt.f_eloss_max > 1.f || opt.boundary_nudge < 0.f ||
-        !(opt.majorant_scale >= 1.f) || opt.wave_size == 0 || opt.bank_factor == 0 ||
+        !(opt.majorant_scale >= 1.f) || opt.wave_size == 0 || opt.bank_factor == 0 || opt.warp_stack > (1u << 20) ||
         static_cast<unsigned long long>(opt.wave_size) * opt.bank_factor > 0x7fffffffull) {
         set_error(nullptr, "bad options");
         return GPUMCD_ERR_INVALID_ARG;
@@ -278,65 +339,15 @@ static int create_impl(gpumcd_ctx **out, const float *density, const uint8_t *ma
     const size_t nvox = ctx->nvox;
     const int nE = t->n_energy, nK = t->n_K, nM = t->n_materials;
 
-    // ---- phantom ----
-    const float *d_density = density;
-    const uint8_t *d_material = material;
-    float *tmp_density = nullptr;
-    uint8_t *tmp_material = nullptr;
-    if (on_host) {
-        CK(cudaMalloc(&tmp_density, nvox * sizeof(float)));
-        CK(cudaMalloc(&tmp_material, nvox));
-        CK(cudaMemcpy(tmp_density, density, nvox * sizeof(float), cudaMemcpyHostToDevice));
-        CK(cudaMemcpy(tmp_material, material, nvox, cudaMemcpyHostToDevice));
-        d_density = tmp_density;
-        d_material = tmp_material;
-    }
-    CK(cudaMalloc(&ctx->phantom, nvox * sizeof(float2)));
-    unsigned *d_scratch = nullptr;
-    CK(cudaMalloc(&d_scratch, 9 * sizeof(unsigned)));
-    CK(cudaMemset(d_scratch, 0, 9 * sizeof(unsigned)));
-    {
-        const int grid = static_cast<int>(std::min<size_t>((nvox + kBlock - 1) / kBlock, 148 * 8));
-        k_pack_phantom<<<grid, kBlock>>>(d_density, d_material, nvox, nM, ctx->phantom, d_scratch, d_scratch + 8);
-        CK(cudaGetLastError());
-    }
-    unsigned h_scratch[9];
-    CK(cudaMemcpy(h_scratch, d_scratch, sizeof h_scratch, cudaMemcpyDeviceToHost));
-    cudaFree(d_scratch);
-    cudaFree(tmp_density);
-    cudaFree(tmp_material);
-    if (h_scratch[8] != 0) {
-        set_error(ctx, "phantom has a material id >= n_materials or a density that is not a positive finite number");
-        return GPUMCD_ERR_INVALID_ARG;
-    }
-    double rho_max[8];
-    for (int m = 0; m < 8; ++m) { float f; memcpy(&f, &h_scratch[m], 4); rho_max[m] = f; }
-
-    // ---- tables: one device blob = photon | electron | mu_max | m_e | ms_a ----
-    // H10 majorants: mu_max(E_i) = max_m rho_max[m] mu_m(E_i) (Eq. 3); M_e = running max in E of
-    // max_m rho_max[m] (Sigma_Moller + Sigma_brems) (L110-113 made rigorous).
+    // ---- tables: one device blob = photon | electron | mu_max | m_e | ms_a (majorants filled per phantom) ----
     const size_t n_ph = static_cast<size_t>(nM) * 3 * nE, n_el = static_cast<size_t>(nM) * 4 * nE;
     const size_t blob_len = n_ph + n_el + 2 * static_cast<size_t>(nE) + nK;
-    std::vector<float> blob((blob_len + 3) & ~static_cast<size_t>(3), 0.0f); // padded for 16-byte bulk copies
-    memcpy(blob.data(), t->photon, n_ph * sizeof(float));
-    memcpy(blob.data() + n_ph, t->electron, n_el * sizeof(float));
-    float *mu_max = blob.data() + n_ph + n_el, *m_e = mu_max + nE;
-    double run = 0.0;
-    for (int i = 0; i < nE; ++i) {
-        double mu = 0.0, se = 0.0;
-        for (int m = 0; m < nM; ++m) {
-            const float *p = t->photon + static_cast<size_t>(m) * 3 * nE;
-            const float *e = t->electron + static_cast<size_t>(m) * 4 * nE;
-            mu = std::max(mu, rho_max[m] * (static_cast<double>(p[i]) + p[nE + i] + p[2 * nE + i]));
-            se = std::max(se, rho_max[m] * (static_cast<double>(e[nE + i]) + e[2 * nE + i]));
-        }
-        run = std::max(run, se);
-        mu_max[i] = static_cast<float>(mu * opt.majorant_scale);
-        m_e[i] = static_cast<float>(run * opt.majorant_scale);
-    }
-    memcpy(m_e + nE, t->ms_a, static_cast<size_t>(nK) * sizeof(float));
-    CK(cudaMalloc(&ctx->table_blob, blob.size() * sizeof(float)));
-    CK(cudaMemcpy(ctx->table_blob, blob.data(), blob.size() * sizeof(float), cudaMemcpyHostToDevice));
+    ctx->blob_host.assign((blob_len + 3) & ~static_cast<size_t>(3), 0.0f); // padded for 16-byte bulk copies
+    memcpy(ctx->blob_host.data(), t->photon, n_ph * sizeof(float));
+    memcpy(ctx->blob_host.data() + n_ph, t->electron, n_el * sizeof(float));
+    memcpy(ctx->blob_host.data() + n_ph + n_el + 2 * static_cast<size_t>(nE), t->ms_a, static_cast<size_t>(nK) * sizeof(float));
+    ctx->n_mat = nM; ctx->n_E = nE;
+    CK(cudaMalloc(&ctx->table_blob, ctx->blob_host.size() * sizeof(float)));
     Tables &tb = ctx->tab;
     tb.blob = ctx->table_blob;
     tb.off_el = static_cast<unsigned>(n_ph);
@@ -352,13 +363,21 @@ static int create_impl(gpumcd_ctx **out, const float *density, const uint8_t *ma
     tb.e_min = t->e_min; tb.e_cut = t->e_cut; tb.p_cut = t->p_cut;
     ctx->e_max = t->e_max;
     tb.n_mat = nM;
-    ctx->table_floats = static_cast<unsigned>(blob.size());
+    ctx->table_floats = static_cast<unsigned>(ctx->blob_host.size());
+
+    // ---- phantom (and the majorants that depend on it) ----
+    CK(cudaMalloc(&ctx->phantom, nvox * sizeof(float2)));
+    CK(cudaMalloc(&ctx->scratch, 9 * sizeof(unsigned)));
+    {
+        const int rc = load_phantom(ctx, density, material, on_host);
+        if (rc != GPUMCD_OK) return rc;
+    }
 
     // ---- tally, counters, queues ----
     CK(cudaMalloc(&ctx->edep, nvox * sizeof(double)));
     CK(cudaMalloc(&ctx->cnt, sizeof(DevCounters)));
     CK(cudaMalloc(&ctx->qcount, kMaxQueues * sizeof(unsigned)));
-    ctx->n_queues = opt.scheduler == 1 ? 6 : 4;
+    ctx->n_queues = opt.scheduler == 1 ? 0 : 4;
     ctx->qcap = opt.wave_size * opt.bank_factor;
     for (int k = 0; k < ctx->n_queues; ++k) {
         CK(cudaMalloc(&ctx->qA[k], static_cast<size_t>(ctx->qcap) * sizeof(float4)));
@@ -388,13 +407,14 @@ static int create_impl(gpumcd_ctx **out, const float *density, const uint8_t *ma
             CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_persistent<false, false>, kPThreads, 0));
         if (per_sm < 1) { set_error(ctx, "persistent kernel does not fit on an SM"); return GPUMCD_ERR_CUDA; }
         ctx->p_grid = n_sm; // one CTA per SM
-        ctx->priv_ready = 1024;
+        ctx->cap_r = std::max(opt.warp_stack, kMustMargin + 32u);
+        ctx->stride = 2 * ctx->cap_r + 2 * kPend;
         const size_t n_warps = static_cast<size_t>(ctx->p_grid) * (kPThreads / 32);
-        const size_t recs = n_warps * (ctx->priv_ready + kHardCap);
-        CK(cudaMalloc(&ctx->privA, recs * sizeof(float4)));
-        CK(cudaMalloc(&ctx->privB, recs * sizeof(float4)));
-        CK(cudaMalloc(&ctx->privC, recs * sizeof(uint4)));
-        CK(cudaMalloc(&ctx->heads, kMaxQueues * sizeof(unsigned)));
+        const size_t recs = n_warps * ctx->stride;
+        CK(cudaMalloc(&ctx->stkA, recs * sizeof(float4)));
+        CK(cudaMalloc(&ctx->stkB, recs * sizeof(float4)));
+        CK(cudaMalloc(&ctx->stkC, recs * sizeof(uint4)));
+        CK(cudaMalloc(&ctx->head, sizeof(unsigned)));
     }
     CK(cudaDeviceSynchronize());
     guard.ok = true;
@@ -413,6 +433,20 @@ extern "C" int gpumcd_create_host(gpumcd_ctx **out, const float *density_host, c
                                   const gpumcd_options *opt)
 {
     return create_impl(out, density_host, material_host, true, nx, ny, nz, voxel_cm, tables, opt);
+}
+
+extern "C" int gpumcd_set_phantom_host(gpumcd_ctx *ctx, const float *density_host, const uint8_t *material_host)
+{
+    if (!ctx || !density_host || !material_host) return GPUMCD_ERR_INVALID_ARG;
+    if (ctx->ran) CK(cudaStreamSynchronize(ctx->last_stream)); // the last run still reads the old phantom
+    return load_phantom(ctx, density_host, material_host, true);
+}
+
+extern "C" int gpumcd_set_phantom(gpumcd_ctx *ctx, const float *density_dev, const uint8_t *material_dev)
+{
+    if (!ctx || !density_dev || !material_dev) return GPUMCD_ERR_INVALID_ARG;
+    if (ctx->ran) CK(cudaStreamSynchronize(ctx->last_stream));
+    return load_phantom(ctx, density_dev, material_dev, false);
 }
 
 extern "C" int gpumcd_set_source(gpumcd_ctx *ctx, const gpumcd_source *s)
@@ -548,23 +582,22 @@ static int run_waves_host_loop(gpumcd_ctx *ctx, uint64_t n_hist, uint64_t seed, 
 static int run_persistent(gpumcd_ctx *ctx, uint64_t n_hist, uint64_t seed, float *dose_dev, unsigned long long *trace,
                           cudaStream_t st)
 {
-    CK(cudaMemsetAsync(ctx->qcount, 0, kMaxQueues * sizeof(unsigned), st));
-    CK(cudaMemsetAsync(ctx->heads, 0, kMaxQueues * sizeof(unsigned), st));
     const double h3 = static_cast<double>(ctx->h) * ctx->h * ctx->h;
     uint64_t h0 = ctx->hist_offset;
     const uint64_t h_end = ctx->hist_offset + n_hist;
     while (h0 < h_end) {
-        const uint64_t n = std::min<uint64_t>(h_end - h0, 0x100000000ull - (h0 & 0xffffffffull));
+        uint64_t n = std::min<uint64_t>(h_end - h0, 0x100000000ull - (h0 & 0xffffffffull));
+        n = std::min<uint64_t>(n, 0x80000000ull); // the claim counter is 32 bits wide
         PersistArgs a{};
         a.P = make_params(ctx, seed, static_cast<uint32_t>(h0 >> 32), trace != nullptr, trace);
         a.S = ctx->src;
-        for (int k = 0; k < 3; ++k) { a.qP[k] = make_queue(ctx, k); a.qE[k] = make_queue(ctx, 3 + k); }
-        a.heads = ctx->heads;
-        a.privA = ctx->privA; a.privB = ctx->privB; a.privC = ctx->privC;
-        a.priv_ready = ctx->priv_ready;
+        CK(cudaMemsetAsync(ctx->head, 0, sizeof(unsigned), st));
+        a.head = ctx->head;
+        a.stkA = ctx->stkA; a.stkB = ctx->stkB; a.stkC = ctx->stkC;
+        a.cap_r = ctx->cap_r;
+        a.stride = ctx->stride;
         a.hist0 = h0;
-        a.n_hist = n;
-        a.wave = ctx->opt.wave_size;
+        a.n_hist = static_cast<unsigned>(n);
         a.table_floats = ctx->table_floats;
         a.inv_h3_n = 1.0 / (h3 * static_cast<double>(n_hist));
         a.dose = dose_dev;
@@ -621,15 +654,14 @@ extern "C" int gpumcd_run_host(gpumcd_ctx *ctx, uint64_t n_histories, uint64_t s
 {
     if (!ctx || !dose_out_host) return GPUMCD_ERR_INVALID_ARG;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-    float *tmp = nullptr;
-    CK(cudaMalloc(&tmp, ctx->nvox * sizeof(float)));
+    if (!ctx->dose_stage) CK(cudaMalloc(&ctx->dose_stage, ctx->nvox * sizeof(float)));
+    float *tmp = ctx->dose_stage;
     int rc = run_impl(ctx, n_histories, seed, tmp, nullptr, st);
     if (rc == GPUMCD_OK) {
         cudaError_t e = cudaMemcpyAsync(dose_out_host, tmp, ctx->nvox * sizeof(float), cudaMemcpyDeviceToHost, st);
         if (e == cudaSuccess) e = cudaStreamSynchronize(st);
         if (e != cudaSuccess) { set_error(ctx, cudaGetErrorString(e)); rc = GPUMCD_ERR_CUDA; }
     }
-    cudaFree(tmp);
     return rc;
 }
 
@@ -654,7 +686,7 @@ extern "C" int gpumcd_get_counters(gpumcd_ctx *ctx, gpumcd_counters *out)
     out->photon_photo = d.photon_photo; out->photon_pair = d.photon_pair; out->photon_fict = d.photon_fict;
     out->ch_steps = d.ch_steps; out->hard_moller = d.hard_moller; out->hard_brems = d.hard_brems;
     out->hard_fict = d.hard_fict; out->pushes_e = d.pushes_e; out->pushes_g = d.pushes_g;
-    out->bank_high_water = ctx->high_water;
+    out->bank_high_water = ctx->opt.scheduler == 1 ? d.high_water : ctx->high_water;
     out->overflow_count = d.overflow;
     for (int k = 0; k < kEnergySlots; ++k) {
         out->e_incident += d.slot[k].e_inc;
@@ -708,12 +740,3 @@ extern "C" const char *gpumcd_last_error(gpumcd_ctx *ctx)
 }
 
 extern "C" void gpumcd_destroy(gpumcd_ctx *ctx) { destroy_impl(ctx); }
-
-#ifdef GPUMCD_TIMELINE
-// development aid (only with -DGPUMCD_TIMELINE): copy the phase timeline of the last persistent launch
-extern "C" int gpumcd_debug_timeline(void *host_out, size_t bytes)
-{
-    if (bytes < sizeof(Timeline)) return static_cast<int>(sizeof(Timeline));
-    return cudaMemcpyFromSymbol(host_out, g_timeline, sizeof(Timeline)) == cudaSuccess ? 0 : -2;
-}
-#endif

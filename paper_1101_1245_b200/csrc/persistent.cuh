@@ -1,19 +1,24 @@
-// persistent.cuh -- scheduler 1: one persistent cooperative kernel per gpumcd_run (H7).
+// persistent.cuh -- scheduler 1: one persistent kernel per gpumcd_run, warp-autonomous (H7).
 //
 // The paper alternates one launch per particle type until both lists are empty
 // and reports small gains from stream compaction and a persistent "pool" (L180-182, Tab. VI).
-// On B200 the transport kernels are issue-bound with most lanes idle (profiles/r01_*), so the
-// scheduler is built around keeping all 32 lanes of a warp in the SAME code:
-//   * one CTA per SM stays resident for the whole run; tables are staged into shared memory once
-//     with TMA bulk copies (cp.async.bulk + mbarrier);
-//   * a warp steps 32 particles in lock step and refills finished lanes at once, first from its
-//     private stack of same-type secondaries, then from the phase's input queue (atomic head);
-//   * electrons whose step ended on a hard-event candidate are swapped out into a per-warp buffer
-//     and processed 32 at a time (event-based sorting), so neither the step code nor the
-//     Moller / bremsstrahlung samplers run with a handful of active lanes;
-//   * photons born in an electron phase and electrons born in a photon phase go to global queues
-//     (ballot + popc prefix, one atomic per warp) that the next phase consumes; phases are separated
-//     by grid-wide barriers, so a queue is never read and written at the same time.
+// Here every warp of one resident CTA per SM is a small event-driven simulator of its own:
+//   * it owns four type-sorted stacks of particle records (global memory, L2-resident tops):
+//       ES electrons due a condensed-history step      EH electrons waiting for a hard event
+//       GS photons due a flight                        GI photons waiting for an interaction
+//     so no queue is shared between warps, no push needs a global atomic, and there is no grid-wide
+//     barrier between particle types: the only shared counter is the head of the primary source;
+//   * its 32 lanes hold particles of one type and run ONE piece of code per iteration: the step /
+//     flight code for all lanes, or, once 32 records wait (or nothing else is left), the hard-event /
+//     interaction code for 32 waiting records.  A lane whose particle needs the other code swaps it
+//     out to the waiting stack and takes the next ready record (stack first, then a primary), so the
+//     long step code and the rejection samplers both run with full warps ("grouping particles",
+//     L352; compaction by ballot + popc prefix sums);
+//   * secondaries of the other type pile up in that type's stack; the warp changes type when that
+//     stack passes a high-water mark or its own type runs dry, parking the particles in flight;
+//   * tables are staged into shared memory once with TMA bulk copies (cp.async.bulk + mbarrier).
+// A particle's random stream depends only on its lineage (physics.cuh), so the order in which a
+// warp works through its stacks does not change any history.
 #pragma once
 
 #include <cooperative_groups.h>
@@ -25,12 +30,22 @@ namespace gpumcd {
 namespace cg = cooperative_groups;
 
 #ifndef GPUMCD_PTHREADS
-#define GPUMCD_PTHREADS 512
+#define GPUMCD_PTHREADS 1024
+#endif
+#ifndef GPUMCD_HIGH
+#define GPUMCD_HIGH 512
+#endif
+#ifndef GPUMCD_LOW
+#define GPUMCD_LOW 24
 #endif
 constexpr int kPThreads = GPUMCD_PTHREADS; // threads per persistent CTA (one CTA per SM)
-constexpr unsigned kHardCap = 64; // per-warp buffer of pending hard events
+constexpr int kPWarps = kPThreads / 32;
 constexpr unsigned kFull = 0xffffffffu;
-constexpr unsigned kChunk = 32;   // inputs a warp claims per atomic on the phase's head counter
+constexpr unsigned kChunk = 32;            // primaries a warp claims per atomic on the source head
+constexpr unsigned kPend = 64;             // capacity of a waiting stack (EH, GI): < 32 before a move, + 32 after
+constexpr unsigned kHigh = GPUMCD_HIGH;    // other-type records that make a warp change type
+constexpr unsigned kLow = GPUMCD_LOW;      // own-type particles below which a warp with no source changes type
+constexpr unsigned kMustMargin = 160;      // a ready stack within this many records of its capacity forces the change
 
 struct SourceDev {
     int particle, shape;
@@ -112,19 +127,18 @@ __device__ __forceinline__ void stage_tables(float *dst, const float *src, unsig
     }
 }
 
+
 struct PersistArgs {
     Params P;
     SourceDev S;
-    Queue qP[3];       // photon queues, rotating: read [i%3], written [(i+1)%3], reset [(i+2)%3]
-    Queue qE[3];       // electron queues, same rotation
-    unsigned *heads;   // pop heads: [0..2] photon queues, [3..5] electron queues
-    float4 *privA;     // per-warp private records: ready stack [priv_ready] then hard buffer [kHardCap]
-    float4 *privB;
-    uint4 *privC;
-    unsigned priv_ready;           // capacity of a warp's ready stack
-    unsigned long long hist0;      // first history of the run (low word never wraps inside a launch)
-    unsigned long long n_hist;
-    unsigned wave;
+    unsigned *head;    // next primary of this launch to be claimed (the only counter the warps share)
+    float4 *stkA;      // per-warp stacks, `stride` records per warp: [ES cap_r | GS cap_r | EH kPend | GI kPend]
+    float4 *stkB;
+    uint4 *stkC;
+    unsigned cap_r;                // capacity of a ready stack (ES, GS)
+    unsigned stride;               // 2 cap_r + 2 kPend
+    unsigned long long hist0;      // first history of the launch (low word never wraps inside a launch)
+    unsigned n_hist;               // histories of the launch (< 2^32)
     unsigned table_floats;         // length of the table blob, padded to a multiple of 4 floats
     double inv_h3_n;
     float *dose;                   // or nullptr
@@ -132,262 +146,278 @@ struct PersistArgs {
     int finalize;                  // 0 for all but the last launch of a run split at a 2^32 history boundary
 };
 
-// ---------------------------------------------------------------------------------------------
-// Photon phase: every warp steps 32 photons; finished lanes are refilled from the input.
-// SRC: the input is the source itself (primaries generated on the fly), else queue `in`.
-// Event counts are warp-level (ballot + popc into warp-uniform counters): no per-lane registers.
-// ---------------------------------------------------------------------------------------------
-template <bool TRACE, bool SRC>
-__device__ void photon_phase(const Params &P, const float *__restrict__ TB, const SourceDev &S,
-                             unsigned long long hist_base, const Queue &in, unsigned n_queue, unsigned n_in,
-                             unsigned *head, const Queue &qE, const Queue &qG)
-{
-    const int lane = threadIdx.x & 31;
-    const unsigned lt = (1u << lane) - 1u;
-    const Acc acc(P);
-    Particle p;
-    Trace tr;
-    bool alive = false, exhausted = (n_in == 0);
-    unsigned n_flight = 0, n_compton = 0, n_photo = 0, n_pair = 0, n_fict = 0;
-    unsigned w_next = 0, w_end = 0; // this warp's chunk of the input, [w_next, w_end)
-    for (;;) {
-        const unsigned dead = __ballot_sync(kFull, !alive);
-        if (dead && !(exhausted && w_next == w_end)) {
-            if (w_next == w_end) { // take the next chunk of kChunk inputs: one atomic per chunk
-                unsigned base = 0;
-                if (lane == 0) base = atomicAdd(head, kChunk);
-                base = __shfl_sync(kFull, base, 0);
-                w_next = min(base, n_in);
-                w_end = min(base + kChunk, n_in);
-                if (base + kChunk >= n_in) exhausted = true;
+// Event counters of one warp, in shared memory (lane 0 adds ballot counts; flushed once per kernel).
+// DevCounters lists its first eleven members in this order.
+enum : int { WC_FLIGHT = 0, WC_COMPTON, WC_PHOTO, WC_PAIR, WC_FICT, WC_STEP, WC_MOLLER, WC_BREMS, WC_HFICT,
+             WC_PUSH_E, WC_PUSH_G, WC_N };
+enum : int { SK_ES = 0, SK_GS = 1, SK_EH = 2, SK_GI = 3 };
+
+struct WarpCtl {          // one per warp, shared memory
+    unsigned n_es, n_gs;  // stack counts while divergent code pushes (photon_interact); else in registers
+    unsigned wc[WC_N];
+};
+
+// This warp's next chunk of the primary source: [next, end) out of [0, n_in); one atomic per chunk.
+struct Claim {
+    unsigned next = 0, end = 0;
+    bool exhausted = false;
+    __device__ __forceinline__ bool empty() const { return exhausted && next == end; }
+    __device__ __forceinline__ void refill(unsigned *head, unsigned n_in)
+    {
+        if (next != end || exhausted) return;
+        unsigned base = 0;
+        if ((threadIdx.x & 31) == 0) base = atomicAdd(head, kChunk);
+        base = __shfl_sync(kFull, base, 0);
+        next = min(base, n_in);
+        end = min(base + kChunk, n_in);
+        if (base + kChunk >= n_in) exhausted = true;
+    }
+};
+
+// The calling warp: its stacks, their counts (warp-uniform registers) and its shared-memory block.
+struct Warp {
+    float4 *A;
+    float4 *B;
+    uint4 *C;
+    unsigned cap_r;
+    unsigned n[4];
+    unsigned lt;   // lanes below this one
+    unsigned hw;   // fullest ready stack seen
+    WarpCtl *ctl;
+    double *e_inc; // this thread's account of the primaries' energy (shared memory)
+
+    __device__ __forceinline__ unsigned off(int s) const
+    {
+        return s == SK_ES ? 0u : (s == SK_GS ? cap_r : (s == SK_EH ? 2u * cap_r : 2u * cap_r + kPend));
+    }
+    __device__ __forceinline__ unsigned cap(int s) const { return s < 2 ? cap_r : kPend; }
+    __device__ __forceinline__ void count(int k, unsigned mask) const
+    {
+        if ((threadIdx.x & 31) == 0 && mask) ctl->wc[k] += static_cast<unsigned>(__popc(mask));
+    }
+    // Converged code: the lanes with `on` append their record to stack s (ballot + popc prefix).
+    __device__ __forceinline__ unsigned push(const Params &P, int s, bool on, const Particle &c, uint32_t extra)
+    {
+        const unsigned m = __ballot_sync(kFull, on);
+        if (m) {
+            if (on) {
+                const unsigned slot = n[s] + __popc(m & lt);
+                if (slot < cap(s)) store_rec(A, B, C, off(s) + slot, c, extra);
+                else atomicAdd(&P.cnt->overflow, 1ull);
             }
-            const unsigned take = min(static_cast<unsigned>(__popc(dead)), w_end - w_next);
-            const unsigned rank = __popc(dead & lt);
-            double e_new = 0.0;
-            if (!alive && rank < take) {
-                const unsigned idx = w_next + rank;
-                uint32_t extra;
-                if (SRC && idx >= n_queue) {
-                    p = make_primary(P, S, hist_base + (idx - n_queue));
-                    e_new = static_cast<double>(p.E);
-                } else {
-                    p = load_rec(in.A, in.B, in.C, idx, extra);
-                }
-                alive = true;
-                tr = Trace{};
-            }
-            w_next += take;
-            if (SRC) {
-                e_new = wsum(e_new);
-                if (lane == 0 && e_new != 0.0) acc.inc(e_new);
-            }
+            n[s] = min(n[s] + static_cast<unsigned>(__popc(m)), cap(s));
+            __syncwarp(); // the records are read back by other lanes of this warp
         }
-        const unsigned am = __ballot_sync(kFull, alive);
-        if (am == 0u) {
-            if (exhausted && w_next == w_end) break;
+        return m;
+    }
+    // Converged code: the lanes with `want` take the top records of stack s while there are any.
+    __device__ __forceinline__ bool pop(int s, bool want, Particle &p, uint32_t &extra)
+    {
+        const unsigned m = __ballot_sync(kFull, want);
+        const unsigned take = min(static_cast<unsigned>(__popc(m)), n[s]);
+        const unsigned rank = __popc(m & lt);
+        const bool got = want && rank < take;
+        if (got) p = load_rec(A, B, C, off(s) + n[s] - 1u - rank, extra);
+        n[s] -= take;
+        return got;
+    }
+    // Converged code: the lanes with `want` take the next primaries of the source (H0).
+    __device__ __forceinline__ bool primaries(const PersistArgs &a, Claim &cl, bool want, Particle &p)
+    {
+        cl.refill(a.head, a.n_hist);
+        const unsigned m = __ballot_sync(kFull, want);
+        const unsigned take = min(static_cast<unsigned>(__popc(m)), cl.end - cl.next);
+        const unsigned rank = __popc(m & lt);
+        const bool got = want && rank < take;
+        if (got) {
+            p = make_primary(a.P, a.S, a.hist0 + (cl.next + rank));
+            *e_inc += static_cast<double>(p.E);
+        }
+        cl.next += take;
+        return got;
+    }
+};
+
+// ---------------------------------------------------------------------------------------------
+// Electron mode: the lanes hold electrons due a condensed-history step.  Returns the type to go on
+// with (0 photons, 1 electrons never, -1 nothing left); on return no lane holds a particle.
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ int electron_mode(const PersistArgs &a, const float *__restrict__ TB, Warp &w, Claim &cl)
+{
+    const Params &P = a.P;
+    const unsigned lane = threadIdx.x & 31;
+    const bool src_is_e = a.S.particle == 1;
+    Particle p;
+    float lnT = 0.f, M = 0.f;
+    bool alive = false;
+    for (;;) {
+        const unsigned live = __ballot_sync(kFull, alive);
+        const bool src_e = src_is_e && !cl.empty();
+        // ---- hard events of 32 waiting electrons (or of what is left when nothing else can move)
+        if (w.n[SK_EH] >= 32u || (w.n[SK_EH] != 0u && live == 0u && w.n[SK_ES] == 0u && !src_e)) {
+            w.push(P, SK_ES, alive, p, 0u); // park the electrons in flight
+            alive = false;
+            const unsigned nb = min(32u, w.n[SK_EH]);
+            Particle c;
+            int kind = -1;
+            if (lane < nb) {
+                uint32_t mbits;
+                p = load_rec(w.A, w.B, w.C, w.off(SK_EH) + w.n[SK_EH] - 1u - lane, mbits);
+                lnT = flog(p.E);
+                alive = electron_hard(P, TB, p, lnT, __uint_as_float(mbits), c, kind) == ST_ALIVE;
+            }
+            w.n[SK_EH] -= nb;
+            __syncwarp();
+            const unsigned gm = w.push(P, SK_GS, kind == HK_BREMS, c, 0u);  // bremsstrahlung photons
+            const unsigned em = w.push(P, SK_ES, kind == HK_MOLLER, c, 0u); // knock-on electrons
+            w.count(WC_MOLLER, em);
+            w.count(WC_BREMS, gm);
+            w.count(WC_PUSH_E, em);
+            w.count(WC_PUSH_G, gm);
+            w.count(WC_HFICT, __ballot_sync(kFull, kind == HK_FICT));
+            w.hw = max(w.hw, max(w.n[SK_ES], w.n[SK_GS]));
             continue;
         }
-        int ev = -1;
-        if (alive) {
-            ev = photon_step<TRACE>(P, TB, p, acc, qE, qG, tr);
-            if (!photon_alive(ev)) {
-                write_trace<TRACE>(P, p, tr);
-                alive = false;
+        // ---- change of particle type?  (E, G: all electrons / photons this warp holds; both are
+        // unchanged by parking, and the two modes' rules exclude each other, so a change is never
+        // undone before some work has been done)
+        const unsigned ready = static_cast<unsigned>(__popc(live)) + w.n[SK_ES];
+        const unsigned E = ready + w.n[SK_EH], G = w.n[SK_GS] + w.n[SK_GI];
+        const unsigned must = w.cap_r - kMustMargin;
+        const bool src_g = !src_is_e && !cl.empty();
+        bool leave = G >= kHigh && (E < kHigh || (G >= must && E < must));
+        if (!src_e) {
+            if (ready == 0u) return (G != 0u || src_g) ? 0 : -1; // (EH is empty here)
+            leave = leave || (ready < kLow && (src_g || w.n[SK_GS] >= 32u));
+        }
+        if (leave) {
+            w.push(P, SK_ES, alive, p, 0u);
+            w.hw = max(w.hw, w.n[SK_ES]);
+            return 0;
+        }
+        // ---- refill the free lanes: the stack first (depth first keeps it short), then primaries
+        if (~live) {
+            uint32_t extra;
+            bool got = w.pop(SK_ES, !alive, p, extra);
+            if (src_e && __any_sync(kFull, !alive && !got)) {
+                if (w.primaries(a, cl, !alive && !got, p)) {
+                    if (electron_tracked(P, p.E)) {
+                        got = true;
+                    } else { // below the cutoff (or photon_only): deposited where it is born
+                        deposit(P, voxel_index(P.geo, p), p.E);
+                        Acc(P).cut(p.E);
+                    }
+                }
+            }
+            if (got) {
+                lnT = flog(p.E);
+                alive = true;
             }
         }
-        n_flight += __popc(am);
-        n_compton += __popc(__ballot_sync(kFull, ev == PH_COMPTON || ev == PH_ABSORBED));
-        n_photo += __popc(__ballot_sync(kFull, ev == PH_PHOTO));
-        n_pair += __popc(__ballot_sync(kFull, ev == PH_PAIR));
-        n_fict += __popc(__ballot_sync(kFull, ev == PH_FICT));
-    }
-    if (lane == 0) {
-        DevCounters *c = P.cnt;
-        bump(&c->photon_flights, n_flight); bump(&c->photon_compton, n_compton); bump(&c->photon_photo, n_photo);
-        bump(&c->photon_pair, n_pair); bump(&c->photon_fict, n_fict);
+        const unsigned sm = __ballot_sync(kFull, alive);
+        if (sm == 0u) continue;
+        // ---- one condensed-history step for every lane that holds an electron
+        int st = ST_ALIVE;
+        if (alive) st = electron_step(P, TB, p, lnT, M);
+        w.count(WC_STEP, sm);
+        w.push(P, SK_EH, alive && st == ST_HARD, p, __float_as_uint(M));
+        if (st != ST_ALIVE) alive = false;
     }
 }
 
 // ---------------------------------------------------------------------------------------------
-// Electron phase: lock-step condensed-history steps with lane refill and event-sorted hard events.
+// Photon mode: the lanes hold photons due a flight.  Returns the type to go on with (1 electrons,
+// -1 nothing left); on return no lane holds a particle.
 // ---------------------------------------------------------------------------------------------
-template <bool SRC>
-__device__ void electron_phase(const Params &P, const float *__restrict__ TB, const SourceDev &S,
-                               unsigned long long hist_base, const Queue &in, unsigned n_queue, unsigned n_in,
-                               unsigned *head, const Queue &qG, float4 *pA, float4 *pB, uint4 *pC,
-                               unsigned ready_cap)
+template <bool TRACE>
+__device__ __forceinline__ int photon_mode(const PersistArgs &a, const float *__restrict__ TB, Warp &w, Claim &cl)
 {
-    const int lane = threadIdx.x & 31;
-    const unsigned lt = (1u << lane) - 1u;
-    const Acc acc(P);
-    // private records of this warp: [0, ready_cap) ready stack (extra word = ln T),
-    // [ready_cap, ready_cap + kHardCap) pending hard events (extra word = majorant M)
+    const Params &P = a.P;
+    const unsigned lane = threadIdx.x & 31;
+    const bool src_is_g = a.S.particle == 0;
     Particle p;
-    float lnT = 0.f, M = 0.f;
-    bool alive = false, exhausted = (n_in == 0);
-    unsigned n_ready = 0, n_hard = 0;
-    unsigned n_step = 0, n_moller = 0, n_brems = 0, n_hfict = 0;
-    unsigned w_next = 0, w_end = 0; // this warp's chunk of the input, [w_next, w_end)
+    bool alive = false;
     for (;;) {
-        // ---- refill dead lanes: private stack first, then the phase input
-        const unsigned dead = __ballot_sync(kFull, !alive);
-        if (dead) {
-            const unsigned k = __popc(dead), rank = __popc(dead & lt);
-            const unsigned take = min(k, n_ready);
-            if (!alive && rank < take) {
-                uint32_t extra;
-                p = load_rec(pA, pB, pC, n_ready - 1u - rank, extra);
-                lnT = __uint_as_float(extra);
-                alive = true;
+        const unsigned live = __ballot_sync(kFull, alive);
+        const bool src_g = src_is_g && !cl.empty();
+        // ---- interactions of 32 waiting photons (or of what is left when nothing else can move)
+        if (w.n[SK_GI] >= 32u || (w.n[SK_GI] != 0u && live == 0u && w.n[SK_GS] == 0u && !src_g)) {
+            w.push(P, SK_GS, alive, p, 0u); // park the photons in flight
+            alive = false;
+            const unsigned nb = min(32u, w.n[SK_GI]);
+            // the interaction code pushes from divergent branches: the two ready stacks' counts go
+            // through shared memory for its duration
+            if (lane == 0) {
+                w.ctl->n_es = w.n[SK_ES];
+                w.ctl->n_gs = w.n[SK_GS];
             }
-            n_ready -= take;
-            if (k > take && !(exhausted && w_next == w_end)) {
-                if (w_next == w_end) { // next chunk of the input: one atomic per kChunk particles
-                    unsigned base = 0;
-                    if (lane == 0) base = atomicAdd(head, kChunk);
-                    base = __shfl_sync(kFull, base, 0);
-                    w_next = min(base, n_in);
-                    w_end = min(base + kChunk, n_in);
-                    if (base + kChunk >= n_in) exhausted = true;
-                }
-                const unsigned take2 = min(k - take, w_end - w_next);
-                double e_new = 0.0;
-                if (!alive && rank >= take && rank - take < take2) {
-                    const unsigned idx = w_next + rank - take;
-                    uint32_t extra;
-                    if (SRC && idx >= n_queue) {
-                        p = make_primary(P, S, hist_base + (idx - n_queue));
-                        e_new = static_cast<double>(p.E);
-                        if (electron_tracked(P, p.E)) {
-                            alive = true;
-                        } else { // below the cutoff (or photon_only): deposited where it is born
-                            deposit(P, voxel_index(P.geo, p), p.E);
-                            acc.cut(p.E);
-                        }
-                    } else {
-                        p = load_rec(in.A, in.B, in.C, idx, extra);
-                        alive = true;
-                    }
-                    lnT = flog(p.E);
-                }
-                w_next += take2;
-                if (SRC) {
-                    e_new = wsum(e_new);
-                    if (lane == 0 && e_new != 0.0) acc.inc(e_new);
-                }
+            __syncwarp();
+            int kind = 0;
+            if (lane < nb) {
+                uint32_t kbits;
+                p = load_rec(w.A, w.B, w.C, w.off(SK_GI) + w.n[SK_GI] - 1u - lane, kbits);
+                kind = static_cast<int>(kbits);
+                const WarpStack qE{w.A + w.off(SK_ES), w.B + w.off(SK_ES), w.C + w.off(SK_ES), &w.ctl->n_es,
+                                   &w.ctl->wc[WC_PUSH_E], w.cap_r};
+                const WarpStack qG{w.A + w.off(SK_GS), w.B + w.off(SK_GS), w.C + w.off(SK_GS), &w.ctl->n_gs,
+                                   &w.ctl->wc[WC_PUSH_G], w.cap_r};
+                alive = photon_interact<TRACE>(P, p, kind, qE, qG) == PM_FLIGHT;
             }
-        }
-        const unsigned am = __ballot_sync(kFull, alive);
-        // ---- hard events, 32 at a time (or whatever is left when nothing else can run)
-        if (n_hard >= 32u || (n_hard > 0u && am == 0u && n_ready == 0u && exhausted && w_next == w_end)) {
-            const unsigned nb = min(32u, n_hard);
-            Particle q, c;
-            float qlnT = 0.f;
-            int st = ST_DEAD, kind = -1;
-            if (static_cast<unsigned>(lane) < nb) {
-                uint32_t mbits;
-                q = load_rec(pA, pB, pC, ready_cap + n_hard - 1u - lane, mbits);
-                qlnT = flog(q.E);
-                st = electron_hard(P, TB, q, qlnT, __uint_as_float(mbits), acc, c, kind);
-            }
-            n_hard -= nb;
-            // bremsstrahlung photons -> global photon queue of the next photon phase
-            const unsigned gm = __ballot_sync(kFull, kind == HK_BREMS);
-            if (gm) {
-                unsigned base = 0;
-                if (lane == 0) base = atomicAdd(qG.count, static_cast<unsigned>(__popc(gm)));
-                base = __shfl_sync(kFull, base, 0);
-                if (kind == HK_BREMS) {
-                    const unsigned slot = base + __popc(gm & lt);
-                    if (slot < qG.cap) store_rec(qG.A, qG.B, qG.C, slot, c, 0u);
-                    else atomicAdd(&P.cnt->overflow, 1ull);
-                }
-            }
-            // knock-on electrons and the surviving primaries -> this warp's ready stack
-            const unsigned em = __ballot_sync(kFull, kind == HK_MOLLER);
-            if (kind == HK_MOLLER) {
-                const unsigned slot = n_ready + __popc(em & lt);
-                if (slot < ready_cap) store_rec(pA, pB, pC, slot, c, __float_as_uint(flog(c.E)));
-                else atomicAdd(&P.cnt->overflow, 1ull);
-            }
-            n_ready = min(n_ready + __popc(em), ready_cap);
-            const bool cont = (kind >= 0) && st == ST_ALIVE;
-            const unsigned cm = __ballot_sync(kFull, cont);
-            if (cont) {
-                const unsigned slot = n_ready + __popc(cm & lt);
-                if (slot < ready_cap) store_rec(pA, pB, pC, slot, q, __float_as_uint(qlnT));
-                else atomicAdd(&P.cnt->overflow, 1ull);
-            }
-            n_ready = min(n_ready + __popc(cm), ready_cap);
-            n_moller += __popc(em);
-            n_brems += __popc(gm);
-            n_hfict += __popc(__ballot_sync(kFull, kind == HK_FICT));
+            __syncwarp();
+            w.n[SK_ES] = w.ctl->n_es;
+            w.n[SK_GS] = w.ctl->n_gs;
+            w.n[SK_GI] -= nb;
+            w.hw = max(w.hw, max(w.n[SK_ES], w.n[SK_GS]));
+            w.count(WC_COMPTON, __ballot_sync(kFull, kind == PM_COMPTON));
+            w.count(WC_PHOTO, __ballot_sync(kFull, kind == PM_PHOTO));
+            w.count(WC_PAIR, __ballot_sync(kFull, kind == PM_PAIR));
             __syncwarp();
             continue;
         }
-        if (am == 0u) {
-            if (exhausted && w_next == w_end && n_ready == 0u) break;
-            continue;
+        // ---- change of particle type?  (see electron_mode)
+        const unsigned ready = static_cast<unsigned>(__popc(live)) + w.n[SK_GS];
+        const unsigned G = ready + w.n[SK_GI], E = w.n[SK_ES] + w.n[SK_EH];
+        const unsigned must = w.cap_r - kMustMargin;
+        const bool src_e = !src_is_g && !cl.empty();
+        bool leave = E >= kHigh && (G < kHigh || E >= must);
+        if (!src_g) {
+            if (ready == 0u) return (E != 0u || src_e) ? 1 : -1; // (GI is empty here)
+            leave = leave || (ready < kLow && (src_e || w.n[SK_ES] >= 32u));
         }
-        // ---- one condensed-history step for every live lane
-        int st = ST_ALIVE;
-        if (alive) st = electron_step(P, TB, p, lnT, M, acc);
-        n_step += __popc(am);
-        const bool hard = alive && st == ST_HARD;
-        const unsigned hm = __ballot_sync(kFull, hard);
-        if (hard) {
-            store_rec(pA, pB, pC, ready_cap + n_hard + __popc(hm & lt), p, __float_as_uint(M));
-            alive = false;
+        if (leave) {
+            w.push(P, SK_GS, alive, p, 0u);
+            w.hw = max(w.hw, w.n[SK_GS]);
+            return 1;
         }
-        n_hard += __popc(hm);
-        if (st == ST_DEAD) alive = false;
-        __syncwarp();
-    }
-    if (lane == 0) {
-        DevCounters *c = P.cnt;
-        bump(&c->ch_steps, n_step); bump(&c->hard_moller, n_moller); bump(&c->hard_brems, n_brems);
-        bump(&c->hard_fict, n_hfict); bump(&c->pushes_e, n_moller); bump(&c->pushes_g, n_brems);
+        // ---- refill the free lanes: the stack first, then primaries
+        if (~live) {
+            uint32_t extra;
+            bool got = w.pop(SK_GS, !alive, p, extra);
+            if (src_g && __any_sync(kFull, !alive && !got)) got = w.primaries(a, cl, !alive && !got, p) || got;
+            if (got) alive = true;
+        }
+        const unsigned fl = __ballot_sync(kFull, alive);
+        if (fl == 0u) continue;
+        // ---- one flight for every lane that holds a photon
+        int mode = PM_DEAD;
+        if (alive) mode = photon_flight<TRACE>(P, TB, p);
+        w.count(WC_FLIGHT, fl);
+        w.count(WC_FICT, __ballot_sync(kFull, mode == PM_FLIGHT));
+        w.push(P, SK_GI, mode >= PM_COMPTON, p, static_cast<uint32_t>(mode));
+        alive = mode == PM_FLIGHT;
     }
 }
-
-// ---------------------------------------------------------------------------------------------
-// Optional phase timeline (compile with -DGPUMCD_TIMELINE; development aid, not in the default build):
-// per phase the input size, start time, the time each CTA finished and the time the barrier opened.
-// ---------------------------------------------------------------------------------------------
-#ifdef GPUMCD_TIMELINE
-constexpr int kTlPhases = 256, kTlBlocks = 160;
-struct Timeline {
-    unsigned n_phase;
-    unsigned type[kTlPhases], n_in[kTlPhases];
-    unsigned long long t0[kTlPhases], t1[kTlPhases];
-    unsigned long long done[kTlPhases][kTlBlocks];
-};
-__device__ Timeline g_timeline;
-__device__ __forceinline__ unsigned long long gtime()
-{
-    unsigned long long t;
-    asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
-    return t;
-}
-#define TL_BEGIN(np, ne) do { if (leader && tl < kTlPhases) { g_timeline.type[tl] = (np); g_timeline.n_in[tl] = (ne); g_timeline.t0[tl] = gtime(); } } while (0)
-#define TL_DONE() do { __syncthreads(); if (threadIdx.x == 0 && tl < kTlPhases && blockIdx.x < kTlBlocks) g_timeline.done[tl][blockIdx.x] = gtime(); } while (0)
-#define TL_END() do { if (leader && tl < kTlPhases) { g_timeline.t1[tl] = gtime(); g_timeline.n_phase = tl + 1; } ++tl; } while (0)
-#else
-#define TL_BEGIN(np, ne) do {} while (0)
-#define TL_DONE() do {} while (0)
-#define TL_END() do {} while (0)
-#endif
 
 // ---------------------------------------------------------------------------------------------
 // The persistent kernel
 // ---------------------------------------------------------------------------------------------
-__device__ __forceinline__ unsigned ld_volatile(const unsigned *p) { return *reinterpret_cast<const volatile unsigned *>(p); }
-
 template <bool TRACE, bool SMEM_TABLES>
-__global__ void __launch_bounds__(kPThreads, 1) k_persistent(const PersistArgs a)
+__global__ void __launch_bounds__(kPThreads, 1) k_persistent(const __grid_constant__ PersistArgs a)
 {
     extern __shared__ __align__(128) float smem[];
     __shared__ uint64_t bar;
+    __shared__ WarpCtl s_ctl[kPWarps];
+    __shared__ double s_einc[kPThreads];
     cg::grid_group grid = cg::this_grid();
 
     const Params &P = a.P;
@@ -396,61 +426,38 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(const PersistArgs a
         stage_tables(smem, P.tab.blob, a.table_floats, &bar);
         TB = smem;
     }
-    const unsigned gwarp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-    const size_t stride = static_cast<size_t>(a.priv_ready) + kHardCap;
-    float4 *pA = a.privA + gwarp * stride, *pB = a.privB + gwarp * stride;
-    uint4 *pC = a.privC + gwarp * stride;
-    const bool leader = (blockIdx.x == 0 && threadIdx.x == 0);
-#ifdef GPUMCD_TIMELINE
-    unsigned tl = 0;
-#endif
+    const unsigned lane = threadIdx.x & 31;
+    const size_t gwarp = (blockIdx.x * static_cast<size_t>(blockDim.x) + threadIdx.x) >> 5;
+    Warp w;
+    w.A = a.stkA + gwarp * a.stride;
+    w.B = a.stkB + gwarp * a.stride;
+    w.C = a.stkC + gwarp * a.stride;
+    w.cap_r = a.cap_r;
+    w.n[0] = w.n[1] = w.n[2] = w.n[3] = 0u;
+    w.lt = (1u << lane) - 1u;
+    w.hw = 0u;
+    w.ctl = &s_ctl[threadIdx.x >> 5];
+    w.e_inc = &s_einc[threadIdx.x];
+    s_einc[threadIdx.x] = 0.0;
+    if (lane < WC_N) w.ctl->wc[lane] = 0u;
+    __syncwarp();
 
-    // One iteration = one photon phase and one electron phase that do NOT depend on each other:
-    // iteration i reads photon queue X[i%3] and electron queue Y[i%3] and writes X[(i+1)%3] /
-    // Y[(i+1)%3]; the third pair was read in iteration i-1 and is reset now, to be written in i+1.
-    // So one grid barrier per iteration suffices, a warp that runs out of one type's input moves on
-    // to the other type without waiting, and odd / even warps start with different types, which
-    // keeps latency-bound photon warps and issue-bound electron warps on every SM at the same time.
-    // Each iteration also injects the next wave of primaries, so what is left over from a wave
-    // rides along with the bulk of the next one; only the very end of the run has a tail.
-    unsigned long long done = 0;
-    unsigned it = 0;
-    unsigned nP = 0, nE = 0; // queued photons in X[it%3] / electrons in Y[it%3]
-    const bool e_first = ((threadIdx.x >> 5) & 1) != 0;
-    for (;;) {
-        const unsigned r = it % 3u, w = (it + 1u) % 3u, z = (it + 2u) % 3u;
-        const unsigned n_src = static_cast<unsigned>(min(static_cast<unsigned long long>(a.wave), a.n_hist - done));
-        const unsigned long long hist_base = a.hist0 + done;
-        const unsigned srcP = (a.S.particle == 0) ? n_src : 0u, srcE = (a.S.particle == 1) ? n_src : 0u;
-        if (leader) {
-            *a.qP[z].count = 0u; a.heads[z] = 0u;
-            *a.qE[z].count = 0u; a.heads[3 + z] = 0u;
-        }
-        TL_BEGIN(nP + srcP, nE + srcE);
-#pragma unroll 1
-        for (int t = 0; t < 2; ++t) {
-            if ((t == 0) != e_first) {
-                // photons: read X[r] and the source, electrons -> Y[w], annihilation photons -> X[w]
-                if (nP + srcP) {
-                    if (srcP) photon_phase<TRACE, true>(P, TB, a.S, hist_base, a.qP[r], nP, nP + srcP, a.heads + r, a.qE[w], a.qP[w]);
-                    else photon_phase<TRACE, false>(P, TB, a.S, hist_base, a.qP[r], nP, nP, a.heads + r, a.qE[w], a.qP[w]);
-                }
-            } else {
-                // electrons: read Y[r] and the source, bremsstrahlung photons -> X[w], knock-ons stay in the warp
-                if (nE + srcE) {
-                    if (srcE) electron_phase<true>(P, TB, a.S, hist_base, a.qE[r], nE, nE + srcE, a.heads + 3 + r, a.qP[w], pA, pB, pC, a.priv_ready);
-                    else electron_phase<false>(P, TB, a.S, hist_base, a.qE[r], nE, nE, a.heads + 3 + r, a.qP[w], pA, pB, pC, a.priv_ready);
-                }
-            }
-        }
-        TL_DONE();
-        grid.sync();
-        TL_END();
-        nP = min(ld_volatile(a.qP[w].count), a.qP[w].cap);
-        nE = min(ld_volatile(a.qE[w].count), a.qE[w].cap);
-        done += n_src;
-        ++it;
-        if (nP == 0u && nE == 0u && done >= a.n_hist) break;
+    // Each warp works on its own until the source is exhausted and its stacks are empty.
+    Claim cl;
+    cl.exhausted = (a.n_hist == 0u);
+    int type = a.S.particle;
+    while (type >= 0) type = (type == 1) ? electron_mode(a, TB, w, cl) : photon_mode<TRACE>(a, TB, w, cl);
+
+    // ---- flush this warp's event counts and accounts
+    __syncwarp();
+    if (lane < WC_N) {
+        const unsigned v = w.ctl->wc[lane];
+        if (v) atomicAdd(&P.cnt->photon_flights + lane, static_cast<unsigned long long>(v));
+    }
+    const double e_new = wsum(s_einc[threadIdx.x]);
+    if (lane == 0) {
+        if (e_new != 0.0) Acc(P).inc(e_new);
+        if (w.hw) atomicMax(&P.cnt->high_water, static_cast<unsigned long long>(w.hw));
     }
     if (!a.finalize) return;
     grid.sync();
@@ -463,12 +470,12 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(const PersistArgs a
         if (a.dose) a.dose[i] = static_cast<float>(e / static_cast<double>(P.geo.phantom[i].x) * a.inv_h3_n);
     }
     s = wsum(s);
-    __shared__ double part[kPThreads / 32];
-    if ((threadIdx.x & 31) == 0) part[threadIdx.x >> 5] = s;
+    __shared__ double part[kPWarps];
+    if (lane == 0) part[threadIdx.x >> 5] = s;
     __syncthreads();
     if (threadIdx.x == 0) {
         double t = 0.0;
-        for (int k = 0; k < kPThreads / 32; ++k) t += part[k];
+        for (int k = 0; k < kPWarps; ++k) t += part[k];
         atomicAdd(&P.cnt->e_dep_total, t);
     }
 }

@@ -56,6 +56,7 @@ struct DevCounters {
     unsigned long long ch_steps, hard_moller, hard_brems, hard_fict;
     unsigned long long pushes_e, pushes_g;
     unsigned long long overflow;
+    unsigned long long high_water; // scheduler 1: fullest per-warp stack seen
     double e_dep_total;
     EnergySlot slot[kEnergySlots];
 };
@@ -71,15 +72,19 @@ struct Params {
     unsigned long long trace_off; // id of the run's first history
 };
 
-// energy accounts of the calling warp
+// energy accounts of the calling warp (rare events: the slot address is recomputed at every use
+// instead of being kept in registers)
 struct Acc {
-    EnergySlot *s;
-    __device__ __forceinline__ explicit Acc(const Params &P)
-        : s(&P.cnt->slot[((blockIdx.x * blockDim.x + threadIdx.x) >> 5) & (kEnergySlots - 1)]) {}
-    __device__ __forceinline__ void esc(float e) const { atomicAdd(&s->e_esc, static_cast<double>(e)); }
-    __device__ __forceinline__ void cut(float e) const { atomicAdd(&s->e_cut, static_cast<double>(e)); }
-    __device__ __forceinline__ void pair() const { atomicAdd(&s->e_pair, 2.0 * static_cast<double>(kMe)); }
-    __device__ __forceinline__ void inc(double e) const { atomicAdd(&s->e_inc, e); }
+    DevCounters *cnt;
+    __device__ __forceinline__ explicit Acc(const Params &P) : cnt(P.cnt) {}
+    __device__ __forceinline__ EnergySlot *slot() const
+    {
+        return &cnt->slot[((blockIdx.x * blockDim.x + threadIdx.x) >> 5) & (kEnergySlots - 1)];
+    }
+    __device__ __forceinline__ void esc(float e) const { atomicAdd(&slot()->e_esc, static_cast<double>(e)); }
+    __device__ __forceinline__ void cut(float e) const { atomicAdd(&slot()->e_cut, static_cast<double>(e)); }
+    __device__ __forceinline__ void pair() const { atomicAdd(&slot()->e_pair, 2.0 * static_cast<double>(kMe)); }
+    __device__ __forceinline__ void inc(double e) const { atomicAdd(&slot()->e_inc, e); }
 };
 
 __device__ __forceinline__ bool inside(const Geom &g, const Particle &p)
@@ -123,7 +128,20 @@ __device__ __forceinline__ Particle load_rec(const float4 *A, const float4 *B, c
 }
 
 // H7 push from divergent code: one atomic per group of converged lanes (activemask + popc prefix),
-// then three 16-byte stores per record.  `tally` counts the pushed records.
+// then three 16-byte stores per record.
+//   Queue     : a global queue shared by the whole grid (scheduler 0); counter in global memory
+//   WarpStack : a stack owned by the calling warp (scheduler 1); counter in shared memory.  A lane
+//               that finds the stack full gives its claim back, so the counter ends at the number of
+//               records stored and never above the capacity.
+struct WarpStack {
+    float4 *A;
+    float4 *B;
+    uint4 *C;
+    unsigned *count;  // shared memory
+    unsigned *pushed; // shared memory: event counter (pushes_e / pushes_g)
+    unsigned cap;
+};
+
 __device__ __forceinline__ void push(const Params &P, const Queue &q, const Particle &c, unsigned long long *tally)
 {
     const unsigned mask = __activemask();
@@ -139,6 +157,29 @@ __device__ __forceinline__ void push(const Params &P, const Queue &q, const Part
     if (slot < q.cap) store_rec(q.A, q.B, q.C, slot, c, 0u);
     else atomicAdd(&P.cnt->overflow, 1ull);
 }
+__device__ __forceinline__ void push(const Params &P, const WarpStack &q, const Particle &c)
+{
+    const unsigned mask = __activemask();
+    const int lane = threadIdx.x & 31;
+    const int leader = __ffs(mask) - 1;
+    unsigned base = 0;
+    if (lane == leader) {
+        base = atomicAdd(q.count, static_cast<unsigned>(__popc(mask)));
+        atomicAdd(q.pushed, static_cast<unsigned>(__popc(mask)));
+    }
+    base = __shfl_sync(mask, base, leader);
+    const unsigned slot = base + __popc(mask & ((1u << lane) - 1u));
+    if (slot < q.cap) {
+        store_rec(q.A, q.B, q.C, slot, c, 0u);
+    } else {
+        atomicSub(q.count, 1u);
+        atomicAdd(&P.cnt->overflow, 1ull);
+    }
+}
+__device__ __forceinline__ void push_e(const Params &P, const Queue &q, const Particle &c) { push(P, q, c, &P.cnt->pushes_e); }
+__device__ __forceinline__ void push_g(const Params &P, const Queue &q, const Particle &c) { push(P, q, c, &P.cnt->pushes_g); }
+__device__ __forceinline__ void push_e(const Params &P, const WarpStack &q, const Particle &c) { push(P, q, c); }
+__device__ __forceinline__ void push_g(const Params &P, const WarpStack &q, const Particle &c) { push(P, q, c); }
 
 __device__ __forceinline__ bool electron_tracked(const Params &P, float T)
 {
@@ -146,60 +187,73 @@ __device__ __forceinline__ bool electron_tracked(const Params &P, float T)
 }
 
 // ---------------------------------------------------------------------------------------------
-// One photon flight + interaction (H1, H2).  Returns the event; the photon is alive afterwards
-// iff the event is PH_COMPTON or PH_FICT.  Secondaries are pushed to qE (electrons) and qG
-// (annihilation photons).  TRACE records the primary track's event codes (gpumcd_run_trace).
+// Photon transport in two halves, so that a scheduler can run them with different lane sets:
+//   photon_flight   (H1 + the selection of H2): one Woodcock flight, then which interaction
+//   photon_interact (H2): the interaction itself; secondaries are pushed to qE (electrons) and qG
+//                   (annihilation photons)
+// photon_step = flight + interaction, for one-thread-per-particle schedulers.  A photon's mode:
+// PM_DEAD, PM_FLIGHT (next: a flight), PM_COMPTON / PM_PHOTO / PM_PAIR (next: that interaction at
+// the current position).  TRACE records the primary track's event codes (gpumcd_run_trace).
 // ---------------------------------------------------------------------------------------------
+enum : int { PM_DEAD = 0, PM_FLIGHT = 1, PM_COMPTON = 2, PM_PHOTO = 3, PM_PAIR = 4 };
 enum : int { PH_ESCAPE = 0, PH_COMPTON = 1, PH_ABSORBED = 2, PH_PHOTO = 3, PH_PAIR = 4, PH_FICT = 5 };
 __device__ __forceinline__ bool photon_alive(int ev) { return ev == PH_COMPTON || ev == PH_FICT; }
 
-struct Trace {
-    unsigned long long bits = 0ull;
-    int n = 0;
-};
+// Replay trace (gpumcd_run_trace): the primary track appends its event codes, 3 bits each, to the
+// history's word in global memory.  The codes are non-zero, so the number of events recorded so far
+// is the index of the highest non-zero group + 1 and no per-particle trace state exists: a photon
+// can be parked in a stack and picked up by another lane of its warp (persistent.cuh) in between.
 template <bool TRACE>
-__device__ __forceinline__ void record(Trace &tr, const Particle &p, int code)
+__device__ __forceinline__ void record(const Params &P, const Particle &p, int code)
 {
-    if (TRACE && p.track == 0u && tr.n < 21) {
-        tr.bits |= static_cast<unsigned long long>(code) << (3 * tr.n);
-        ++tr.n;
+    if (TRACE && p.track == 0u) {
+        volatile unsigned long long *t =
+            P.trace + (((static_cast<unsigned long long>(P.rng.hist_hi) << 32) | p.hist) - P.trace_off);
+        const unsigned long long bits = *t;
+        const int n = bits ? (66 - __clzll(static_cast<long long>(bits))) / 3 : 0;
+        if (n < 21) *t = bits | (static_cast<unsigned long long>(code) << (3 * n));
     }
 }
-template <bool TRACE>
-__device__ __forceinline__ void write_trace(const Params &P, const Particle &p, const Trace &tr)
-{
-    if (TRACE && p.track == 0u)
-        P.trace[((static_cast<unsigned long long>(P.rng.hist_hi) << 32) | p.hist) - P.trace_off] = tr.bits;
-}
 
+// One flight (Eq. 1 with the Woodcock majorant of Eq. 3) and the choice of the interaction at its
+// end (Eq. 2 per type; the remainder up to mu_max is fictitious, L59).  Returns the next mode:
+// PM_DEAD (escaped), PM_FLIGHT (fictitious interaction: nothing changes), or the interaction.
 template <bool TRACE>
-__device__ int photon_step(const Params &P, const float *__restrict__ TB, Particle &p, const Acc &acc,
-                           const Queue &qE, const Queue &qG, Trace &tr)
+__device__ __forceinline__ int photon_flight(const Params &P, const float *__restrict__ TB, Particle &p)
 {
     const Tables &tb = P.tab;
     const uint4 w = draw(P.rng, p);
     const Interp iE = locate(tb.gE, flog(p.E));
     const float mu_max = interp(TB + tb.off_mu, iE);
-    // Eq. 1 with the Woodcock majorant of Eq. 3
     const float s = fdiv(-flog(u01(w.x)), mu_max);
     advance(p, s * P.geo.inv_h);
     if (!inside(P.geo, p)) {
-        acc.esc(p.E);
-        record<TRACE>(tr, p, 4);
-        return PH_ESCAPE;
+        Acc(P).esc(p.E);
+        record<TRACE>(P, p, 4);
+        return PM_DEAD;
     }
-    const unsigned lin = voxel_index(P.geo, p);
-    const float2 pv = __ldg(&P.geo.phantom[lin]);
+    const float2 pv = __ldg(&P.geo.phantom[voxel_index(P.geo, p)]);
     const float rho = pv.x;
     const float *col = TB + __float_as_int(pv.y) * 3 * tb.gE.n;
     const float r = u01(w.y) * mu_max;
     const float c1 = rho * interp(col, iE);
     const float c2 = fmaf(rho, interp(col + tb.gE.n, iE), c1);
     const float c3 = fmaf(rho, interp(col + 2 * tb.gE.n, iE), c2);
-    if (r >= c3) return PH_FICT; // fictitious interaction (L59): nothing changes
-    if (r < c1) {
+    if (r >= c3) return PM_FLIGHT;
+    return r < c1 ? PM_COMPTON : (r < c2 ? PM_PHOTO : PM_PAIR);
+}
+
+// The interaction `kind` (PM_COMPTON / PM_PHOTO / PM_PAIR) at the photon's position.  Returns
+// PM_FLIGHT if the photon goes on (Compton above P_cut), else PM_DEAD.
+template <bool TRACE, class QE, class QG>
+__device__ __forceinline__ int photon_interact(const Params &P, Particle &p, int kind, const QE &qE, const QG &qG)
+{
+    const Tables &tb = P.tab;
+    const Acc acc(P);
+    const unsigned lin = voxel_index(P.geo, p);
+    if (kind == PM_COMPTON) {
         // ---- Compton (L65) ----
-        record<TRACE>(tr, p, 1);
+        record<TRACE>(P, p, 1);
         float eps, t, uphi, nu, nv, nw, sp, cp;
         sample_compton(P.rng, p, eps, t, uphi);
         sincos2pi(uphi, sp, cp);
@@ -214,7 +268,7 @@ __device__ int photon_step(const Params &P, const float *__restrict__ TB, Partic
             c.E = Te;
             c.track = lineage(P.rng, p).x;
             c.ctr = 0u;
-            push(P, qE, c, &P.cnt->pushes_e);
+            push_e(P, qE, c);
         } else {
             deposit(P, lin, Te);
             acc.cut(Te);
@@ -224,14 +278,14 @@ __device__ int photon_step(const Params &P, const float *__restrict__ TB, Partic
         if (p.E < tb.p_cut) {
             deposit(P, lin, p.E);
             acc.cut(p.E);
-            record<TRACE>(tr, p, 5);
-            return PH_ABSORBED;
+            record<TRACE>(P, p, 5);
+            return PM_DEAD;
         }
-        return PH_COMPTON;
+        return PM_FLIGHT;
     }
-    if (r < c2) {
+    if (kind == PM_PHOTO) {
         // ---- photoelectric (L67-72): one electron with T = E_phot ----
-        record<TRACE>(tr, p, 2);
+        record<TRACE>(P, p, 2);
         if (electron_tracked(P, p.E)) {
             float nu_, uphi, sp, cp;
             sample_sauter(P.rng, p, p.E, nu_, uphi);
@@ -240,15 +294,15 @@ __device__ int photon_step(const Params &P, const float *__restrict__ TB, Partic
             rotate(p.u, p.v, p.w, 1.0f - nu_, sqrtf(fmaxf(nu_ * (2.0f - nu_), 0.0f)), cp, sp, c.u, c.v, c.w);
             c.track = lineage(P.rng, p).x;
             c.ctr = 0u;
-            push(P, qE, c, &P.cnt->pushes_e);
+            push_e(P, qE, c);
         } else {
             deposit(P, lin, p.E);
             acc.cut(p.E);
         }
-        return PH_PHOTO;
+        return PM_DEAD;
     }
     // ---- pair production (L74): two electrons, no positron ----
-    record<TRACE>(tr, p, 3);
+    record<TRACE>(P, p, 3);
     const uint4 v = draw(P.rng, p);
     const float Tsum = p.E - 2.0f * kMe;
     const float T1 = u01(v.x) * Tsum;
@@ -275,7 +329,7 @@ __device__ int photon_step(const Params &P, const float *__restrict__ TB, Partic
     if (t1) {
         rotate(p.u, p.v, p.w, ca, sa, cp, sp, c.u, c.v, c.w);
         c.E = T1; c.track = id.x;
-        push(P, qE, c, &P.cnt->pushes_e);
+        push_e(P, qE, c);
     } else {
         deposit(P, lin, T1);
         acc.cut(T1);
@@ -283,7 +337,7 @@ __device__ int photon_step(const Params &P, const float *__restrict__ TB, Partic
     if (t2) {
         rotate(p.u, p.v, p.w, cb, sb, -cp, -sp, c.u, c.v, c.w); // opposite azimuth
         c.E = T2; c.track = id.y;
-        push(P, qE, c, &P.cnt->pushes_e);
+        push_e(P, qE, c);
     } else {
         deposit(P, lin, T2);
         acc.cut(T2);
@@ -292,14 +346,27 @@ __device__ int photon_step(const Params &P, const float *__restrict__ TB, Partic
     if (P.opt.pair_mode == 1) {
         c.E = kMe;
         c.u = ax; c.v = ay; c.w = az; c.track = id.z;
-        push(P, qG, c, &P.cnt->pushes_g);
+        push_g(P, qG, c);
         c.u = -ax; c.v = -ay; c.w = -az; c.track = id.w;
-        push(P, qG, c, &P.cnt->pushes_g);
+        push_g(P, qG, c);
     } else {
         deposit(P, lin, 2.0f * kMe);
         acc.cut(2.0f * kMe);
     }
-    return PH_PAIR;
+    return PM_DEAD;
+}
+
+// flight + interaction; returns the event (the photon is alive afterwards iff photon_alive(event))
+template <bool TRACE>
+__device__ int photon_step(const Params &P, const float *__restrict__ TB, Particle &p, const Queue &qE,
+                           const Queue &qG)
+{
+    const int kind = photon_flight<TRACE>(P, TB, p);
+    if (kind == PM_DEAD) return PH_ESCAPE;
+    if (kind == PM_FLIGHT) return PH_FICT;
+    const int next = photon_interact<TRACE>(P, p, kind, qE, qG);
+    if (kind == PM_COMPTON) return next == PM_FLIGHT ? PH_COMPTON : PH_ABSORBED;
+    return kind == PM_PHOTO ? PH_PHOTO : PH_PAIR;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -310,8 +377,9 @@ __device__ int photon_step(const Params &P, const float *__restrict__ TB, Partic
 enum : int { ST_ALIVE = 0, ST_DEAD = 1, ST_HARD = 2 };
 
 __device__ __forceinline__ int electron_step(const Params &P, const float *__restrict__ TB, Particle &p, float &lnT,
-                                             float &M, const Acc &acc)
+                                             float &M)
 {
+    const Acc acc(P);
     const Tables &tb = P.tab;
     const int nE = tb.gE.n;
     const unsigned lin = voxel_index(P.geo, p);
@@ -385,8 +453,9 @@ __device__ __forceinline__ int electron_step(const Params &P, const float *__res
 enum : int { HK_FICT = 0, HK_MOLLER = 1, HK_BREMS = 2 };
 
 __device__ __forceinline__ int electron_hard(const Params &P, const float *__restrict__ TB, Particle &p, float &lnT,
-                                             float M, const Acc &acc, Particle &child, int &kind)
+                                             float M, Particle &child, int &kind)
 {
+    const Acc acc(P);
     const Tables &tb = P.tab;
     const int nE = tb.gE.n;
     const uint4 b = draw(P.rng, p);
@@ -480,11 +549,9 @@ struct Local {
 template <bool TRACE>
 __device__ void photon_run(const Params &P, Particle p, Local &L, const Queue &qE, const Queue &qG)
 {
-    Trace tr;
     const float *TB = P.tab.blob;
-    const Acc acc(P);
     for (;;) {
-        const int ev = photon_step<TRACE>(P, TB, p, acc, qE, qG, tr);
+        const int ev = photon_step<TRACE>(P, TB, p, qE, qG);
         L.flights++;
         L.compton += (ev == PH_COMPTON || ev == PH_ABSORBED);
         L.photo += (ev == PH_PHOTO);
@@ -492,23 +559,21 @@ __device__ void photon_run(const Params &P, Particle p, Local &L, const Queue &q
         L.fict += (ev == PH_FICT);
         if (!photon_alive(ev)) break;
     }
-    write_trace<TRACE>(P, p, tr);
 }
 
 __device__ void electron_run(const Params &P, Particle p, Local &L, const Queue &qE, const Queue &qG)
 {
     float lnT = flog(p.E), M;
     const float *TB = P.tab.blob;
-    const Acc acc(P);
     for (;;) {
-        int st = electron_step(P, TB, p, lnT, M, acc);
+        int st = electron_step(P, TB, p, lnT, M);
         L.steps++;
         if (st == ST_HARD) {
             Particle c;
             int kind;
-            st = electron_hard(P, TB, p, lnT, M, acc, c, kind);
-            if (kind == HK_MOLLER) { L.moller++; push(P, qE, c, &P.cnt->pushes_e); }
-            else if (kind == HK_BREMS) { L.brems++; push(P, qG, c, &P.cnt->pushes_g); }
+            st = electron_hard(P, TB, p, lnT, M, c, kind);
+            if (kind == HK_MOLLER) { L.moller++; push_e(P, qE, c); }
+            else if (kind == HK_BREMS) { L.brems++; push_g(P, qG, c); }
             else L.hfict++;
         }
         if (st == ST_DEAD) return;

@@ -236,6 +236,40 @@ def test_host_entry_points_match_device_entry_points(workloads):
     np.testing.assert_allclose(dose, ref["dose"], rtol=1e-6, atol=0)
 
 
+def test_set_phantom_replaces_the_volumes_and_majorants(workloads):
+    """A context re-targeted at another phantom of the same grid gives what a fresh context gives."""
+    import torch
+
+    import paper_1101_1245_b200 as g
+
+    w4, n = workloads[4], 30_000
+    ref = run_gpu(w4, n)
+    water = np.ones_like(w4.density)
+    zeros = np.zeros_like(w4.material)
+    dev = torch.device("cuda:0")
+    dose = np.empty(w4.density.shape, np.float32)
+    with g.gpumcd_create_host(water, zeros, w4.voxel_cm, w4.tables) as ctx:       # starts as plain water
+        g.gpumcd_set_source(ctx, w4.source)
+        g.gpumcd_run_host(ctx, n, w4.seed, dose)
+        c_water = g.gpumcd_get_counters(ctx)
+        g.gpumcd_set_phantom_host(ctx, w4.density, w4.material)                  # host volumes
+        g.gpumcd_run_host(ctx, n, w4.seed, dose)
+        c_host = g.gpumcd_get_counters(ctx)
+        np.testing.assert_allclose(dose, ref["dose"], rtol=1e-6, atol=0)
+        g.gpumcd_set_phantom(ctx, torch.from_numpy(water).to(dev), torch.from_numpy(zeros).to(dev))
+        g.gpumcd_set_phantom(ctx, torch.from_numpy(w4.density).to(dev), torch.from_numpy(w4.material).to(dev))
+        g.gpumcd_run_host(ctx, n, w4.seed, dose)                                   # device volumes
+        c_dev = g.gpumcd_get_counters(ctx)
+        bad = w4.material.copy()
+        bad[0, 0, 0] = 7
+        with pytest.raises(g.GpumcdError) as e:
+            g.gpumcd_set_phantom_host(ctx, w4.density, bad)
+        assert e.value.status == -1
+    for k in INT_KEYS:
+        assert c_host[k] == ref["counters"][k] == c_dev[k], k
+    assert c_water["photon_fict"] < 0.5 * c_host["photon_fict"]      # bone raises the majorant (PAPER.md L357-362)
+
+
 def test_error_paths(workloads):
     import torch
 
@@ -270,13 +304,14 @@ def test_error_paths(workloads):
     rho2 = torch.from_numpy(w2.density).to(dev)
     mat2 = torch.from_numpy(w2.material).to(dev)
     dose2 = torch.empty(rho2.shape, dtype=torch.float32, device=dev)
-    for sched in SCHEDULERS:
-        # 20000 electrons of 15 MeV make ~60000 knock-on electrons (scheduler 0 banks them in a global queue)
-        # and ~32000 bremsstrahlung photons (both schedulers bank those): more than 1 x 20000 slots
-        opt = g.gpumcd_default_options(wave_size=20000, bank_factor=1, scheduler=sched)
+    # scheduler 0 banks the ~60000 knock-on electrons and ~32000 bremsstrahlung photons of 20000 electrons of
+    # 15 MeV in global queues of 1 x 20000 slots; with scheduler 1 a warp simulates ~200 of 1e6 histories and
+    # banks their ~400 bremsstrahlung photons in its own photon stack, here 192 records deep
+    for sched, n, opts in ((0, 20000, dict(wave_size=20000, bank_factor=1)), (1, 1_000_000, dict(warp_stack=192))):
+        opt = g.gpumcd_default_options(scheduler=sched, **opts)
         with g.gpumcd_create(rho2, mat2, w2.voxel_cm, w2.tables, opt) as ctx:
             g.gpumcd_set_source(ctx, w2.source)
             with pytest.raises(g.GpumcdError) as e:
-                g.gpumcd_run(ctx, 20000, 1, dose2)
+                g.gpumcd_run(ctx, n, 1, dose2)
                 g.gpumcd_get_counters(ctx)
             assert e.value.status == -4
