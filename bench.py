@@ -181,6 +181,7 @@ def main():
     ap.add_argument("--histories", type=int, default=0, help="override histories per step (0 = the config's)")
     ap.add_argument("--scheduler", type=int, default=-1)
     ap.add_argument("--wave", type=int, default=0, help="override wave_size (0 = library default)")
+    ap.add_argument("--cta-threads", type=int, default=0, help="override cta_threads (0 = the library's choice)")
     ap.add_argument("--ref-histories", type=int, default=50_000)
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -224,6 +225,8 @@ def main():
         opts["scheduler"] = args.scheduler
     if args.wave > 0:
         opts["wave_size"] = args.wave
+    if args.cta_threads > 0:
+        opts["cta_threads"] = args.cta_threads
     opt = g.gpumcd_default_options(**opts)
     ctx = g.gpumcd_create(rho, mat, w.voxel_cm, w.tables, opt)
     g.gpumcd_set_source(ctx, w.source)

@@ -88,6 +88,10 @@ typedef struct {
     uint32_t warp_stack;   /* scheduler 1: capacity of a warp's electron stack and of its photon
                               stack, records; default 1024 (smaller values only make sense in
                               tests of the overflow report; at least 192)                          */
+    uint32_t cta_threads;  /* scheduler 1: threads of the persistent kernel's one CTA per SM, 512 or
+                              1024; 0 (default) chooses 512 where the mean density is at least 0.8 of
+                              the largest (few fictitious interactions, little waiting on memory)
+                              and 1024 elsewhere                                                    */
 } gpumcd_options;
 
 typedef struct {

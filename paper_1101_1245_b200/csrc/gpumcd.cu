@@ -22,11 +22,12 @@ constexpr int kBlock = 256;
 // (H10; positive floats order like their bit patterns, so atomicMax on the bits is a float max).
 __global__ void k_pack_phantom(const float *__restrict__ density, const uint8_t *__restrict__ material,
                                size_t nvox, int n_mat, float2 *__restrict__ out, unsigned *rho_max_bits,
-                               unsigned *n_bad)
+                               unsigned *n_bad, double *rho_sum)
 {
     __shared__ unsigned s_max[8];
     if (threadIdx.x < 8) s_max[threadIdx.x] = 0u;
     __syncthreads();
+    double sum = 0.0;
     for (size_t i = blockIdx.x * static_cast<size_t>(blockDim.x) + threadIdx.x; i < nvox;
          i += static_cast<size_t>(gridDim.x) * blockDim.x) {
         const float d = density[i];
@@ -37,8 +38,11 @@ __global__ void k_pack_phantom(const float *__restrict__ density, const uint8_t 
         } else {
             atomicMax(&s_max[m], __float_as_uint(d));
             out[i] = make_float2(d, __int_as_float(m));
+            sum += static_cast<double>(d);
         }
     }
+    sum = wsum(sum);
+    if ((threadIdx.x & 31) == 0 && sum != 0.0) atomicAdd(rho_sum, sum);
     __syncthreads();
     if (threadIdx.x < 8 && s_max[threadIdx.x]) atomicMax(&rho_max_bits[threadIdx.x], s_max[threadIdx.x]);
 }
@@ -135,7 +139,8 @@ struct gpumcd_ctx {
     float2 *phantom = nullptr;
     float *stage_density = nullptr;   // device staging of host volumes (gpumcd_create_host / set_phantom_host)
     uint8_t *stage_material = nullptr;
-    unsigned *scratch = nullptr;      // 8 rho_max bit patterns + 1 bad-voxel count
+    unsigned *scratch = nullptr;      // 8 rho_max bit patterns + 1 bad-voxel count + (at word 10) the fp64 sum of the densities
+    double rho_mean_over_max = 1.0;   // homogeneity of the phantom: mean density / largest density
     float *dose_stage = nullptr;      // device dose of gpumcd_run_host
     float *table_blob = nullptr;
     std::vector<float> blob_host;     // host copy of the table blob (majorants are rebuilt per phantom)
@@ -230,6 +235,7 @@ extern "C" int gpumcd_default_options(gpumcd_options *opt)
     opt->bank_factor = 8;
     opt->scheduler = 1;
     opt->warp_stack = 1024;
+    opt->cta_threads = 0;
     return GPUMCD_OK;
 }
 
@@ -273,11 +279,12 @@ static int load_phantom(gpumcd_ctx *ctx, const float *density, const uint8_t *ma
         d_density = ctx->stage_density;
         d_material = ctx->stage_material;
     }
-    CK(cudaMemsetAsync(ctx->scratch, 0, 9 * sizeof(unsigned), nullptr));
+    CK(cudaMemsetAsync(ctx->scratch, 0, 12 * sizeof(unsigned), nullptr));
     const int grid = static_cast<int>(std::min<size_t>((nvox + kBlock - 1) / kBlock, 148 * 8));
-    k_pack_phantom<<<grid, kBlock>>>(d_density, d_material, nvox, ctx->n_mat, ctx->phantom, ctx->scratch, ctx->scratch + 8);
+    k_pack_phantom<<<grid, kBlock>>>(d_density, d_material, nvox, ctx->n_mat, ctx->phantom, ctx->scratch, ctx->scratch + 8,
+                                   reinterpret_cast<double *>(ctx->scratch + 10));
     CK(cudaGetLastError());
-    unsigned h_scratch[9];
+    unsigned h_scratch[12];
     CK(cudaMemcpy(h_scratch, ctx->scratch, sizeof h_scratch, cudaMemcpyDeviceToHost));
     if (h_scratch[8] != 0) {
         set_error(ctx, "phantom has a material id >= n_materials or a density that is not a positive finite number");
@@ -285,6 +292,12 @@ static int load_phantom(gpumcd_ctx *ctx, const float *density, const uint8_t *ma
     }
     double rho_max[8];
     for (int m = 0; m < 8; ++m) { float f; memcpy(&f, &h_scratch[m], 4); rho_max[m] = f; }
+    {
+        double sum;
+        memcpy(&sum, &h_scratch[10], 8);
+        const double top = *std::max_element(rho_max, rho_max + 8);
+        ctx->rho_mean_over_max = top > 0.0 ? sum / static_cast<double>(nvox) / top : 1.0;
+    }
     const int nE = ctx->n_E, nM = ctx->n_mat;
     const float *ph = ctx->blob_host.data(), *el = ph + ctx->tab.off_el;
     float *mu_max = ctx->blob_host.data() + ctx->tab.off_mu, *m_e = ctx->blob_host.data() + ctx->tab.off_me;
@@ -327,6 +340,7 @@ static int create_impl(gpumcd_ctx **out, const float *density, const uint8_t *ma
     if (opt_in) opt = *opt_in;
     if (!(opt.es_max_cm > 0.f) || !(opt.f_eloss_max > 0.f) || opt.f_eloss_max > 1.f || opt.boundary_nudge < 0.f ||
         !(opt.majorant_scale >= 1.f) || opt.wave_size == 0 || opt.bank_factor == 0 || opt.warp_stack > (1u << 20) ||
+        (opt.cta_threads != 0 && opt.cta_threads != 512 && opt.cta_threads != 1024) ||
         static_cast<unsigned long long>(opt.wave_size) * opt.bank_factor > 0x7fffffffull) {
         set_error(nullptr, "bad options");
         return GPUMCD_ERR_INVALID_ARG;
@@ -367,7 +381,7 @@ static int create_impl(gpumcd_ctx **out, const float *density, const uint8_t *ma
 
     // ---- phantom (and the majorants that depend on it) ----
     CK(cudaMalloc(&ctx->phantom, nvox * sizeof(float2)));
-    CK(cudaMalloc(&ctx->scratch, 9 * sizeof(unsigned)));
+    CK(cudaMalloc(&ctx->scratch, 12 * sizeof(unsigned)));
     {
         const int rc = load_phantom(ctx, density, material, on_host);
         if (rc != GPUMCD_OK) return rc;
@@ -393,23 +407,25 @@ static int create_impl(gpumcd_ctx **out, const float *density, const uint8_t *ma
         if (!coop) { set_error(ctx, "device does not support cooperative launches (scheduler 1)"); return GPUMCD_ERR_CUDA; }
         const size_t table_bytes = static_cast<size_t>(ctx->table_floats) * sizeof(float);
         cudaFuncAttributes fa{};
-        CK(cudaFuncGetAttributes(&fa, k_persistent<false, true>));
+        CK(cudaFuncGetAttributes(&fa, k_persistent<false, true, 1024>));
         ctx->smem_tables = table_bytes + fa.sharedSizeBytes + 1024 <= static_cast<size_t>(max_smem);
         const size_t dyn = ctx->smem_tables ? table_bytes : 0;
         if (ctx->smem_tables) {
-            CK(cudaFuncSetAttribute(k_persistent<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(dyn)));
-            CK(cudaFuncSetAttribute(k_persistent<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(dyn)));
+            CK(cudaFuncSetAttribute(k_persistent<false, true, 512>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(dyn)));
+            CK(cudaFuncSetAttribute(k_persistent<true, true, 512>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(dyn)));
+            CK(cudaFuncSetAttribute(k_persistent<false, true, 1024>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(dyn)));
+            CK(cudaFuncSetAttribute(k_persistent<true, true, 1024>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(dyn)));
         }
         int per_sm = 0;
         if (ctx->smem_tables)
-            CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_persistent<false, true>, kPThreads, dyn));
+            CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_persistent<false, true, 1024>, 1024, dyn));
         else
-            CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_persistent<false, false>, kPThreads, 0));
+            CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_persistent<false, false, 1024>, 1024, 0));
         if (per_sm < 1) { set_error(ctx, "persistent kernel does not fit on an SM"); return GPUMCD_ERR_CUDA; }
         ctx->p_grid = n_sm; // one CTA per SM
         ctx->cap_r = std::max(opt.warp_stack, kMustMargin + 32u);
         ctx->stride = 2 * ctx->cap_r + 2 * kPend;
-        const size_t n_warps = static_cast<size_t>(ctx->p_grid) * (kPThreads / 32);
+        const size_t n_warps = static_cast<size_t>(ctx->p_grid) * (kPThreadsMax / 32);
         const size_t recs = n_warps * ctx->stride;
         CK(cudaMalloc(&ctx->stkA, recs * sizeof(float4)));
         CK(cudaMalloc(&ctx->stkB, recs * sizeof(float4)));
@@ -603,13 +619,22 @@ static int run_persistent(gpumcd_ctx *ctx, uint64_t n_hist, uint64_t seed, float
         a.dose = dose_dev;
         a.nvox = ctx->nvox;
         a.finalize = (h0 + n == h_end) ? 1 : 0;
+        // CTA size (see persistent.cuh): 512 threads in a nearly homogeneous phantom, else 1024
+        int threads = static_cast<int>(ctx->opt.cta_threads);
+        if (threads == 0) threads = ctx->rho_mean_over_max >= 0.8 ? 512 : 1024;
+        a.high = threads == 512 ? 256u : 512u;
         void *args[] = {&a};
         const void *fn;
-        if (ctx->smem_tables) fn = trace ? (const void *)k_persistent<true, true> : (const void *)k_persistent<false, true>;
-        else fn = trace ? (const void *)k_persistent<true, false> : (const void *)k_persistent<false, false>;
+        if (threads == 512) {
+            if (ctx->smem_tables) fn = trace ? (const void *)k_persistent<true, true, 512> : (const void *)k_persistent<false, true, 512>;
+            else fn = trace ? (const void *)k_persistent<true, false, 512> : (const void *)k_persistent<false, false, 512>;
+        } else {
+            if (ctx->smem_tables) fn = trace ? (const void *)k_persistent<true, true, 1024> : (const void *)k_persistent<false, true, 1024>;
+            else fn = trace ? (const void *)k_persistent<true, false, 1024> : (const void *)k_persistent<false, false, 1024>;
+        }
         const size_t dyn = ctx->smem_tables ? static_cast<size_t>(ctx->table_floats) * sizeof(float) : 0;
         { LaunchScope ls(ctx, st, CLS_ELECTRON);
-        CK(cudaLaunchCooperativeKernel(fn, dim3(ctx->p_grid), dim3(kPThreads), args, dyn, st)); }
+        CK(cudaLaunchCooperativeKernel(fn, dim3(ctx->p_grid), dim3(threads), args, dyn, st)); }
         h0 += n;
     }
     return GPUMCD_OK;

@@ -29,21 +29,17 @@ namespace gpumcd {
 
 namespace cg = cooperative_groups;
 
-#ifndef GPUMCD_PTHREADS
-#define GPUMCD_PTHREADS 1024
-#endif
-#ifndef GPUMCD_HIGH
-#define GPUMCD_HIGH 512
-#endif
 #ifndef GPUMCD_LOW
 #define GPUMCD_LOW 24
 #endif
-constexpr int kPThreads = GPUMCD_PTHREADS; // threads per persistent CTA (one CTA per SM)
-constexpr int kPWarps = kPThreads / 32;
+// Threads per persistent CTA (one CTA per SM): the kernel is built for 512 (128 registers per
+// thread, no spills, short drain phase: best where flights and steps rarely wait for memory) and
+// for 1024 (64 registers, twice the warps to hide the L2 latency of the phantom fetch: best in
+// heterogeneous phantoms, where most photon flights end in a fictitious interaction).
+constexpr int kPThreadsMax = 1024;
 constexpr unsigned kFull = 0xffffffffu;
 constexpr unsigned kChunk = 32;            // primaries a warp claims per atomic on the source head
 constexpr unsigned kPend = 64;             // capacity of a waiting stack (EH, GI): < 32 before a move, + 32 after
-constexpr unsigned kHigh = GPUMCD_HIGH;    // other-type records that make a warp change type
 constexpr unsigned kLow = GPUMCD_LOW;      // own-type particles below which a warp with no source changes type
 constexpr unsigned kMustMargin = 160;      // a ready stack within this many records of its capacity forces the change
 
@@ -136,6 +132,7 @@ struct PersistArgs {
     float4 *stkB;
     uint4 *stkC;
     unsigned cap_r;                // capacity of a ready stack (ES, GS)
+    unsigned high;                 // other-type records that make a warp change type
     unsigned stride;               // 2 cap_r + 2 kPend
     unsigned long long hist0;      // first history of the launch (low word never wraps inside a launch)
     unsigned n_hist;               // histories of the launch (< 2^32)
@@ -180,6 +177,7 @@ struct Warp {
     float4 *B;
     uint4 *C;
     unsigned cap_r;
+    unsigned high;
     unsigned n[4];
     unsigned lt;   // lanes below this one
     unsigned hw;   // fullest ready stack seen
@@ -285,7 +283,7 @@ __device__ __forceinline__ int electron_mode(const PersistArgs &a, const float *
         const unsigned E = ready + w.n[SK_EH], G = w.n[SK_GS] + w.n[SK_GI];
         const unsigned must = w.cap_r - kMustMargin;
         const bool src_g = !src_is_e && !cl.empty();
-        bool leave = G >= kHigh && (E < kHigh || (G >= must && E < must));
+        bool leave = G >= w.high && (E < w.high || (G >= must && E < must));
         if (!src_e) {
             if (ready == 0u) return (G != 0u || src_g) ? 0 : -1; // (EH is empty here)
             leave = leave || (ready < kLow && (src_g || w.n[SK_GS] >= 32u));
@@ -379,7 +377,7 @@ __device__ __forceinline__ int photon_mode(const PersistArgs &a, const float *__
         const unsigned G = ready + w.n[SK_GI], E = w.n[SK_ES] + w.n[SK_EH];
         const unsigned must = w.cap_r - kMustMargin;
         const bool src_e = !src_is_g && !cl.empty();
-        bool leave = E >= kHigh && (G < kHigh || E >= must);
+        bool leave = E >= w.high && (G < w.high || E >= must);
         if (!src_g) {
             if (ready == 0u) return (E != 0u || src_e) ? 1 : -1; // (GI is empty here)
             leave = leave || (ready < kLow && (src_e || w.n[SK_ES] >= 32u));
@@ -411,10 +409,11 @@ __device__ __forceinline__ int photon_mode(const PersistArgs &a, const float *__
 // ---------------------------------------------------------------------------------------------
 // The persistent kernel
 // ---------------------------------------------------------------------------------------------
-template <bool TRACE, bool SMEM_TABLES>
+template <bool TRACE, bool SMEM_TABLES, int kPThreads>
 __global__ void __launch_bounds__(kPThreads, 1) k_persistent(const __grid_constant__ PersistArgs a)
 {
     extern __shared__ __align__(128) float smem[];
+    constexpr int kPWarps = kPThreads / 32;
     __shared__ uint64_t bar;
     __shared__ WarpCtl s_ctl[kPWarps];
     __shared__ double s_einc[kPThreads];
@@ -433,6 +432,7 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(const __grid_consta
     w.B = a.stkB + gwarp * a.stride;
     w.C = a.stkC + gwarp * a.stride;
     w.cap_r = a.cap_r;
+    w.high = a.high;
     w.n[0] = w.n[1] = w.n[2] = w.n[3] = 0u;
     w.lt = (1u << lane) - 1u;
     w.hw = 0u;

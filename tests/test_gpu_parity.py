@@ -150,6 +150,19 @@ def test_schedulers_agree_exactly(workloads):
         assert np.abs(a["edep"] - b["edep"]).max() <= 1e-12 * a["edep"].max()
 
 
+def test_cta_size_does_not_change_the_result(workloads):
+    """Scheduler 1 runs with 512 or 1024 threads per SM (chosen from the phantom's homogeneity unless
+    cta_threads says otherwise): which lane works a particle off does not matter."""
+    for cfg in (2, 4):
+        w = workloads[cfg]
+        a = run_gpu(w, 60_000, scheduler=1, cta_threads=512)
+        b = run_gpu(w, 60_000, scheduler=1, cta_threads=1024)
+        c = run_gpu(w, 60_000, scheduler=1)
+        for k in INT_KEYS:
+            assert a["counters"][k] == b["counters"][k] == c["counters"][k], k
+        assert np.abs(a["edep"] - b["edep"]).max() <= 1e-12 * a["edep"].max()
+
+
 @pytest.mark.parametrize("scheduler", SCHEDULERS)
 @pytest.mark.parametrize("n,wave", [(1, 1 << 20), (31, 1 << 20), (2500, 1000), (4097, 4096), (70_001, 1 << 15)])
 def test_ragged_sizes_and_waves(n, wave, scheduler, workloads):
