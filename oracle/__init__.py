@@ -60,6 +60,7 @@ def lib():
         _lib.orc_lookup.argtypes = [C.c_void_p, C.c_int32, C.c_double, C.c_double, C.c_double]
         _lib.orc_run.restype = C.c_int
         _lib.orc_run_pathlen.restype = C.c_int
+        _lib.orc_run_moments.restype = C.c_int
     return _lib
 
 
@@ -207,6 +208,37 @@ def run(density, material, voxel_cm, tables, source, n_histories, seed, options:
         raise RuntimeError(f"orc_run failed with code {rc}")
     del keep_t, keep_s
     return Result(edep, dose, cnt.as_dict(), trace)
+
+
+def run_moments(density, material, voxel_cm, tables, source, n_histories, seed, options: Options = None,
+                hist_begin: int = 0, n_threads: int = 0):
+    """History-by-history first and second moments (Eq. 13).  Returns (edep, edep_sq, counters):
+    per voxel the sum over histories of the energy a history deposits, and of its square."""
+    options = options or Options()
+    density = np.ascontiguousarray(density, np.float32)
+    material = np.ascontiguousarray(material, np.uint8)
+    nz, ny, nx = density.shape
+    t, keep_t = _tables_c(tables)
+    s, keep_s = _source_c(source)
+    o = options.c()
+    edep = np.zeros((nz, ny, nx), np.float64)
+    esq = np.zeros((nz, ny, nx), np.float64)
+    cnt = Counters()
+    rc = lib().orc_run_moments(_p(density), _p(material), C.c_int32(nx), C.c_int32(ny), C.c_int32(nz),
+                               C.c_double(float(np.float32(voxel_cm))), C.byref(t), C.byref(o), C.byref(s),
+                               C.c_uint64(hist_begin), C.c_uint64(int(n_histories)), C.c_uint64(seed),
+                               _p(edep), _p(esq), C.byref(cnt), C.c_int32(n_threads))
+    if rc != 0:
+        raise RuntimeError(f"orc_run_moments failed with code {rc}")
+    del keep_t, keep_s
+    return edep, esq, cnt.as_dict()
+
+
+def uncertainty_from_moments(edep, edep_sq, n_histories):
+    """PAPER.md Eq. 13 in energy units per history: sqrt((<e^2> - <e>^2)/(N - 1))."""
+    n = float(n_histories)
+    var = (edep_sq / n - (edep / n) ** 2) / (n - 1.0)
+    return np.sqrt(np.maximum(var, 0.0))
 
 
 def run_workload(w, n_histories=None, options: Options = None, want_trace=False, n_threads=0, hist_begin=0):

@@ -367,6 +367,11 @@ typedef struct {
     int trace_n;
     int want_trace;
     double *pathlen; /* NULL, or where to accumulate the primary electron's path length */
+    /* history-by-history second moment (Eq. 13): NULL unless asked for */
+    double *esq;     /* sum over histories of (energy the history left in the voxel)^2 */
+    double *etmp;    /* energy the current history has left in each voxel so far */
+    size_t *touched; /* voxels the current history has deposited in */
+    size_t n_touched, cap_touched;
 } world_t;
 
 static double tab_photon(const world_t *W, int m, int col, double lnE)
@@ -410,7 +415,18 @@ static size_t vindex(const world_t *W, const int v[3])
 enum { DEP_CONTINUOUS, DEP_CUTOFF };
 static void deposit(world_t *W, const int v[3], double e, int kind)
 {
-    W->edep[vindex(W, v)] += e;
+    const size_t idx = vindex(W, v);
+    W->edep[idx] += e;
+    if (W->esq) {
+        if (W->etmp[idx] == 0.0) {
+            if (W->n_touched == W->cap_touched) {
+                W->cap_touched = W->cap_touched ? 2 * W->cap_touched : 1024;
+                W->touched = (size_t *)realloc(W->touched, sizeof(size_t) * W->cap_touched);
+            }
+            W->touched[W->n_touched++] = idx;
+        }
+        W->etmp[idx] += e;
+    }
     if (kind == DEP_CONTINUOUS) W->c.e_dep_continuous += e; else W->c.e_dep_cutoff += e;
 }
 
@@ -701,7 +717,7 @@ static int run_impl(const float *density, const uint8_t *material, int32_t nx, i
                     int32_t nz, double voxel_cm, const orc_tables *t, const orc_options *opt,
                     const orc_source *src, uint64_t hist_begin, uint64_t n_hist, uint64_t seed,
                     double *edep_out, float *dose_out, uint64_t *trace_out, orc_counters *counters,
-                    int32_t n_threads, double *pathlen_out)
+                    int32_t n_threads, double *pathlen_out, double *edep_sq_out)
 {
     if (!density || !material || !t || !opt || !src || !edep_out) return -1;
     if (nx <= 0 || ny <= 0 || nz <= 0 || voxel_cm <= 0.0) return -1;
@@ -754,6 +770,11 @@ static int run_impl(const float *density, const uint8_t *material, int32_t nx, i
         W->mu_max = mu_max; W->m_e = m_e;
         W->edep = (tid == 0) ? edep_out : (double *)malloc(sizeof(double) * nvox);
         memset(W->edep, 0, sizeof(double) * nvox);
+        if (edep_sq_out) {
+            W->esq = (tid == 0) ? edep_sq_out : (double *)malloc(sizeof(double) * nvox);
+            memset(W->esq, 0, sizeof(double) * nvox);
+            W->etmp = (double *)calloc(nvox, sizeof(double));
+        }
         W->seed = seed;
         W->want_trace = trace_out != NULL;
 #ifdef _OPENMP
@@ -775,6 +796,13 @@ static int run_impl(const float *density, const uint8_t *material, int32_t nx, i
                 if (q.type == 0) photon_history(W, q); else electron_history(W, q);
             }
             if (trace_out) trace_out[ih] = W->trace;
+            /* Eq. 13: the history's contribution to <D^2> is the square of ALL it left in a voxel */
+            for (size_t k = 0; k < W->n_touched; ++k) {
+                const size_t idx = W->touched[k];
+                W->esq[idx] += W->etmp[idx] * W->etmp[idx];
+                W->etmp[idx] = 0.0;
+            }
+            W->n_touched = 0;
         }
     }
 
@@ -788,7 +816,13 @@ static int run_impl(const float *density, const uint8_t *material, int32_t nx, i
         if (k > 0) {
             for (size_t i = 0; i < nvox; ++i) edep_out[i] += W->edep[i];
             free(W->edep);
+            if (W->esq) {
+                for (size_t i = 0; i < nvox; ++i) edep_sq_out[i] += W->esq[i];
+                free(W->esq);
+            }
         }
+        free(W->etmp);
+        free(W->touched);
         const orc_counters *c = &W->c;
         tot.n_histories += c->n_histories;
         tot.photon_flights += c->photon_flights; tot.photon_compton += c->photon_compton;
@@ -819,7 +853,20 @@ int orc_run(const float *density, const uint8_t *material, int32_t nx, int32_t n
             uint64_t *trace_out, orc_counters *counters, int32_t n_threads)
 {
     return run_impl(density, material, nx, ny, nz, voxel_cm, t, opt, src, hist_begin, n_hist, seed,
-                    edep_out, dose_out, trace_out, counters, n_threads, NULL);
+                    edep_out, dose_out, trace_out, counters, n_threads, NULL, NULL);
+}
+
+/* As orc_run, and also the per-voxel sum over histories of the squared energy a history deposits
+ * (edep_sq_out, MeV^2): with edep_out these are N <D> and N <D^2> of PAPER.md Eq. 13 in energy units,
+ * history by history. */
+int orc_run_moments(const float *density, const uint8_t *material, int32_t nx, int32_t ny, int32_t nz,
+                    double voxel_cm, const orc_tables *t, const orc_options *opt, const orc_source *src,
+                    uint64_t hist_begin, uint64_t n_hist, uint64_t seed, double *edep_out,
+                    double *edep_sq_out, orc_counters *counters, int32_t n_threads)
+{
+    if (!edep_sq_out) return -1;
+    return run_impl(density, material, nx, ny, nz, voxel_cm, t, opt, src, hist_begin, n_hist, seed,
+                    edep_out, NULL, NULL, counters, n_threads, NULL, edep_sq_out);
 }
 
 int orc_run_pathlen(const float *density, const uint8_t *material, int32_t nx, int32_t ny,
@@ -830,7 +877,7 @@ int orc_run_pathlen(const float *density, const uint8_t *material, int32_t nx, i
     double *edep = (double *)malloc(sizeof(double) * nvox);
     if (!edep) return -3;
     int rc = run_impl(density, material, nx, ny, nz, voxel_cm, t, opt, src, 0, n_hist, seed, edep,
-                      NULL, NULL, NULL, 1, pathlen_out);
+                      NULL, NULL, NULL, 1, pathlen_out, NULL);
     free(edep);
     return rc;
 }

@@ -111,6 +111,14 @@ int orc_run(const float *density, const uint8_t *material, int32_t nx, int32_t n
             uint64_t hist_begin, uint64_t n_hist, uint64_t seed, double *edep_out,
             float *dose_out, uint64_t *trace_out, orc_counters *counters, int32_t n_threads);
 
+/* As orc_run, plus edep_sq_out[nvox]: the sum over histories of the square of the energy one
+ * history deposits in the voxel (MeV^2).  With edep_out this gives the history-by-history
+ * uncertainty of PAPER.md Eq. 13: Delta D^2 = (<D^2> - <D>^2)/(N - 1). */
+int orc_run_moments(const float *density, const uint8_t *material, int32_t nx, int32_t ny, int32_t nz,
+                    double voxel_cm, const orc_tables *t, const orc_options *opt, const orc_source *src,
+                    uint64_t hist_begin, uint64_t n_hist, uint64_t seed, double *edep_out,
+                    double *edep_sq_out, orc_counters *counters, int32_t n_threads);
+
 /* Mean CSDA path length check helper: total path length travelled by each primary
  * electron track (secondaries excluded) accumulated over a run; n entries. */
 int orc_run_pathlen(const float *density, const uint8_t *material, int32_t nx, int32_t ny,

@@ -2,7 +2,8 @@
 
 Not part of the hot path: these consume finished dose grids.
   gamma_index           Eq. 14-15 (Low & Dempsey), criteria 2 % / 2 mm (L231)
-  relative_uncertainty  Eq. 12 with batch estimates in place of Eq. 13's history-by-history sums
+  relative_uncertainty  Eq. 12 (the per-voxel uncertainty comes from Eq. 13 or from a batch estimate of it)
+  efficiency            Eq. 11
   batch_mean_sigma      mean and standard error over independent batches
   voxel_agreement       fraction of significant voxels within k combined standard errors
 """
@@ -23,6 +24,11 @@ def relative_uncertainty(dose: np.ndarray, sigma: np.ndarray, frac: float = 0.2)
     """Eq. 12: mean relative uncertainty over voxels with D > frac * D_max."""
     sel = dose > frac * dose.max()
     return float(np.mean(sigma[sel] / dose[sel]))
+
+
+def efficiency(s: float, seconds: float) -> float:
+    """Eq. 11: epsilon = 1 / (s^2 T)."""
+    return 1.0 / (s * s * seconds)
 
 
 def voxel_agreement(a, sa, b, sb, frac: float = 0.1, k: float = 3.0) -> float:

@@ -88,3 +88,37 @@ def make_config(i: int, n_histories: Optional[int] = None) -> Workload:
     if n_histories is not None:
         w.n_histories = int(n_histories)
     return w
+
+
+def make_paper_geometry(geom: int, particle: int, n_histories: Optional[int] = None) -> Workload:
+    """The paper's own benchmark cases (Tab. IV-VI): a 64^3 grid of 0.5 cm voxels,
+    a 15 MeV monoenergetic parallel beam, 1e6 histories for electrons and 4e6 for photons.
+      geom 1: water;
+      geom 2: water with a lung box on the axis (electrons: 4 cm long, 4.5 cm wide, from 3 cm depth;
+              photons: 6.5 cm long, 4.5 cm wide, from 5.5 cm);
+      geom 3: slabs (electrons: 2 cm soft tissue, 2 cm lung, 2 cm bone, soft tissue; photons: 3 cm soft
+              tissue, 2 cm lung, 7 cm bone, soft tissue; the text's order, L262-264).
+    The paper does not give the field size: 5 x 5 cm^2 is taken (its Tab. I counts ~120 voxels above 0.2 D_max
+    per depth slice).  Materials are this repository's synthetic ones (materials.py)."""
+    if geom not in (1, 2, 3) or particle not in (PHOTON, ELECTRON):
+        raise ValueError("geom must be 1, 2 or 3 and particle PHOTON or ELECTRON")
+    n, h = 64, 0.5
+    e = particle == ELECTRON
+    if geom == 1:
+        rho, mat = phantoms.homogeneous(n, n, n, 1.0, 0)
+        names = ("water",)
+    elif geom == 2:
+        z0, length = (3.0, 4.0) if e else (5.5, 6.5)
+        rho, mat = phantoms.box_in_background(n, n, n, h, (1.0, 0), (0.26, 1), z0, length, 4.5)
+        names = ("water", "lung")
+    else:
+        slabs = [(4, 1.04, 0), (4, 0.26, 1), (4, 1.85, 2), (None, 1.04, 0)] if e else \
+                [(6, 1.04, 0), (4, 0.26, 1), (14, 1.85, 2), (None, 1.04, 0)]
+        rho, mat = phantoms.z_slabs(n, n, n, slabs)
+        names = ("soft_tissue", "lung", "bone")
+    src = Source(particle, RECTANGLE, 16.0, 16.0, 5.0, 5.0, energy=15.0)
+    w = Workload(f"paper_geom{geom}_15MeV_{'electron' if e else 'photon'}_64", rho, mat, h, _tables(names), src,
+                 1_000_000 if e else 4_000_000, 10 * geom + particle)
+    if n_histories is not None:
+        w.n_histories = int(n_histories)
+    return w

@@ -33,6 +33,25 @@ def z_slabs(nx: int, ny: int, nz: int, slabs):
     return rho, mat
 
 
+def box_in_background(nx: int, ny: int, nz: int, voxel_cm: float, background, box, z0_cm: float, length_cm: float,
+                      width_cm: float):
+    """A box of (density, material) ``box`` inside a phantom of ``background``, centred on the beam axis
+    (the phantom's x-y centre), starting at depth ``z0_cm`` (the paper's lung box).
+    A voxel belongs to the box when its centre lies inside it."""
+    rho, mat = homogeneous(nx, ny, nz, *background)
+    cx, cy = 0.5 * nx * voxel_cm, 0.5 * ny * voxel_cm
+    x = (np.arange(nx) + 0.5) * voxel_cm
+    y = (np.arange(ny) + 0.5) * voxel_cm
+    z = (np.arange(nz) + 0.5) * voxel_cm
+    inx = np.abs(x - cx) < 0.5 * width_cm
+    iny = np.abs(y - cy) < 0.5 * width_cm
+    inz = (z > z0_cm) & (z < z0_cm + length_cm)
+    sel = inz[:, None, None] & iny[None, :, None] & inx[None, None, :]
+    rho[sel] = box[0]
+    mat[sel] = box[1]
+    return rho, mat
+
+
 def ct_like(nx: int, ny: int, nz: int, voxel_cm: float, seed: int = 5, sigma_cm: float = 2.0,
             fractions=(0.10, 0.20, 0.55, 0.15), densities=(0.0012, 0.26, 1.04, 1.85),
             noise: float = 0.03):
