@@ -156,6 +156,21 @@ int gpumcd_run(gpumcd_ctx *ctx, uint64_t n_histories, uint64_t seed, float *dose
 int gpumcd_run_host(gpumcd_ctx *ctx, uint64_t n_histories, uint64_t seed, float *dose_out_host,
                     void *cuda_stream);
 
+/* Dose with its statistical uncertainty (Eq. 11-13).  The n_histories are simulated
+ * in n_batches consecutive batches of (nearly) equal size; with x_b the mean energy per history that
+ * batch b left in a voxel,
+ *     Delta D = sqrt( (<x_b^2> - <x_b>^2) / (n_batches - 1) ) / (rho h^3),
+ * which has the same expectation, sigma_history^2 / N, as Eq. 13's history-by-history sum (the
+ * batches are the independent samples; a warp works on many histories at once, so per-history sums
+ * per voxel do not exist on the device).  The batches cover exactly histories 0 .. n_histories-1, so
+ * dose_out_dev equals the result of gpumcd_run with the same arguments up to fp64 summation order.
+ * dose_out_dev, sigma_out_dev: caller-owned float[nx*ny*nz] on the device, OVERWRITTEN, both in MeV/g
+ * per primary history.  2 <= n_batches <= n_histories.  Counters and the energy tally afterwards are
+ * those of all batches together.  Eq. 12 (s) and Eq. 11 (efficiency) are reductions of these two
+ * grids and are left to the caller. */
+int gpumcd_run_uncertainty(gpumcd_ctx *ctx, uint64_t n_histories, uint32_t n_batches, uint64_t seed,
+                           float *dose_out_dev, float *sigma_out_dev, void *cuda_stream);
+
 /* Photon-only replay run: like gpumcd_run with photon_only = 1 but the output is, per history,
  * the ordered event codes of the primary track, 3 bits each, first event in the low bits, at most
  * 21 events: 1 Compton, 2 photoelectric, 3 pair, 4 escaped, 5 absorbed below P_cut.

@@ -120,6 +120,41 @@ __global__ void k_finalize(const double *__restrict__ edep, const float2 *__rest
     }
 }
 
+// Batch statistics of gpumcd_run_uncertainty (Eq. 13 with batches as the samples): fold the
+// energy tally of one batch of m histories into the running sums and clear it for the next batch.
+//   s1 += e (total energy);  x = e / m (the batch's mean energy per history);  sx += x;  sxx += x^2
+__global__ void k_accumulate_batch(double *__restrict__ edep, double *__restrict__ s1, double *__restrict__ sx,
+                                   double *__restrict__ sxx, size_t nvox, double inv_m)
+{
+    for (size_t i = blockIdx.x * static_cast<size_t>(blockDim.x) + threadIdx.x; i < nvox;
+         i += static_cast<size_t>(gridDim.x) * blockDim.x) {
+        const double e = edep[i];
+        edep[i] = 0.0;
+        const double x = e * inv_m;
+        s1[i] += e;
+        sx[i] += x;
+        sxx[i] += x * x;
+    }
+}
+
+// dose = total energy / mass / histories (H8); Delta D = sqrt((<x^2> - <x>^2) / (B - 1)) / mass (Eq. 13);
+// the energy tally is left holding the total of all batches.
+__global__ void k_finalize_uncertainty(const double *__restrict__ s1, const double *__restrict__ sx,
+                                       const double *__restrict__ sxx, const float2 *__restrict__ phantom,
+                                       size_t nvox, double inv_h3, double inv_n, double n_batches,
+                                       float *__restrict__ dose, float *__restrict__ sigma, double *__restrict__ edep)
+{
+    for (size_t i = blockIdx.x * static_cast<size_t>(blockDim.x) + threadIdx.x; i < nvox;
+         i += static_cast<size_t>(gridDim.x) * blockDim.x) {
+        const double inv_mass = inv_h3 / static_cast<double>(phantom[i].x);
+        const double mean = sx[i] / n_batches;
+        const double var = (sxx[i] / n_batches - mean * mean) / (n_batches - 1.0);
+        dose[i] = static_cast<float>(s1[i] * inv_mass * inv_n);
+        sigma[i] = static_cast<float>(sqrt(fmax(var, 0.0)) * inv_mass);
+        edep[i] = s1[i];
+    }
+}
+
 } // namespace gpumcd
 
 // =============================================================================================
@@ -146,6 +181,7 @@ struct gpumcd_ctx {
     std::vector<float> blob_host;     // host copy of the table blob (majorants are rebuilt per phantom)
     int n_mat = 0, n_E = 0;
     double *edep = nullptr;
+    double *moments = nullptr;        // gpumcd_run_uncertainty: s1 | sx | sxx, nvox each (allocated on first use)
     DevCounters *cnt = nullptr;
     // global particle queues of scheduler 0: PA, PB, EA, EB (scheduler 1 has per-warp stacks instead)
     int n_queues = 4;
@@ -249,6 +285,7 @@ static void destroy_impl(gpumcd_ctx *c)
     cudaFree(c->dose_stage);
     cudaFree(c->table_blob);
     cudaFree(c->edep);
+    cudaFree(c->moments);
     cudaFree(c->cnt);
     cudaFree(c->qcount);
     for (int k = 0; k < kMaxQueues; ++k) { cudaFree(c->qA[k]); cudaFree(c->qB[k]); cudaFree(c->qC[k]); }
@@ -540,13 +577,13 @@ static Params make_params(gpumcd_ctx *ctx, uint64_t seed, uint32_t hist_hi, bool
 
 // Scheduler 0: per wave, fill the source list, then alternate photon and electron
 // passes until both lists are empty; the host reads the list lengths between passes.
-static int run_waves_host_loop(gpumcd_ctx *ctx, uint64_t n_hist, uint64_t seed, bool trace_mode,
+static int run_waves_host_loop(gpumcd_ctx *ctx, uint64_t h_begin, uint64_t n_hist, uint64_t seed, bool trace_mode,
                                unsigned long long *trace, cudaStream_t st)
 {
     enum { PA = 0, PB = 1, EA = 2, EB = 3 };
     int pcur = PA, pnext = PB, ecur = EA, enext = EB;
-    uint64_t h0 = ctx->hist_offset;
-    const uint64_t h_end = ctx->hist_offset + n_hist;
+    uint64_t h0 = h_begin;
+    const uint64_t h_end = h_begin + n_hist;
     while (h0 < h_end) {
         uint64_t n = std::min<uint64_t>(ctx->opt.wave_size, h_end - h0);
         n = std::min<uint64_t>(n, 0x100000000ull - (h0 & 0xffffffffull)); // a wave never straddles 2^32
@@ -595,12 +632,12 @@ static int run_waves_host_loop(gpumcd_ctx *ctx, uint64_t n_hist, uint64_t seed, 
 }
 
 // Scheduler 1: the whole run is one cooperative launch (split only where the history id crosses 2^32).
-static int run_persistent(gpumcd_ctx *ctx, uint64_t n_hist, uint64_t seed, float *dose_dev, unsigned long long *trace,
-                          cudaStream_t st)
+static int run_persistent(gpumcd_ctx *ctx, uint64_t h_begin, uint64_t n_hist, uint64_t seed, float *dose_dev,
+                          unsigned long long *trace, cudaStream_t st)
 {
     const double h3 = static_cast<double>(ctx->h) * ctx->h * ctx->h;
-    uint64_t h0 = ctx->hist_offset;
-    const uint64_t h_end = ctx->hist_offset + n_hist;
+    uint64_t h0 = h_begin;
+    const uint64_t h_end = h_begin + n_hist;
     while (h0 < h_end) {
         uint64_t n = std::min<uint64_t>(h_end - h0, 0x100000000ull - (h0 & 0xffffffffull));
         n = std::min<uint64_t>(n, 0x80000000ull); // the claim counter is 32 bits wide
@@ -640,8 +677,8 @@ static int run_persistent(gpumcd_ctx *ctx, uint64_t n_hist, uint64_t seed, float
     return GPUMCD_OK;
 }
 
-static int run_impl(gpumcd_ctx *ctx, uint64_t n_hist, uint64_t seed, float *dose_dev, unsigned long long *trace_dev,
-                    cudaStream_t st)
+// Bookkeeping and zeroing at the start of a run.
+static int begin_run(gpumcd_ctx *ctx, uint64_t n_hist, unsigned long long *trace_dev, cudaStream_t st)
 {
     if (!ctx) return GPUMCD_ERR_INVALID_ARG;
     if (!ctx->have_source) { set_error(ctx, "gpumcd_run called before gpumcd_set_source"); return GPUMCD_ERR_NO_SOURCE; }
@@ -656,8 +693,16 @@ static int run_impl(gpumcd_ctx *ctx, uint64_t n_hist, uint64_t seed, float *dose
     CK(cudaMemsetAsync(ctx->edep, 0, ctx->nvox * sizeof(double), st));
     CK(cudaMemsetAsync(ctx->cnt, 0, sizeof(DevCounters), st));
     if (trace_dev) CK(cudaMemsetAsync(trace_dev, 0, n_hist * sizeof(unsigned long long), st));
-    if (ctx->opt.scheduler == 1) return run_persistent(ctx, n_hist, seed, dose_dev, trace_dev, st);
-    const int rc = run_waves_host_loop(ctx, n_hist, seed, trace_dev != nullptr, trace_dev, st);
+    return GPUMCD_OK;
+}
+
+// One pass of the whole path over histories [h_begin, h_begin + n_hist): transport with all secondaries,
+// then the total of the tally and (dose_dev != NULL) the dose, normalised by n_hist.
+static int transport(gpumcd_ctx *ctx, uint64_t h_begin, uint64_t n_hist, uint64_t seed, float *dose_dev,
+                     unsigned long long *trace_dev, cudaStream_t st)
+{
+    if (ctx->opt.scheduler == 1) return run_persistent(ctx, h_begin, n_hist, seed, dose_dev, trace_dev, st);
+    const int rc = run_waves_host_loop(ctx, h_begin, n_hist, seed, trace_dev != nullptr, trace_dev, st);
     if (rc != GPUMCD_OK) return rc;
     const double h3 = static_cast<double>(ctx->h) * ctx->h * ctx->h;
     const int grid = static_cast<int>(std::min<size_t>((ctx->nvox + kBlock - 1) / kBlock, 148 * 8));
@@ -666,6 +711,14 @@ static int run_impl(gpumcd_ctx *ctx, uint64_t n_hist, uint64_t seed, float *dose
                                         dose_dev, ctx->cnt); }
     CK(cudaGetLastError());
     return GPUMCD_OK;
+}
+
+static int run_impl(gpumcd_ctx *ctx, uint64_t n_hist, uint64_t seed, float *dose_dev, unsigned long long *trace_dev,
+                    cudaStream_t st)
+{
+    const int rc = begin_run(ctx, n_hist, trace_dev, st);
+    if (rc != GPUMCD_OK) return rc;
+    return transport(ctx, ctx->hist_offset, n_hist, seed, dose_dev, trace_dev, st);
 }
 
 extern "C" int gpumcd_run(gpumcd_ctx *ctx, uint64_t n_histories, uint64_t seed, float *dose_out_dev, void *cuda_stream)
@@ -688,6 +741,43 @@ extern "C" int gpumcd_run_host(gpumcd_ctx *ctx, uint64_t n_histories, uint64_t s
         if (e != cudaSuccess) { set_error(ctx, cudaGetErrorString(e)); rc = GPUMCD_ERR_CUDA; }
     }
     return rc;
+}
+
+extern "C" int gpumcd_run_uncertainty(gpumcd_ctx *ctx, uint64_t n_histories, uint32_t n_batches, uint64_t seed,
+                                      float *dose_out_dev, float *sigma_out_dev, void *cuda_stream)
+{
+    if (!ctx || !dose_out_dev || !sigma_out_dev) return GPUMCD_ERR_INVALID_ARG;
+    if (n_batches < 2 || n_batches > n_histories) {
+        set_error(ctx, "n_batches must be at least 2 and at most n_histories");
+        return GPUMCD_ERR_INVALID_ARG;
+    }
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    int rc = begin_run(ctx, n_histories, nullptr, st);
+    if (rc != GPUMCD_OK) return rc;
+    const size_t nvox = ctx->nvox;
+    if (!ctx->moments) CK(cudaMalloc(&ctx->moments, 3 * nvox * sizeof(double)));
+    CK(cudaMemsetAsync(ctx->moments, 0, 3 * nvox * sizeof(double), st));
+    double *s1 = ctx->moments, *sx = s1 + nvox, *sxx = sx + nvox;
+    const int grid = static_cast<int>(std::min<size_t>((nvox + kBlock - 1) / kBlock, 148 * 8));
+    // batch b simulates histories [h, h + m_b): together the batches cover exactly the histories of a
+    // plain gpumcd_run with the same arguments, so the dose is the same
+    uint64_t h = ctx->hist_offset;
+    for (uint32_t b = 0; b < n_batches; ++b) {
+        const uint64_t m = n_histories / n_batches + (b < n_histories % n_batches ? 1 : 0);
+        rc = transport(ctx, h, m, seed, nullptr, nullptr, st);
+        if (rc != GPUMCD_OK) return rc;
+        { LaunchScope ls(ctx, st, CLS_FINALIZE);
+        k_accumulate_batch<<<grid, kBlock, 0, st>>>(ctx->edep, s1, sx, sxx, nvox, 1.0 / static_cast<double>(m)); }
+        CK(cudaGetLastError());
+        h += m;
+    }
+    const double h3 = static_cast<double>(ctx->h) * ctx->h * ctx->h;
+    { LaunchScope ls(ctx, st, CLS_FINALIZE);
+    k_finalize_uncertainty<<<grid, kBlock, 0, st>>>(s1, sx, sxx, ctx->phantom, nvox, 1.0 / h3,
+                                                    1.0 / static_cast<double>(n_histories), static_cast<double>(n_batches),
+                                                    dose_out_dev, sigma_out_dev, ctx->edep); }
+    CK(cudaGetLastError());
+    return GPUMCD_OK;
 }
 
 extern "C" int gpumcd_run_trace(gpumcd_ctx *ctx, uint64_t n_histories, uint64_t seed, uint64_t *trace_out_dev,
