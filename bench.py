@@ -3,6 +3,7 @@
 
     python bench.py --gpus N --steps K --warmup W            # the CUDA library (this repo)
     python bench.py --impl reference --steps K --warmup W    # the CPU oracle, timed as it stands
+    python bench.py --paper-tables [--steps K]               # PAPER.md Tab. IV-VI measured here (markdown)
 
 A "step" is one gpumcd_run of the whole hot path (source, photon and electron transport with all
 secondaries, tally, finalize) over one batch of synthetic histories.  Workload at N = 1: config 2 of
@@ -171,6 +172,102 @@ def reference_arm(args):
     return 0
 
 
+PAPER_TAB4 = {(1, 1): 0.118, (2, 1): 0.147, (3, 1): 0.162, (1, 0): 0.269, (2, 0): 0.275, (3, 0): 0.366}  # s, GTX480
+
+
+def time_gpu(g, torch, w, n, reps, **opts):
+    """Median device time (ms) of gpumcd_run over ``reps`` runs after three warm-up runs, L2 flushed in between."""
+    dev = torch.device("cuda:0")
+    rho = torch.from_numpy(w.density).to(dev)
+    mat = torch.from_numpy(w.material).to(dev)
+    dose = torch.empty(rho.shape, dtype=torch.float32, device=dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    ts = []
+    with g.gpumcd_create(rho, mat, w.voxel_cm, w.tables, g.gpumcd_default_options(**opts)) as ctx:
+        g.gpumcd_set_source(ctx, w.source)
+        for k in range(reps + 3):
+            flush.fill_(k)
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            a.record()
+            g.gpumcd_run(ctx, n, w.seed + k, dose)
+            b.record()
+            torch.cuda.synchronize()
+            if k >= 3:
+                ts.append(a.elapsed_time(b))
+        c = g.gpumcd_get_counters(ctx)
+    return float(np.median(ts)), c
+
+
+def s_gpu(g, torch, ev, w, n, nb=40):
+    dev = torch.device("cuda:0")
+    rho = torch.from_numpy(w.density).to(dev)
+    mat = torch.from_numpy(w.material).to(dev)
+    dose = torch.empty(rho.shape, dtype=torch.float32, device=dev)
+    sig = torch.empty(rho.shape, dtype=torch.float32, device=dev)
+    with g.gpumcd_create(rho, mat, w.voxel_cm, w.tables) as ctx:
+        g.gpumcd_set_source(ctx, w.source)
+        g.gpumcd_run_uncertainty(ctx, n, nb, w.seed, dose, sig)
+        torch.cuda.synchronize()
+    return ev.relative_uncertainty(dose.cpu().numpy().astype(np.float64), sig.cpu().numpy().astype(np.float64), 0.2)
+
+
+def paper_tables(args):
+    """--paper-tables: PAPER.md Tab. IV, V and VI measured here (markdown on stdout instead of the JSON line).
+    Tab. V's reference systems (EGSnrc, DPM) are not available: the reference is the CPU oracle (this file's
+    cpu_baseline leg), timed on a bounded share of the histories.  Tab. VI's base scheme is scheduler 0."""
+    import torch
+
+    import oracle
+    import paper_1101_1245_b200 as g
+    from paper_1101_1245_b200 import evaluation as ev
+    from paper_1101_1245_b200.inputs import ELECTRON, PHOTON, make_paper_geometry
+
+    assert torch.cuda.is_available(), "needs a CUDA device"
+    cores = os.cpu_count() or 1
+    rows4, rows5, rows6 = [], [], []
+    for particle, pname in ((ELECTRON, "electrons"), (PHOTON, "photons")):
+        for geom in (1, 2, 3):
+            w = make_paper_geometry(geom, particle)
+            n = w.n_histories
+            t1, c = time_gpu(g, torch, w, n, args.steps)
+            t0, _ = time_gpu(g, torch, w, n, args.steps, scheduler=0)
+            ta, _ = time_gpu(g, torch, w, n, args.steps, cta_threads=512)
+            tb, _ = time_gpu(g, torch, w, n, args.steps, cta_threads=1024)
+            s = s_gpu(g, torch, ev, w, n)
+            eps = ev.efficiency(s, t1 * 1e-3)
+            # the oracle on a bounded sample; s scales as 1/sqrt(N) (L334), time as N
+            n_o = max(2000, int(n * args.oracle_fraction))
+            tw = time.perf_counter()
+            e, sq, _ = oracle.run_moments(w.density, w.material, w.voxel_cm, w.tables, w.source, n_o, w.seed)
+            t_o = (time.perf_counter() - tw) * n / n_o
+            mass = w.density.astype(np.float64) * w.voxel_cm ** 3
+            s_o = ev.relative_uncertainty(e / n_o / mass, oracle.uncertainty_from_moments(e, sq, n_o) / mass, 0.2)
+            s_o *= np.sqrt(n_o / n)
+            eps_o = ev.efficiency(s_o, t_o)
+            rows4.append(f"| {pname} | Geom{geom} | {n:.0e} | {t1:.3f} | {n / t1 / 1e3:.1f} | {c['ch_steps'] / t1 / 1e6:.1f} | "
+                         f"{PAPER_TAB4[(geom, particle)] * 1e3:.0f} |")
+            rows5.append(f"| {pname} | Geom{geom} | {t_o:.1f} | {t_o / (t1 * 1e-3):.0f} | {s * 100:.3f} | {s_o * 100:.3f} | "
+                         f"{eps:.3g} | {eps_o:.3g} | {eps / eps_o:.0f} |")
+            rows6.append(f"| {pname} | Geom{geom} | {t0:.3f} | {t0 / t1:.2f} | {t0 / ta:.2f} | {t0 / tb:.2f} |")
+    print("## Tab. IV analogue: absolute times of `gpumcd_run` (device time, CUDA events, median of "
+          f"{args.steps}, L2 flushed between runs)\n")
+    print("| particles | geometry | histories | ms | M histories/s | G CH steps/s | paper, GTX480, ms (context) |")
+    print("|---|---|---|---|---|---|---|")
+    print("\n".join(rows4))
+    print(f"\n## Tab. V analogue: against the CPU oracle on {cores} host cores (timed on "
+          f"{args.oracle_fraction:.0%} of the histories and scaled; a deliberately plain program, not EGSnrc or DPM)\n")
+    print("| particles | geometry | T_oracle, s (scaled) | A = T_oracle / T | s, % (Eq. 12, device, 40 batches) | "
+          "s, % (oracle, history by history, scaled by sqrt(N)) | eps (Eq. 11), 1/s | eps oracle | A_eps |")
+    print("|---|---|---|---|---|---|---|---|---|")
+    print("\n".join(rows5))
+    print("\n## Tab. VI analogue: scheduling strategies against the paper's base scheme (scheduler 0)\n")
+    print("| particles | geometry | T_base = scheduler 0, ms | A, scheduler 1 (default CTA size) | A, 512 threads/SM | A, 1024 threads/SM |")
+    print("|---|---|---|---|---|---|")
+    print("\n".join(rows6))
+
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -186,10 +283,15 @@ def main():
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--paper-tables", action="store_true", help="print PAPER.md Tab. IV-VI measured here (markdown)")
+    ap.add_argument("--oracle-fraction", type=float, default=0.02,
+                    help="--paper-tables: share of the histories the oracle is timed on")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
         return reference_arm(args)
+    if args.paper_tables:
+        return paper_tables(args)
 
     import torch
 

@@ -89,9 +89,9 @@ typedef struct {
                               stack, records; default 1024 (smaller values only make sense in
                               tests of the overflow report; at least 192)                          */
     uint32_t cta_threads;  /* scheduler 1: threads of the persistent kernel's one CTA per SM, 512 or
-                              1024; 0 (default) chooses 512 where the mean density is at least 0.8 of
-                              the largest (few fictitious interactions, little waiting on memory)
-                              and 1024 elsewhere                                                    */
+                              1024; 0 (default) chooses 1024 for a photon source in a phantom whose
+                              mean density is below 0.8 of the largest (most flights end in a
+                              fictitious interaction and wait on memory) and 512 otherwise          */
 } gpumcd_options;
 
 typedef struct {

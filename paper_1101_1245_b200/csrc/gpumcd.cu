@@ -656,9 +656,10 @@ static int run_persistent(gpumcd_ctx *ctx, uint64_t h_begin, uint64_t n_hist, ui
         a.dose = dose_dev;
         a.nvox = ctx->nvox;
         a.finalize = (h0 + n == h_end) ? 1 : 0;
-        // CTA size (see persistent.cuh): 512 threads in a nearly homogeneous phantom, else 1024
+        // CTA size (see persistent.cuh): 1024 threads for a photon beam in a heterogeneous phantom (most
+        // flights end in a fictitious interaction and wait for the phantom fetch), else 512
         int threads = static_cast<int>(ctx->opt.cta_threads);
-        if (threads == 0) threads = ctx->rho_mean_over_max >= 0.8 ? 512 : 1024;
+        if (threads == 0) threads = (ctx->src.particle == 1 || ctx->rho_mean_over_max >= 0.8) ? 512 : 1024;
         a.high = threads == 512 ? 256u : 512u;
         void *args[] = {&a};
         const void *fn;

@@ -34,8 +34,8 @@ namespace cg = cooperative_groups;
 #endif
 // Threads per persistent CTA (one CTA per SM): the kernel is built for 512 (128 registers per
 // thread, no spills, short drain phase: best where flights and steps rarely wait for memory) and
-// for 1024 (64 registers, twice the warps to hide the L2 latency of the phantom fetch: best in
-// heterogeneous phantoms, where most photon flights end in a fictitious interaction).
+// for 1024 (64 registers, twice the warps to hide the L2 latency of the phantom fetch: best for
+// photon beams in heterogeneous phantoms, where most flights end in a fictitious interaction).
 constexpr int kPThreadsMax = 1024;
 constexpr unsigned kFull = 0xffffffffu;
 constexpr unsigned kChunk = 32;            // primaries a warp claims per atomic on the source head
