@@ -33,6 +33,10 @@ if ROOT not in sys.path:
 # thread-instructions one condensed-history step needs at minimum, and the
 # issue peak = 148 SMs x 4 schedulers x 32 lanes x 1 inst/clk x max SM clock.
 ALG_INST_PER_CH_STEP = 330.0
+# dram__bytes_read.sum + dram__bytes_write.sum of k_persistent per launch, from the `ncu --set full` capture
+# summarised in profiles/r01c_ncu_k_persistent_512.md (a profiler figure, per workload; None = not captured).
+# The algorithmic DRAM bytes are the first touch of phantom + tally + dose (42 MB for config 2).
+NCU_DRAM_BYTES_PER_LAUNCH = {"cfg2_15MeV_electron_10x10_water128": 57.0e6 + 106.3e6}
 N_SM, N_SCHED, LANES = 148, 4, 32
 
 
@@ -391,7 +395,8 @@ def main():
     local_ch = ch_steps / world
     achieved = ALG_INST_PER_CH_STEP * local_ch / (ms_e * 1e-3) if ms_e > 0 else None
     roofline = {"bound": "alu", "kernel": "electron transport", "achieved": achieved, "peak": peak_inst,
-                "unit": "thread-inst/s", "frac": (achieved / peak_inst) if achieved else None, "traffic": None,
+                "unit": "thread-inst/s", "frac": (achieved / peak_inst) if achieved else None,
+                "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(w.name) if n == w.n_histories else None,
                 "peak_source": f"148 SMs x 4 x 32 x sm_max_mhz ({peak_kind})",
                 "kernel_ms_per_step": ms_e / args.steps, "kernel_launches_per_step": n_e / args.steps,
                 "kernel_share_of_step": ms_e / t_ms if t_ms else None,
