@@ -29,7 +29,7 @@ class _Tables(C.Structure):
 class _Options(C.Structure):
     _fields_ = [("es_max_cm", C.c_double), ("f_eloss_max", C.c_double),
                 ("boundary_nudge", C.c_double), ("pair_mode", C.c_int32),
-                ("photon_only", C.c_int32), ("majorant_scale", C.c_double)]
+                ("photon_only", C.c_int32), ("majorant_scale", C.c_double), ("hom_tol", C.c_double)]
 
 
 class _Source(C.Structure):
@@ -76,11 +76,12 @@ class Options:
     pair_mode: int = 1
     photon_only: int = 0
     majorant_scale: float = 1.0
+    hom_tol: float = 0.0
 
     def c(self):
         f32 = lambda v: float(np.float32(v))
         return _Options(f32(self.es_max_cm), f32(self.f_eloss_max), f32(self.boundary_nudge), self.pair_mode,
-                        self.photon_only, f32(self.majorant_scale))
+                        self.photon_only, f32(self.majorant_scale), f32(self.hom_tol))
 
 
 def _tables_c(tb):

@@ -573,6 +573,77 @@ static void photon_history(world_t *W, particle_t p)
     }
 }
 
+/* ---------------- multi-voxel steps (R32; the paper's "improvements to the electron-step
+ * algorithm", L364-368, are future work there) ---------------- */
+
+/* Distance from x (inside voxel v) along d to the face through which the ray leaves voxel v; *axis
+ * receives the axis of that face. */
+static double exit_distance(const world_t *W, const double x[3], const double d[3], const int v[3], int *axis)
+{
+    double best = HUGE_VAL;
+    *axis = 0;
+    for (int k = 0; k < 3; ++k) {
+        double dk = HUGE_VAL;
+        if (d[k] > 0.0) dk = ((double)(v[k] + 1) * W->h - x[k]) / d[k];
+        else if (d[k] < 0.0) dk = ((double)v[k] * W->h - x[k]) / d[k];
+        if (dk < best) { best = dk; *axis = k; }
+    }
+    return best < 0.0 ? 0.0 : best;
+}
+
+/* d_hom: distance along d to the first voxel that does not continue the start voxel's medium (other
+ * material, density off by more than hom_tol, or outside the phantom); HUGE_VAL if none within s_max. */
+static double hom_distance(const world_t *W, const double x0[3], const double d[3], const int v0[3], double s_max)
+{
+    const size_t i0 = vindex(W, v0);
+    const int m0 = W->material[i0];
+    const double rho0 = (double)W->density[i0];
+    double x[3] = {x0[0], x0[1], x0[2]};
+    int v[3] = {v0[0], v0[1], v0[2]};
+    double t = 0.0;
+    for (;;) {
+        int axis;
+        const double te = exit_distance(W, x, d, v, &axis);
+        t += te;
+        if (t >= s_max) return HUGE_VAL;
+        for (int k = 0; k < 3; ++k) x[k] += te * d[k];
+        v[axis] += d[axis] > 0.0 ? 1 : -1;
+        x[axis] = (double)(d[axis] > 0.0 ? v[axis] : v[axis] + 1) * W->h; /* exactly on the face */
+        if (v[0] < 0 || v[0] >= W->nx || v[1] < 0 || v[1] >= W->ny || v[2] < 0 || v[2] >= W->nz) return t;
+        const size_t i = vindex(W, v);
+        if (W->material[i] != m0 || fabs((double)W->density[i] - rho0) > W->opt.hom_tol * rho0) return t;
+    }
+}
+
+/* Move x by `len` along d, leaving e_per_cm * (path length) in every voxel crossed.  Path outside the
+ * phantom is credited to the last voxel inside.  x is updated; v is the voxel it started in. */
+static void deposit_along(world_t *W, double x[3], const double d[3], const int v0[3], double len, double e_per_cm)
+{
+    int v[3] = {v0[0], v0[1], v0[2]};
+    double left = len;
+    for (;;) {
+        int axis;
+        const double te = exit_distance(W, x, d, v, &axis);
+        if (te >= left) {
+            deposit(W, v, left * e_per_cm, DEP_CONTINUOUS);
+            for (int k = 0; k < 3; ++k) x[k] += left * d[k];
+            return;
+        }
+        int vn[3] = {v[0], v[1], v[2]};
+        vn[axis] += d[axis] > 0.0 ? 1 : -1;
+        if (vn[0] < 0 || vn[0] >= W->nx || vn[1] < 0 || vn[1] >= W->ny || vn[2] < 0 || vn[2] >= W->nz) {
+            deposit(W, v, left * e_per_cm, DEP_CONTINUOUS); /* the rest of the leg lies outside */
+            for (int k = 0; k < 3; ++k) x[k] += left * d[k];
+            return;
+        }
+        deposit(W, v, te * e_per_cm, DEP_CONTINUOUS);
+        for (int k = 0; k < 3; ++k) x[k] += te * d[k];
+        x[axis] = (double)(d[axis] > 0.0 ? vn[axis] : vn[axis] + 1) * W->h;
+        left -= te;
+        v[0] = vn[0]; v[1] = vn[1]; v[2] = vn[2];
+    }
+}
+
 /* ---------------- electron history: PAPER.md Sec. II.B (L78-139) ---------------- */
 static void electron_history(world_t *W, particle_t p)
 {
@@ -605,6 +676,11 @@ static void electron_history(world_t *W, particle_t p)
         double L0 = rho * tab_electron(W, m, 0, lnT);
         double e_cap = W->opt.f_eloss_max * T / L0; /* R9 */
         if (W->opt.es_max_cm < e_cap) e_cap = W->opt.es_max_cm;
+        const int multi = W->opt.hom_tol > 0.0;
+        if (multi) { /* R32: the boundary that limits the step is the next change of medium along d */
+            d_vox = hom_distance(W, p.x, p.d, v, e_hard < e_cap ? e_hard : e_cap);
+            d_vox += W->opt.boundary_nudge * h;
+        }
         /* Eq. 4: e_s = min{d_vox, e_s-max, e_hard} */
         int hard = (e_hard <= d_vox && e_hard <= e_cap);
         double es = hard ? e_hard : (d_vox < e_cap ? d_vox : e_cap);
@@ -620,10 +696,14 @@ static void electron_history(world_t *W, particle_t p)
             return;
         }
         if (W->pathlen && p.primary) *W->pathlen += es;
-        deposit(W, v, dE, DEP_CONTINUOUS); /* at the hinge, which lies in the step-start voxel (R11) */
-        /* random hinge (L137): first leg zeta e_s */
         double zeta = U(a[1]);
-        for (int k = 0; k < 3; ++k) p.x[k] += zeta * es * p.d[k];
+        if (!multi) {
+            deposit(W, v, dE, DEP_CONTINUOUS); /* at the hinge, which lies in the step-start voxel (R11) */
+            /* random hinge (L137): first leg zeta e_s */
+            for (int k = 0; k < 3; ++k) p.x[k] += zeta * es * p.d[k];
+        } else {
+            deposit_along(W, p.x, p.d, v, zeta * es, dE / es);
+        }
         /* Bielajew's alternate hinge (L139, R12): scattering strength at the energy before
          * or after the loss, chosen by the low bit of a[0] (unused by U) */
         double Tms = (a[0] & 1u) ? T : T - dE;
@@ -637,7 +717,13 @@ static void electron_history(world_t *W, particle_t p)
             memcpy(p.d, dnew, sizeof dnew);
         }
         /* second leg (1 - zeta) e_s (L137 prints (zeta-1): sign garble, R2) */
-        for (int k = 0; k < 3; ++k) p.x[k] += (1.0 - zeta) * es * p.d[k];
+        if (!multi) {
+            for (int k = 0; k < 3; ++k) p.x[k] += (1.0 - zeta) * es * p.d[k];
+        } else {
+            int vh[3];
+            if (!locate(W, p.x, vh)) { vh[0] = v[0]; vh[1] = v[1]; vh[2] = v[2]; } /* hinge within the nudge of the phantom's edge */
+            deposit_along(W, p.x, p.d, vh, (1.0 - zeta) * es, dE / es);
+        }
         p.E = T - dE;
         if (!locate(W, p.x, v)) { W->c.e_escaped += p.E; return; }
         if (!hard) continue;

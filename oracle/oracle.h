@@ -57,6 +57,11 @@ typedef struct {
     int32_t pair_mode;     /* 1: 2m leaves as two 0.511 MeV photons; 0: deposited     */
     int32_t photon_only;   /* 1: every electron is deposited where it is born         */
     double majorant_scale; /* >=1; inflates mu_max and M_e (Woodcock invariance pin)  */
+    double hom_tol;        /* 0: Eq. 4 as printed.  > 0: multi-voxel steps (R32): d_vox
+                              becomes the distance to the first voxel along d whose material
+                              differs or whose density differs by more than hom_tol (relative)
+                              from the start voxel's; the step's energy loss is spread over the
+                              voxels its two legs cross, by path length                     */
 } orc_options;
 
 typedef struct {
