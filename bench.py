@@ -283,6 +283,8 @@ def main():
     ap.add_argument("--scheduler", type=int, default=-1)
     ap.add_argument("--wave", type=int, default=0, help="override wave_size (0 = library default)")
     ap.add_argument("--cta-threads", type=int, default=0, help="override cta_threads (0 = the library's choice)")
+    ap.add_argument("--hom-tol", type=float, default=0.0,
+                    help="multi-voxel electron steps (gpumcd_options.hom_tol; 0 = Eq. 4 as printed, the default)")
     ap.add_argument("--ref-histories", type=int, default=50_000)
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -333,6 +335,8 @@ def main():
         opts["wave_size"] = args.wave
     if args.cta_threads > 0:
         opts["cta_threads"] = args.cta_threads
+    if args.hom_tol > 0:
+        opts["hom_tol"] = args.hom_tol
     opt = g.gpumcd_default_options(**opts)
     ctx = g.gpumcd_create(rho, mat, w.voxel_cm, w.tables, opt)
     g.gpumcd_set_source(ctx, w.source)
@@ -452,7 +456,7 @@ def main():
             "ch_steps_per_s": ch_steps / t_s, "photon_flights_per_s": flights / t_s,
             "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": t_ms / args.steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": {"workload": w.name, "histories_per_step_per_gpu": n, "scheduler": int(opt.scheduler),
+            "config": {"workload": w.name, "histories_per_step_per_gpu": n, "scheduler": int(opt.scheduler), "hom_tol": float(opt.hom_tol),
                        "wave_size": int(opt.wave_size), "l2": "flushed between timed steps (512 MiB write)",
                        "tally": "fp64 atomics", "parallelism": f"histories x{world}"},
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu,

@@ -92,6 +92,15 @@ typedef struct {
                               1024; 0 (default) chooses 1024 for a photon source in a phantom whose
                               mean density is below 0.8 of the largest (most flights end in a
                               fictitious interaction and wait on memory) and 512 otherwise          */
+    float hom_tol;         /* 0 (default): electron steps end at every voxel boundary, Eq. 4 as printed.
+                              > 0: multi-voxel steps (the paper's "improvements to the electron-step
+                              algorithm", L364-368, are future work there; R32): d_vox of
+                              Eq. 4 becomes the distance along the direction of flight to the first
+                              voxel whose material differs from the start voxel's or whose density
+                              differs by more than hom_tol (relative), and the step's energy loss
+                              (Eq. 8) is spread over the voxels its two hinge legs cross, in
+                              proportion to path length.  e_s-max then bounds the step in uniform
+                              regions: 2-2.5 x fewer steps at 0.25 cm voxels                        */
 } gpumcd_options;
 
 typedef struct {

@@ -40,7 +40,7 @@ class gpumcd_options(C.Structure):
     _fields_ = [("es_max_cm", C.c_float), ("f_eloss_max", C.c_float), ("boundary_nudge", C.c_float),
                 ("pair_mode", C.c_int32), ("photon_only", C.c_int32), ("majorant_scale", C.c_float),
                 ("wave_size", C.c_uint32), ("bank_factor", C.c_uint32), ("scheduler", C.c_int32),
-                ("warp_stack", C.c_uint32), ("cta_threads", C.c_uint32)]
+                ("warp_stack", C.c_uint32), ("cta_threads", C.c_uint32), ("hom_tol", C.c_float)]
 
 
 class gpumcd_source(C.Structure):

@@ -86,6 +86,7 @@ __global__ void __launch_bounds__(kBlock) k_photon_pass(Params P, Queue in, unsi
     flush(P, L);
 }
 
+template <bool MULTI>
 __global__ void __launch_bounds__(kBlock) k_electron_pass(Params P, Queue in, unsigned n_in, Queue qE, Queue qG)
 {
     const unsigned i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -93,7 +94,7 @@ __global__ void __launch_bounds__(kBlock) k_electron_pass(Params P, Queue in, un
     if (i < n_in) {
         uint32_t extra;
         const Particle p = load_rec(in.A, in.B, in.C, i, extra);
-        if (p.E >= 0.0f) electron_run(P, p, L, qE, qG);
+        if (p.E >= 0.0f) electron_run<MULTI>(P, p, L, qE, qG);
     }
     flush(P, L);
 }
@@ -272,6 +273,7 @@ extern "C" int gpumcd_default_options(gpumcd_options *opt)
     opt->scheduler = 1;
     opt->warp_stack = 1024;
     opt->cta_threads = 0;
+    opt->hom_tol = 0.0f;
     return GPUMCD_OK;
 }
 
@@ -377,7 +379,7 @@ static int create_impl(gpumcd_ctx **out, const float *density, const uint8_t *ma
     if (opt_in) opt = *opt_in;
     if (!(opt.es_max_cm > 0.f) || !(opt.f_eloss_max > 0.f) || opt.f_eloss_max > 1.f || opt.boundary_nudge < 0.f ||
         !(opt.majorant_scale >= 1.f) || opt.wave_size == 0 || opt.bank_factor == 0 || opt.warp_stack > (1u << 20) ||
-        (opt.cta_threads != 0 && opt.cta_threads != 512 && opt.cta_threads != 1024) ||
+        (opt.cta_threads != 0 && opt.cta_threads != 512 && opt.cta_threads != 1024) || !(opt.hom_tol >= 0.f) ||
         static_cast<unsigned long long>(opt.wave_size) * opt.bank_factor > 0x7fffffffull) {
         set_error(nullptr, "bad options");
         return GPUMCD_ERR_INVALID_ARG;
@@ -444,20 +446,22 @@ static int create_impl(gpumcd_ctx **out, const float *density, const uint8_t *ma
         if (!coop) { set_error(ctx, "device does not support cooperative launches (scheduler 1)"); return GPUMCD_ERR_CUDA; }
         const size_t table_bytes = static_cast<size_t>(ctx->table_floats) * sizeof(float);
         cudaFuncAttributes fa{};
-        CK(cudaFuncGetAttributes(&fa, k_persistent<false, true, 1024>));
+        CK(cudaFuncGetAttributes(&fa, k_persistent<false, true, 1024, false>));
         ctx->smem_tables = table_bytes + fa.sharedSizeBytes + 1024 <= static_cast<size_t>(max_smem);
         const size_t dyn = ctx->smem_tables ? table_bytes : 0;
         if (ctx->smem_tables) {
-            CK(cudaFuncSetAttribute(k_persistent<false, true, 512>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(dyn)));
-            CK(cudaFuncSetAttribute(k_persistent<true, true, 512>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(dyn)));
-            CK(cudaFuncSetAttribute(k_persistent<false, true, 1024>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(dyn)));
-            CK(cudaFuncSetAttribute(k_persistent<true, true, 1024>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(dyn)));
+            CK(cudaFuncSetAttribute(k_persistent<false, true, 512, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(dyn)));
+            CK(cudaFuncSetAttribute(k_persistent<true, true, 512, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(dyn)));
+            CK(cudaFuncSetAttribute(k_persistent<false, true, 1024, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(dyn)));
+            CK(cudaFuncSetAttribute(k_persistent<true, true, 1024, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(dyn)));
+            CK(cudaFuncSetAttribute(k_persistent<false, true, 512, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(dyn)));
+            CK(cudaFuncSetAttribute(k_persistent<false, true, 1024, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(dyn)));
         }
         int per_sm = 0;
         if (ctx->smem_tables)
-            CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_persistent<false, true, 1024>, 1024, dyn));
+            CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_persistent<false, true, 1024, false>, 1024, dyn));
         else
-            CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_persistent<false, false, 1024>, 1024, 0));
+            CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_persistent<false, false, 1024, false>, 1024, 0));
         if (per_sm < 1) { set_error(ctx, "persistent kernel does not fit on an SM"); return GPUMCD_ERR_CUDA; }
         ctx->p_grid = n_sm; // one CTA per SM
         ctx->cap_r = std::max(opt.warp_stack, kMustMargin + 32u);
@@ -563,6 +567,7 @@ static Params make_params(gpumcd_ctx *ctx, uint64_t seed, uint32_t hist_hi, bool
     P.opt.es_max = ctx->opt.es_max_cm;
     P.opt.f_eloss = ctx->opt.f_eloss_max;
     P.opt.nudge = ctx->opt.boundary_nudge;
+    P.opt.hom_tol = ctx->opt.hom_tol;
     P.opt.pair_mode = ctx->opt.pair_mode;
     P.opt.photon_only = photon_only ? 1 : ctx->opt.photon_only;
     P.rng.k0 = static_cast<uint32_t>(seed);
@@ -618,7 +623,10 @@ static int run_waves_host_loop(gpumcd_ctx *ctx, uint64_t h_begin, uint64_t n_his
             } else if (cnt[ecur] > 0) {
                 const unsigned m = cnt[ecur];
                 { LaunchScope ls(ctx, st, CLS_ELECTRON);
-                k_electron_pass<<<(m + kBlock - 1) / kBlock, kBlock, 0, st>>>(P, make_queue(ctx, ecur), m, make_queue(ctx, enext), make_queue(ctx, pcur)); }
+                if (ctx->opt.hom_tol > 0.f)
+                    k_electron_pass<true><<<(m + kBlock - 1) / kBlock, kBlock, 0, st>>>(P, make_queue(ctx, ecur), m, make_queue(ctx, enext), make_queue(ctx, pcur));
+                else
+                    k_electron_pass<false><<<(m + kBlock - 1) / kBlock, kBlock, 0, st>>>(P, make_queue(ctx, ecur), m, make_queue(ctx, enext), make_queue(ctx, pcur)); }
                 CK(cudaGetLastError());
                 CK(cudaMemsetAsync(ctx->qcount + ecur, 0, sizeof(unsigned), st));
                 std::swap(ecur, enext);
@@ -662,13 +670,18 @@ static int run_persistent(gpumcd_ctx *ctx, uint64_t h_begin, uint64_t n_hist, ui
         if (threads == 0) threads = (ctx->src.particle == 1 || ctx->rho_mean_over_max >= 0.8) ? 512 : 1024;
         a.high = threads == 512 ? 256u : 512u;
         void *args[] = {&a};
+        // the kernel variant: trace (photon-only replay) x tables in shared memory x CTA size x multi-voxel steps
+        const bool multi = ctx->opt.hom_tol > 0.f && !trace; // a trace run tracks no electrons
         const void *fn;
-        if (threads == 512) {
-            if (ctx->smem_tables) fn = trace ? (const void *)k_persistent<true, true, 512> : (const void *)k_persistent<false, true, 512>;
-            else fn = trace ? (const void *)k_persistent<true, false, 512> : (const void *)k_persistent<false, false, 512>;
+        if (multi) {
+            if (threads == 512) fn = ctx->smem_tables ? (const void *)k_persistent<false, true, 512, true> : (const void *)k_persistent<false, false, 512, true>;
+            else fn = ctx->smem_tables ? (const void *)k_persistent<false, true, 1024, true> : (const void *)k_persistent<false, false, 1024, true>;
+        } else if (threads == 512) {
+            if (ctx->smem_tables) fn = trace ? (const void *)k_persistent<true, true, 512, false> : (const void *)k_persistent<false, true, 512, false>;
+            else fn = trace ? (const void *)k_persistent<true, false, 512, false> : (const void *)k_persistent<false, false, 512, false>;
         } else {
-            if (ctx->smem_tables) fn = trace ? (const void *)k_persistent<true, true, 1024> : (const void *)k_persistent<false, true, 1024>;
-            else fn = trace ? (const void *)k_persistent<true, false, 1024> : (const void *)k_persistent<false, false, 1024>;
+            if (ctx->smem_tables) fn = trace ? (const void *)k_persistent<true, true, 1024, false> : (const void *)k_persistent<false, true, 1024, false>;
+            else fn = trace ? (const void *)k_persistent<true, false, 1024, false> : (const void *)k_persistent<false, false, 1024, false>;
         }
         const size_t dyn = ctx->smem_tables ? static_cast<size_t>(ctx->table_floats) * sizeof(float) : 0;
         { LaunchScope ls(ctx, st, CLS_ELECTRON);

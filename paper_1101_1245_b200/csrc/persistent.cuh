@@ -240,6 +240,7 @@ struct Warp {
 // Electron mode: the lanes hold electrons due a condensed-history step.  Returns the type to go on
 // with (0 photons, 1 electrons never, -1 nothing left); on return no lane holds a particle.
 // ---------------------------------------------------------------------------------------------
+template <bool MULTI>
 __device__ __forceinline__ int electron_mode(const PersistArgs &a, const float *__restrict__ TB, Warp &w, Claim &cl)
 {
     const Params &P = a.P;
@@ -316,7 +317,7 @@ __device__ __forceinline__ int electron_mode(const PersistArgs &a, const float *
         if (sm == 0u) continue;
         // ---- one condensed-history step for every lane that holds an electron
         int st = ST_ALIVE;
-        if (alive) st = electron_step(P, TB, p, lnT, M);
+        if (alive) st = electron_step<MULTI>(P, TB, p, lnT, M);
         w.count(WC_STEP, sm);
         w.push(P, SK_EH, alive && st == ST_HARD, p, __float_as_uint(M));
         if (st != ST_ALIVE) alive = false;
@@ -409,7 +410,7 @@ __device__ __forceinline__ int photon_mode(const PersistArgs &a, const float *__
 // ---------------------------------------------------------------------------------------------
 // The persistent kernel
 // ---------------------------------------------------------------------------------------------
-template <bool TRACE, bool SMEM_TABLES, int kPThreads>
+template <bool TRACE, bool SMEM_TABLES, int kPThreads, bool MULTI>
 __global__ void __launch_bounds__(kPThreads, 1) k_persistent(const __grid_constant__ PersistArgs a)
 {
     extern __shared__ __align__(128) float smem[];
@@ -446,7 +447,7 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(const __grid_consta
     Claim cl;
     cl.exhausted = (a.n_hist == 0u);
     int type = a.S.particle;
-    while (type >= 0) type = (type == 1) ? electron_mode(a, TB, w, cl) : photon_mode<TRACE>(a, TB, w, cl);
+    while (type >= 0) type = (type == 1) ? electron_mode<MULTI>(a, TB, w, cl) : photon_mode<TRACE>(a, TB, w, cl);
 
     // ---- flush this warp's event counts and accounts
     __syncwarp();

@@ -34,7 +34,7 @@ struct Geom {
 };
 
 struct Opts {
-    float es_max, f_eloss, nudge;
+    float es_max, f_eloss, nudge, hom_tol;
     int pair_mode, photon_only;
 };
 
@@ -376,6 +376,82 @@ __device__ int photon_step(const Params &P, const float *__restrict__ TB, Partic
 // ---------------------------------------------------------------------------------------------
 enum : int { ST_ALIVE = 0, ST_DEAD = 1, ST_HARD = 2 };
 
+// ---- multi-voxel steps (R32; gpumcd_options.hom_tol > 0) ------------------------------
+// Both walk the voxel grid along a direction in the kernels' (voxel, fraction) coordinates, lengths in
+// voxel sizes.  kWalkMax bounds the walk (e_s-max / h voxels are crossed at most, a handful).
+constexpr int kWalkMax = 256;
+
+// distance to the face through which the ray leaves the voxel, and the axis of that face
+__device__ __forceinline__ float exit_distance(float fx, float fy, float fz, float u, float v, float w, int &axis)
+{
+    const float tx = fdiv((u > 0.0f) ? 1.0f - fx : fx, fabsf(u));
+    const float ty = fdiv((v > 0.0f) ? 1.0f - fy : fy, fabsf(v));
+    const float tz = fdiv((w > 0.0f) ? 1.0f - fz : fz, fabsf(w));
+    const float te = fminf(tx, fminf(ty, tz)); // a zero direction cosine gives +inf or NaN: dropped
+    axis = (te == tx) ? 0 : ((te == ty) ? 1 : 2);
+    return fmaxf(te, 0.0f);
+}
+
+// d_hom: distance along the direction to the first voxel that does not continue the start voxel's
+// medium (other material, density off by more than hom_tol, outside the phantom); +inf if none
+// within s_max.
+__device__ __forceinline__ float hom_distance(const Params &P, const Particle &p, float2 pv0, float s_max)
+{
+    float fx = p.fx, fy = p.fy, fz = p.fz, t = 0.0f;
+    int ix = p.ix, iy = p.iy, iz = p.iz;
+    const float band = P.opt.hom_tol * pv0.x;
+    for (int it = 0; it < kWalkMax; ++it) {
+        int axis;
+        const float te = exit_distance(fx, fy, fz, p.u, p.v, p.w, axis);
+        t += te;
+        if (t >= s_max) return __int_as_float(0x7f800000);
+        fx = fmaf(te, p.u, fx); fy = fmaf(te, p.v, fy); fz = fmaf(te, p.w, fz);
+        if (axis == 0) { const bool up = p.u > 0.0f; ix += up ? 1 : -1; fx = up ? 0.0f : 1.0f; }
+        else if (axis == 1) { const bool up = p.v > 0.0f; iy += up ? 1 : -1; fy = up ? 0.0f : 1.0f; }
+        else { const bool up = p.w > 0.0f; iz += up ? 1 : -1; fz = up ? 0.0f : 1.0f; }
+        if (static_cast<unsigned>(ix) >= static_cast<unsigned>(P.geo.nx) ||
+            static_cast<unsigned>(iy) >= static_cast<unsigned>(P.geo.ny) ||
+            static_cast<unsigned>(iz) >= static_cast<unsigned>(P.geo.nz)) return t;
+        const float2 pv = __ldg(&P.geo.phantom[static_cast<unsigned>(ix) + static_cast<unsigned>(P.geo.nx) *
+                                               (static_cast<unsigned>(iy) + static_cast<unsigned>(P.geo.ny) * static_cast<unsigned>(iz))]);
+        if (__float_as_int(pv.y) != __float_as_int(pv0.y) || fabsf(pv.x - pv0.x) > band) return t;
+    }
+    return t;
+}
+
+// Move the particle by `len` along its direction, leaving e_per_len x (path length) in every voxel
+// crossed; path outside the phantom is credited to the last voxel inside.  (voxel, fraction) are
+// renormalised at the end.
+__device__ __forceinline__ void deposit_along(const Params &P, Particle &p, float len, float e_per_len)
+{
+    float left = len;
+    for (int it = 0; it < kWalkMax; ++it) {
+        int axis;
+        const float te = exit_distance(p.fx, p.fy, p.fz, p.u, p.v, p.w, axis);
+        const unsigned lin = voxel_index(P.geo, p);
+        int nx_ = p.ix, ny_ = p.iy, nz_ = p.iz;
+        if (axis == 0) nx_ += (p.u > 0.0f) ? 1 : -1;
+        else if (axis == 1) ny_ += (p.v > 0.0f) ? 1 : -1;
+        else nz_ += (p.w > 0.0f) ? 1 : -1;
+        const bool leaves = static_cast<unsigned>(nx_) >= static_cast<unsigned>(P.geo.nx) ||
+                            static_cast<unsigned>(ny_) >= static_cast<unsigned>(P.geo.ny) ||
+                            static_cast<unsigned>(nz_) >= static_cast<unsigned>(P.geo.nz);
+        if (te >= left || leaves || it == kWalkMax - 1) {
+            deposit(P, lin, left * e_per_len);
+            break;
+        }
+        deposit(P, lin, te * e_per_len);
+        p.fx = fmaf(te, p.u, p.fx); p.fy = fmaf(te, p.v, p.fy); p.fz = fmaf(te, p.w, p.fz);
+        if (axis == 0) p.fx = (p.u > 0.0f) ? 0.0f : 1.0f;
+        else if (axis == 1) p.fy = (p.v > 0.0f) ? 0.0f : 1.0f;
+        else p.fz = (p.w > 0.0f) ? 0.0f : 1.0f;
+        p.ix = nx_; p.iy = ny_; p.iz = nz_;
+        left -= te;
+    }
+    advance(p, left);
+}
+
+template <bool MULTI>
 __device__ __forceinline__ int electron_step(const Params &P, const float *__restrict__ TB, Particle &p, float &lnT,
                                              float &M)
 {
@@ -399,9 +475,13 @@ __device__ __forceinline__ int electron_step(const Params &P, const float *__res
     const float dx = fdiv((p.u > 0.0f) ? 1.0f - p.fx : p.fx, fabsf(p.u));
     const float dy = fdiv((p.v > 0.0f) ? 1.0f - p.fy : p.fy, fabsf(p.v));
     const float dz = fdiv((p.w > 0.0f) ? 1.0f - p.fz : p.fz, fabsf(p.w));
-    const float d_vox = (fminf(dx, fminf(dy, dz)) + P.opt.nudge) * P.geo.h;
     const float L0 = rho * interp(el, iT);
     const float e_cap = fminf(P.opt.es_max, fdiv(P.opt.f_eloss * T, L0));
+    float d_vox;
+    if (MULTI) // R32: the boundary that limits the step is the next change of medium along d
+        d_vox = (hom_distance(P, p, pv, fminf(e_hard, e_cap) * P.geo.inv_h) + P.opt.nudge) * P.geo.h;
+    else
+        d_vox = (fminf(dx, fminf(dy, dz)) + P.opt.nudge) * P.geo.h;
     // Eq. 4
     const bool hard = (e_hard <= d_vox) && (e_hard <= e_cap);
     const float es = hard ? e_hard : fminf(d_vox, e_cap);
@@ -413,16 +493,21 @@ __device__ __forceinline__ int electron_step(const Params &P, const float *__res
         acc.cut(T);
         return ST_DEAD;
     }
-    deposit(P, lin, dE);
     // random hinge (L137): legs zeta*es and (1-zeta)*es around the deflection
     const float zeta = u01(a.y);
     const float esv = es * P.geo.inv_h;
     const float T1 = T - dE;
     const float lnT1 = flog(T1);
     const float leg1 = zeta * esv;
-    p.fx = fmaf(leg1, p.u, p.fx);
-    p.fy = fmaf(leg1, p.v, p.fy);
-    p.fz = fmaf(leg1, p.w, p.fz);
+    const float e_per_v = fdiv(dE, esv); // MULTI: the loss is spread over the path, by length
+    if (MULTI) {
+        deposit_along(P, p, leg1, e_per_v);
+    } else {
+        deposit(P, lin, dE);
+        p.fx = fmaf(leg1, p.u, p.fx);
+        p.fy = fmaf(leg1, p.v, p.fy);
+        p.fz = fmaf(leg1, p.w, p.fz);
+    }
     // Bielajew's alternate hinge (L139): scattering strength before or after the loss
     const float lnTms = (a.x & 1u) ? lnT : lnT1;
     const float K = es * rho * interp(el + 3 * nE, locate(tb.gE, lnTms));
@@ -435,7 +520,12 @@ __device__ __forceinline__ int electron_step(const Params &P, const float *__res
         sincos2pi(u01(a.w), sp, cp);
         rotate(p.u, p.v, p.w, fmaf(-2.0f, mu, 1.0f), 2.0f * sqrtf(mu * (1.0f - mu)), cp, sp, p.u, p.v, p.w);
     }
-    advance(p, (1.0f - zeta) * esv);
+    if (MULTI) {
+        if (inside(P.geo, p)) deposit_along(P, p, (1.0f - zeta) * esv, e_per_v);
+        else advance(p, (1.0f - zeta) * esv); // hinge within the nudge of the phantom's edge
+    } else {
+        advance(p, (1.0f - zeta) * esv);
+    }
     p.E = T1;
     lnT = lnT1;
     if (!inside(P.geo, p)) {
@@ -561,12 +651,13 @@ __device__ void photon_run(const Params &P, Particle p, Local &L, const Queue &q
     }
 }
 
+template <bool MULTI>
 __device__ void electron_run(const Params &P, Particle p, Local &L, const Queue &qE, const Queue &qG)
 {
     float lnT = flog(p.E), M;
     const float *TB = P.tab.blob;
     for (;;) {
-        int st = electron_step(P, TB, p, lnT, M);
+        int st = electron_step<MULTI>(P, TB, p, lnT, M);
         L.steps++;
         if (st == ST_HARD) {
             Particle c;

@@ -1,0 +1,77 @@
+"""-m gpu: multi-voxel electron steps (gpumcd_options.hom_tol > 0, R32) against the oracle's
+implementation of the same algorithm, through the C ABI; BASELINE.json's bars."""
+import numpy as np
+import pytest
+
+import oracle
+from gpu_util import run_gpu
+from paper_1101_1245_b200 import evaluation as ev
+from paper_1101_1245_b200.inputs import ELECTRON, PHOTON, make_config, make_paper_geometry
+
+pytestmark = pytest.mark.gpu
+
+TOL = 0.1
+MV = oracle.Options(hom_tol=TOL)
+INT_KEYS = ("photon_flights", "photon_compton", "photon_photo", "photon_pair", "photon_fict", "ch_steps",
+            "hard_moller", "hard_brems", "hard_fict", "pushes_e", "pushes_g")
+
+
+def total(c):
+    return c["e_dep_continuous"] + c["e_dep_cutoff"]
+
+
+@pytest.mark.parametrize("scheduler", [0, 1])
+@pytest.mark.parametrize("cfg,n", [(2, 300_000), (4, 2_000_000), (5, 2_000_000)])
+def test_dose_parity_with_multi_voxel_steps(cfg, n, scheduler):
+    w = make_config(cfg)
+    nb = 4
+    gs, os_, cg, co = [], [], None, None
+    for b in range(nb):
+        g = run_gpu(w, n // nb, seed=w.seed + 1000 * b, scheduler=scheduler, hom_tol=TOL)
+        o = oracle.run(w.density, w.material, w.voxel_cm, w.tables, w.source, n // nb, seed=w.seed + 1000 * b, options=MV)
+        gs.append(g["edep"]); os_.append(o.edep)
+        cg = g["counters"] if cg is None else {k: cg[k] + v for k, v in g["counters"].items()}
+        co = o.counters if co is None else {k: co[k] + v for k, v in o.counters.items()}
+    for k in INT_KEYS:
+        assert abs(cg[k] - co[k]) <= 10 + 2e-3 * co[k], k
+    assert cg["overflow_count"] == 0
+    # energy conservation on the device and agreement of the total with the oracle
+    out = total(cg) + cg["e_escaped"]
+    assert abs(out / cg["e_incident"] - 1.0) <= 1e-6
+    assert total(cg) == pytest.approx(total(co), rel=5e-5)
+    gm, gsig = ev.batch_mean_sigma(np.stack(gs))
+    om, osig = ev.batch_mean_sigma(np.stack(os_))
+    assert ev.voxel_agreement(om, osig, gm, gsig, frac=0.1, k=3.0) >= 0.99
+    mass = w.density.astype(np.float64) * w.voxel_cm ** 3
+    assert ev.gamma_pass_rate(om / mass, gm / mass, w.voxel_cm, frac=0.1) >= 0.99
+    # replay fidelity: the two sides follow the same histories, so they differ by far less than noise
+    sel = om > 0.1 * om.max()
+    assert np.sqrt(np.mean((gm[sel] - om[sel]) ** 2)) < 0.35 * np.sqrt(np.mean(osig[sel] ** 2)) * np.sqrt(nb)
+
+
+def test_steps_are_fewer_and_schedulers_agree():
+    w = make_config(2)
+    a = run_gpu(w, 40_000, scheduler=1)
+    b = run_gpu(w, 40_000, scheduler=1, hom_tol=TOL)
+    c = run_gpu(w, 40_000, scheduler=0, hom_tol=TOL)
+    d = run_gpu(w, 40_000, scheduler=1, hom_tol=TOL, cta_threads=1024)
+    assert a["counters"]["ch_steps"] > 2.0 * b["counters"]["ch_steps"]
+    for k in INT_KEYS:
+        assert b["counters"][k] == c["counters"][k] == d["counters"][k], k
+    assert np.abs(b["edep"] - c["edep"]).max() <= 1e-12 * b["edep"].max()
+    assert np.abs(b["edep"] - d["edep"]).max() <= 1e-12 * b["edep"].max()
+
+
+def test_paper_slab_geometry_with_multi_voxel_steps():
+    """Geom3 (soft tissue / lung / bone slabs): steps must end at every change of medium."""
+    w = make_paper_geometry(3, ELECTRON)
+    n = w.n_histories
+    g = run_gpu(w, n, hom_tol=TOL)
+    o = oracle.run_workload(w, n, MV)
+    for k in INT_KEYS:
+        assert abs(g["counters"][k] - o.counters[k]) <= 10 + 2e-3 * o.counters[k], k
+    assert total(g["counters"]) == pytest.approx(total(o.counters), rel=3e-5)
+    assert ev.gamma_pass_rate(o.dose.astype(np.float64), g["dose"].astype(np.float64), w.voxel_cm, frac=0.1) >= 0.99
+    # planar depth-dose: identical within 0.2 % of the maximum
+    dg, do = g["edep"].sum(axis=(1, 2)), o.edep.sum(axis=(1, 2))
+    assert np.abs(dg - do).max() <= 2e-3 * do.max()
