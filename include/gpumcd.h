@@ -98,9 +98,10 @@ typedef struct {
                               Eq. 4 becomes the distance along the direction of flight to the first
                               voxel whose material differs from the start voxel's or whose density
                               differs by more than hom_tol (relative), and the step's energy loss
-                              (Eq. 8) is spread over the voxels its two hinge legs cross, in
-                              proportion to path length.  e_s-max then bounds the step in uniform
-                              regions: 2-2.5 x fewer steps at 0.25 cm voxels                        */
+                              (Eq. 8) is deposited in the voxel of a point drawn uniformly along
+                              the path of its two hinge legs (every voxel's path-length share in
+                              expectation).  e_s-max then bounds the step in uniform regions:
+                              2-2.5 x fewer steps at 0.25 cm voxels                                 */
 } gpumcd_options;
 
 typedef struct {

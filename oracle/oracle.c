@@ -615,33 +615,12 @@ static double hom_distance(const world_t *W, const double x0[3], const double d[
     }
 }
 
-/* Move x by `len` along d, leaving e_per_cm * (path length) in every voxel crossed.  Path outside the
- * phantom is credited to the last voxel inside.  x is updated; v is the voxel it started in. */
-static void deposit_along(world_t *W, double x[3], const double d[3], const int v0[3], double len, double e_per_cm)
+/* The uniform of the deposit point (R32): 23 bits from the low 9 bits of the step block's words 1-3,
+ * which U() does not use (word 0's low bit chooses the hinge alternative). */
+static double U_low(const uint32_t a[4])
 {
-    int v[3] = {v0[0], v0[1], v0[2]};
-    double left = len;
-    for (;;) {
-        int axis;
-        const double te = exit_distance(W, x, d, v, &axis);
-        if (te >= left) {
-            deposit(W, v, left * e_per_cm, DEP_CONTINUOUS);
-            for (int k = 0; k < 3; ++k) x[k] += left * d[k];
-            return;
-        }
-        int vn[3] = {v[0], v[1], v[2]};
-        vn[axis] += d[axis] > 0.0 ? 1 : -1;
-        if (vn[0] < 0 || vn[0] >= W->nx || vn[1] < 0 || vn[1] >= W->ny || vn[2] < 0 || vn[2] >= W->nz) {
-            deposit(W, v, left * e_per_cm, DEP_CONTINUOUS); /* the rest of the leg lies outside */
-            for (int k = 0; k < 3; ++k) x[k] += left * d[k];
-            return;
-        }
-        deposit(W, v, te * e_per_cm, DEP_CONTINUOUS);
-        for (int k = 0; k < 3; ++k) x[k] += te * d[k];
-        x[axis] = (double)(d[axis] > 0.0 ? vn[axis] : vn[axis] + 1) * W->h;
-        left -= te;
-        v[0] = vn[0]; v[1] = vn[1]; v[2] = vn[2];
-    }
+    uint32_t bits = (a[1] & 0x1ffu) | ((a[2] & 0x1ffu) << 9) | ((a[3] & 0x1fu) << 18);
+    return ((double)bits + 0.5) * (1.0 / 8388608.0);
 }
 
 /* ---------------- electron history: PAPER.md Sec. II.B (L78-139) ---------------- */
@@ -697,13 +676,19 @@ static void electron_history(world_t *W, particle_t p)
         }
         if (W->pathlen && p.primary) *W->pathlen += es;
         double zeta = U(a[1]);
+        /* R32: the loss of a multi-voxel step goes to the voxel of a point drawn uniformly along the
+         * step's path (first leg, then second leg): the path-length share of every voxel in expectation */
+        const double s_dep = multi ? U_low(a) * es : 0.0;
         if (!multi) {
             deposit(W, v, dE, DEP_CONTINUOUS); /* at the hinge, which lies in the step-start voxel (R11) */
-            /* random hinge (L137): first leg zeta e_s */
-            for (int k = 0; k < 3; ++k) p.x[k] += zeta * es * p.d[k];
-        } else {
-            deposit_along(W, p.x, p.d, v, zeta * es, dE / es);
+        } else if (s_dep <= zeta * es) {
+            double xd[3];
+            int vd[3];
+            for (int k = 0; k < 3; ++k) xd[k] = p.x[k] + s_dep * p.d[k];
+            deposit(W, locate(W, xd, vd) ? vd : v, dE, DEP_CONTINUOUS);
         }
+        /* random hinge (L137): first leg zeta e_s */
+        for (int k = 0; k < 3; ++k) p.x[k] += zeta * es * p.d[k];
         /* Bielajew's alternate hinge (L139, R12): scattering strength at the energy before
          * or after the loss, chosen by the low bit of a[0] (unused by U) */
         double Tms = (a[0] & 1u) ? T : T - dE;
@@ -717,13 +702,13 @@ static void electron_history(world_t *W, particle_t p)
             memcpy(p.d, dnew, sizeof dnew);
         }
         /* second leg (1 - zeta) e_s (L137 prints (zeta-1): sign garble, R2) */
-        if (!multi) {
-            for (int k = 0; k < 3; ++k) p.x[k] += (1.0 - zeta) * es * p.d[k];
-        } else {
-            int vh[3];
-            if (!locate(W, p.x, vh)) { vh[0] = v[0]; vh[1] = v[1]; vh[2] = v[2]; } /* hinge within the nudge of the phantom's edge */
-            deposit_along(W, p.x, p.d, vh, (1.0 - zeta) * es, dE / es);
+        if (multi && s_dep > zeta * es) {
+            double xd[3];
+            int vd[3];
+            for (int k = 0; k < 3; ++k) xd[k] = p.x[k] + (s_dep - zeta * es) * p.d[k];
+            deposit(W, locate(W, xd, vd) ? vd : v, dE, DEP_CONTINUOUS); /* a point outside: the start voxel */
         }
+        for (int k = 0; k < 3; ++k) p.x[k] += (1.0 - zeta) * es * p.d[k];
         p.E = T - dE;
         if (!locate(W, p.x, v)) { W->c.e_escaped += p.E; return; }
         if (!hard) continue;

@@ -60,8 +60,8 @@ typedef struct {
     double hom_tol;        /* 0: Eq. 4 as printed.  > 0: multi-voxel steps (R32): d_vox
                               becomes the distance to the first voxel along d whose material
                               differs or whose density differs by more than hom_tol (relative)
-                              from the start voxel's; the step's energy loss is spread over the
-                              voxels its two legs cross, by path length                     */
+                              from the start voxel's; the step's energy loss goes to the voxel
+                              of a point drawn uniformly along the path of its two legs     */
 } orc_options;
 
 typedef struct {

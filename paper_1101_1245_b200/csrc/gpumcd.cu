@@ -47,6 +47,36 @@ __global__ void k_pack_phantom(const float *__restrict__ density, const uint8_t 
     if (threadIdx.x < 8 && s_max[threadIdx.x]) atomicMax(&rho_max_bits[threadIdx.x], s_max[threadIdx.x]);
 }
 
+// Multi-voxel steps (hom_tol > 0): the uniform radius of every voxel, R = the largest r <= r_max such that
+// all voxels within Chebyshev distance r lie inside the phantom and continue the voxel's medium (same
+// material, |density - own| <= hom_tol * own); stored in bits 8-10 of the record's material word.
+__global__ void k_uniform_radius(float2 *__restrict__ phantom, int nx, int ny, int nz, float hom_tol, int r_max)
+{
+    const size_t nvox = static_cast<size_t>(nx) * ny * nz;
+    for (size_t i = blockIdx.x * static_cast<size_t>(blockDim.x) + threadIdx.x; i < nvox;
+         i += static_cast<size_t>(gridDim.x) * blockDim.x) {
+        const int ix = static_cast<int>(i % nx), iy = static_cast<int>((i / nx) % ny), iz = static_cast<int>(i / (static_cast<size_t>(nx) * ny));
+        const float2 pv0 = phantom[i];
+        const int m0 = __float_as_int(pv0.y) & 0xff;
+        const float band = hom_tol * pv0.x;
+        int R = 0;
+        for (int r = 1; r <= r_max; ++r) {
+            bool ok = ix - r >= 0 && ix + r < nx && iy - r >= 0 && iy + r < ny && iz - r >= 0 && iz + r < nz;
+            for (int dz = -r; ok && dz <= r; ++dz)
+                for (int dy = -r; ok && dy <= r; ++dy) {
+                    const bool shell_row = (dz == -r || dz == r || dy == -r || dy == r);
+                    for (int dx = -r; ok && dx <= r; dx += (shell_row ? 1 : 2 * r)) { // the shell at distance r only
+                        const float2 pv = phantom[static_cast<size_t>(ix + dx) + static_cast<size_t>(nx) * ((iy + dy) + static_cast<size_t>(ny) * (iz + dz))];
+                        ok = ((__float_as_int(pv.y) & 0xff) == m0) && fabsf(pv.x - pv0.x) <= band;
+                    }
+                }
+            if (!ok) break;
+            R = r;
+        }
+        reinterpret_cast<int *>(phantom)[2 * i + 1] = m0 | (R << 8);
+    }
+}
+
 // H0: one primary per history from block (hist, track 0, ctr 0); transport starts at ctr 1.
 __global__ void k_source(Params P, SourceDev S, Queue q, unsigned long long hist0, unsigned n)
 {
@@ -323,6 +353,11 @@ static int load_phantom(gpumcd_ctx *ctx, const float *density, const uint8_t *ma
     k_pack_phantom<<<grid, kBlock>>>(d_density, d_material, nvox, ctx->n_mat, ctx->phantom, ctx->scratch, ctx->scratch + 8,
                                    reinterpret_cast<double *>(ctx->scratch + 10));
     CK(cudaGetLastError());
+    if (ctx->opt.hom_tol > 0.f) {
+        const int r_max = std::min(7, static_cast<int>(std::ceil(ctx->opt.es_max_cm / ctx->h)) + 1);
+        k_uniform_radius<<<grid, kBlock>>>(ctx->phantom, ctx->nx, ctx->ny, ctx->nz, ctx->opt.hom_tol, r_max);
+        CK(cudaGetLastError());
+    }
     unsigned h_scratch[12];
     CK(cudaMemcpy(h_scratch, ctx->scratch, sizeof h_scratch, cudaMemcpyDeviceToHost));
     if (h_scratch[8] != 0) {

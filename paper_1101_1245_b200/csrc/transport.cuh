@@ -87,6 +87,13 @@ struct Acc {
     __device__ __forceinline__ void inc(double e) const { atomicAdd(&slot()->e_inc, e); }
 };
 
+// Phantom record: x = density, y = bits: material id in the low 8 bits; bits 8-10 (multi-voxel steps
+// only, else 0) = the uniform radius R of the voxel: every voxel within Chebyshev distance R continues
+// its medium (same material, density within hom_tol), so no ray from inside it meets a change of
+// medium before R voxel sizes.
+__device__ __forceinline__ int mat_of(float2 pv) { return __float_as_int(pv.y) & 0xff; }
+__device__ __forceinline__ int radius_of(float2 pv) { return (__float_as_int(pv.y) >> 8) & 7; }
+
 __device__ __forceinline__ bool inside(const Geom &g, const Particle &p)
 {
     return (static_cast<unsigned>(p.ix) < static_cast<unsigned>(g.nx)) &
@@ -234,7 +241,7 @@ __device__ __forceinline__ int photon_flight(const Params &P, const float *__res
     }
     const float2 pv = __ldg(&P.geo.phantom[voxel_index(P.geo, p)]);
     const float rho = pv.x;
-    const float *col = TB + __float_as_int(pv.y) * 3 * tb.gE.n;
+    const float *col = TB + mat_of(pv) * 3 * tb.gE.n;
     const float r = u01(w.y) * mu_max;
     const float c1 = rho * interp(col, iE);
     const float c2 = fmaf(rho, interp(col + tb.gE.n, iE), c1);
@@ -397,6 +404,8 @@ __device__ __forceinline__ float exit_distance(float fx, float fy, float fz, flo
 // within s_max.
 __device__ __forceinline__ float hom_distance(const Params &P, const Particle &p, float2 pv0, float s_max)
 {
+    // the voxel's uniform radius (precomputed per phantom) answers most look-aheads without a walk
+    if (s_max < static_cast<float>(radius_of(pv0))) return __int_as_float(0x7f800000);
     float fx = p.fx, fy = p.fy, fz = p.fz, t = 0.0f;
     int ix = p.ix, iy = p.iy, iz = p.iz;
     const float band = P.opt.hom_tol * pv0.x;
@@ -414,41 +423,22 @@ __device__ __forceinline__ float hom_distance(const Params &P, const Particle &p
             static_cast<unsigned>(iz) >= static_cast<unsigned>(P.geo.nz)) return t;
         const float2 pv = __ldg(&P.geo.phantom[static_cast<unsigned>(ix) + static_cast<unsigned>(P.geo.nx) *
                                                (static_cast<unsigned>(iy) + static_cast<unsigned>(P.geo.ny) * static_cast<unsigned>(iz))]);
-        if (__float_as_int(pv.y) != __float_as_int(pv0.y) || fabsf(pv.x - pv0.x) > band) return t;
+        if (mat_of(pv) != mat_of(pv0) || fabsf(pv.x - pv0.x) > band) return t;
     }
     return t;
 }
 
-// Move the particle by `len` along its direction, leaving e_per_len x (path length) in every voxel
-// crossed; path outside the phantom is credited to the last voxel inside.  (voxel, fraction) are
-// renormalised at the end.
-__device__ __forceinline__ void deposit_along(const Params &P, Particle &p, float len, float e_per_len)
+// The voxel of the point a distance t (voxel sizes) along the direction from the particle's position, or
+// `fallback` if that point lies outside the phantom.
+__device__ __forceinline__ unsigned voxel_ahead(const Geom &g, const Particle &p, float t, unsigned fallback)
 {
-    float left = len;
-    for (int it = 0; it < kWalkMax; ++it) {
-        int axis;
-        const float te = exit_distance(p.fx, p.fy, p.fz, p.u, p.v, p.w, axis);
-        const unsigned lin = voxel_index(P.geo, p);
-        int nx_ = p.ix, ny_ = p.iy, nz_ = p.iz;
-        if (axis == 0) nx_ += (p.u > 0.0f) ? 1 : -1;
-        else if (axis == 1) ny_ += (p.v > 0.0f) ? 1 : -1;
-        else nz_ += (p.w > 0.0f) ? 1 : -1;
-        const bool leaves = static_cast<unsigned>(nx_) >= static_cast<unsigned>(P.geo.nx) ||
-                            static_cast<unsigned>(ny_) >= static_cast<unsigned>(P.geo.ny) ||
-                            static_cast<unsigned>(nz_) >= static_cast<unsigned>(P.geo.nz);
-        if (te >= left || leaves || it == kWalkMax - 1) {
-            deposit(P, lin, left * e_per_len);
-            break;
-        }
-        deposit(P, lin, te * e_per_len);
-        p.fx = fmaf(te, p.u, p.fx); p.fy = fmaf(te, p.v, p.fy); p.fz = fmaf(te, p.w, p.fz);
-        if (axis == 0) p.fx = (p.u > 0.0f) ? 0.0f : 1.0f;
-        else if (axis == 1) p.fy = (p.v > 0.0f) ? 0.0f : 1.0f;
-        else p.fz = (p.w > 0.0f) ? 0.0f : 1.0f;
-        p.ix = nx_; p.iy = ny_; p.iz = nz_;
-        left -= te;
-    }
-    advance(p, left);
+    const int ix = p.ix + static_cast<int>(floorf(fmaf(t, p.u, p.fx)));
+    const int iy = p.iy + static_cast<int>(floorf(fmaf(t, p.v, p.fy)));
+    const int iz = p.iz + static_cast<int>(floorf(fmaf(t, p.w, p.fz)));
+    const bool in = (static_cast<unsigned>(ix) < static_cast<unsigned>(g.nx)) & (static_cast<unsigned>(iy) < static_cast<unsigned>(g.ny)) &
+                    (static_cast<unsigned>(iz) < static_cast<unsigned>(g.nz));
+    return in ? static_cast<unsigned>(ix) + static_cast<unsigned>(g.nx) * (static_cast<unsigned>(iy) + static_cast<unsigned>(g.ny) * static_cast<unsigned>(iz))
+              : fallback;
 }
 
 template <bool MULTI>
@@ -461,7 +451,7 @@ __device__ __forceinline__ int electron_step(const Params &P, const float *__res
     const unsigned lin = voxel_index(P.geo, p);
     const float2 pv = __ldg(&P.geo.phantom[lin]);
     const float rho = pv.x;
-    const float *el = TB + tb.off_el + __float_as_int(pv.y) * 4 * nE;
+    const float *el = TB + tb.off_el + mat_of(pv) * 4 * nE;
     const float T = p.E;
     const uint4 a = draw(P.rng, p);
     const Interp iT = locate(tb.gE, lnT);
@@ -499,15 +489,20 @@ __device__ __forceinline__ int electron_step(const Params &P, const float *__res
     const float T1 = T - dE;
     const float lnT1 = flog(T1);
     const float leg1 = zeta * esv;
-    const float e_per_v = fdiv(dE, esv); // MULTI: the loss is spread over the path, by length
+    // R32: the loss of a multi-voxel step goes to the voxel of a point drawn uniformly along the step's
+    // path (first leg, then second leg); its uniform comes from the low bits of a.y, a.z, a.w that u01
+    // does not use
+    float s_dep = 0.0f;
     if (MULTI) {
-        deposit_along(P, p, leg1, e_per_v);
+        const uint32_t bits = (a.y & 0x1ffu) | ((a.z & 0x1ffu) << 9) | ((a.w & 0x1fu) << 18);
+        s_dep = fmaf(__uint2float_rz(bits), 1.0f / 8388608.0f, 1.0f / 16777216.0f) * esv;
+        if (s_dep <= leg1) deposit(P, voxel_ahead(P.geo, p, s_dep, lin), dE);
     } else {
         deposit(P, lin, dE);
-        p.fx = fmaf(leg1, p.u, p.fx);
-        p.fy = fmaf(leg1, p.v, p.fy);
-        p.fz = fmaf(leg1, p.w, p.fz);
     }
+    p.fx = fmaf(leg1, p.u, p.fx);
+    p.fy = fmaf(leg1, p.v, p.fy);
+    p.fz = fmaf(leg1, p.w, p.fz);
     // Bielajew's alternate hinge (L139): scattering strength before or after the loss
     const float lnTms = (a.x & 1u) ? lnT : lnT1;
     const float K = es * rho * interp(el + 3 * nE, locate(tb.gE, lnTms));
@@ -520,12 +515,8 @@ __device__ __forceinline__ int electron_step(const Params &P, const float *__res
         sincos2pi(u01(a.w), sp, cp);
         rotate(p.u, p.v, p.w, fmaf(-2.0f, mu, 1.0f), 2.0f * sqrtf(mu * (1.0f - mu)), cp, sp, p.u, p.v, p.w);
     }
-    if (MULTI) {
-        if (inside(P.geo, p)) deposit_along(P, p, (1.0f - zeta) * esv, e_per_v);
-        else advance(p, (1.0f - zeta) * esv); // hinge within the nudge of the phantom's edge
-    } else {
-        advance(p, (1.0f - zeta) * esv);
-    }
+    if (MULTI && s_dep > leg1) deposit(P, voxel_ahead(P.geo, p, s_dep - leg1, lin), dE);
+    advance(p, (1.0f - zeta) * esv);
     p.E = T1;
     lnT = lnT1;
     if (!inside(P.geo, p)) {
@@ -551,7 +542,7 @@ __device__ __forceinline__ int electron_hard(const Params &P, const float *__res
     const uint4 b = draw(P.rng, p);
     const unsigned lin1 = voxel_index(P.geo, p);
     const float2 pv1 = __ldg(&P.geo.phantom[lin1]);
-    const float *el1 = TB + tb.off_el + __float_as_int(pv1.y) * 4 * nE;
+    const float *el1 = TB + tb.off_el + mat_of(pv1) * 4 * nE;
     const Interp i1 = locate(tb.gE, lnT);
     const float sM = pv1.x * interp(el1 + nE, i1);
     const float sB = pv1.x * interp(el1 + 2 * nE, i1);

@@ -75,3 +75,22 @@ def test_paper_slab_geometry_with_multi_voxel_steps():
     # planar depth-dose: identical within 0.2 % of the maximum
     dg, do = g["edep"].sum(axis=(1, 2)), o.edep.sum(axis=(1, 2))
     assert np.abs(dg - do).max() <= 2e-3 * do.max()
+
+
+@pytest.mark.parametrize("cfg,n", [(2, 4_000_000), (4, 20_000_000)])
+def test_multi_voxel_dose_is_the_dose_of_the_eq4_transport(cfg, n):
+    """Longer steps, same physics.  Where the noise is small enough to tell (laterally integrated depth dose,
+    the 2 x 2 cm^2 column around the axis) the two step algorithms agree within 1 % / 1.5 % of the maximum:
+    the step-size artefact of 0.5 cm steps is a ~0.2 mm shift of the fall-off, far below 2 % / 2 mm.
+    (Voxel by voxel two Eq. 4 runs with different seeds differ more than that at these sizes.)"""
+    w = make_config(cfg)
+    a = run_gpu(w, n)
+    b = run_gpu(w, n, hom_tol=TOL)
+    assert b["counters"]["ch_steps"] < 0.62 * a["counters"]["ch_steps"]
+    da, db = a["edep"].sum(axis=(1, 2)), b["edep"].sum(axis=(1, 2))
+    assert np.abs(da - db).max() <= 0.01 * da.max()
+    ny, nx = a["edep"].shape[1:]
+    col = (slice(None), slice(ny // 2 - 4, ny // 2 + 4), slice(nx // 2 - 4, nx // 2 + 4))
+    ca, cb = a["edep"][col].sum(axis=(1, 2)), b["edep"][col].sum(axis=(1, 2))
+    assert np.abs(ca - cb).max() <= 0.015 * ca.max()
+    assert total(b["counters"]) == pytest.approx(total(a["counters"]), rel=2e-3)

@@ -60,15 +60,16 @@ def test_csda_range_is_unchanged(T0, slab_tables_csda):
 def test_depth_profile_in_slabs_follows_the_csda_equation(slab_tables_csda):
     """No scattering, no hard events, normal incidence: dT/dz = -rho(z) L_m(z)(T) exactly; the energy left
     in voxel j is T(z_j) - T(z_j+1).  A multi-voxel step must stop at every change of medium (water ->
-    bone -> lung -> water) and spread its loss over the voxels it crosses."""
+    bone -> lung -> water), and its loss, put at a point drawn uniformly along the step, must give every
+    voxel its path-length share in the mean over histories."""
     tb = slab_tables_csda
-    h, nz = 0.25, 64
+    h, nz, n = 0.25, 64, 20000
     slabs = [(6, 1.0, 0), (4, 1.85, 1), (12, 0.26, 2), (None, 1.0, 0)]
     rho, mat = phantoms.z_slabs(1, 1, nz, slabs)
     src = Source(ELECTRON, PENCIL, 0.125, 0.125, energy=15.0)
-    r = oracle.run(rho, mat, h, tb, src, 1, seed=3, options=MV)
+    r = oracle.run(rho, mat, h, tb, src, n, seed=3, options=MV)
     r4 = oracle.run(rho, mat, h, tb, src, 1, seed=3)
-    assert r.counters["ch_steps"] < 0.7 * r4.counters["ch_steps"]
+    assert r.counters["ch_steps"] / n < 0.7 * r4.counters["ch_steps"]
     lnE = np.linspace(np.log(tb.e_min), np.log(tb.e_max), tb.n_energy)
     T = 15.0
     expect = np.zeros(nz)
@@ -77,17 +78,18 @@ def test_depth_profile_in_slabs_follows_the_csda_equation(slab_tables_csda):
         f = lambda z, t: [-d * np.interp(np.log(max(t[0], tb.e_min)), lnE, tb.electron[m, 0].astype(np.float64))]
         sol = integrate.solve_ivp(f, (0.0, h), [T], rtol=1e-10, atol=1e-12)
         T1 = float(sol.y[0, -1])
-        if T1 < tb.e_cut:
+        if T1 < tb.e_cut + 0.6:      # stop the comparison before the last steps (R8 puts the rest in one voxel)
             break
         expect[j] = T - T1
         T = T1
-    got = r.edep[:, 0, 0]
+    got = r.edep[:, 0, 0] / n
     live = expect > 0
     assert live.sum() > 25
-    assert np.allclose(got[live], expect[live], rtol=6e-3)                      # per voxel
-    assert got[live].sum() == pytest.approx(expect[live].sum(), rel=1e-3)       # no drift
-    # the medium boundaries show: bone voxels take 1.85 x ~0.95 the loss of water voxels, lung 0.26 x
-    assert got[7] / got[3] == pytest.approx(1.85 * tb.electron[1, 0, -40] / tb.electron[0, 0, -40], rel=0.03)
+    assert np.allclose(got[live], expect[live], rtol=0.03)                      # per voxel: ~1 % noise
+    assert got[live].sum() == pytest.approx(expect[live].sum(), rel=3e-3)       # no drift, no lost share
+    # the Eq. 4 transport puts exactly this in every voxel for every history; the medium boundaries show
+    assert np.allclose(r4.edep[:, 0, 0][live], expect[live], rtol=6e-3)
+    assert got[7] / got[3] == pytest.approx(r4.edep[7, 0, 0] / r4.edep[3, 0, 0], rel=0.03)
 
 
 def test_dose_agrees_with_eq4_transport_where_the_medium_is_uniform():
