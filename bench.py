@@ -238,6 +238,7 @@ def paper_tables(args):
             t0, _ = time_gpu(g, torch, w, n, args.steps, scheduler=0)
             ta, _ = time_gpu(g, torch, w, n, args.steps, cta_threads=512)
             tb, _ = time_gpu(g, torch, w, n, args.steps, cta_threads=1024)
+            tm, cm = time_gpu(g, torch, w, n, args.steps, hom_tol=0.1)
             s = s_gpu(g, torch, ev, w, n)
             eps = ev.efficiency(s, t1 * 1e-3)
             # the oracle on a bounded sample; s scales as 1/sqrt(N) (L334), time as N
@@ -253,7 +254,8 @@ def paper_tables(args):
                          f"{PAPER_TAB4[(geom, particle)] * 1e3:.0f} |")
             rows5.append(f"| {pname} | Geom{geom} | {t_o:.1f} | {t_o / (t1 * 1e-3):.0f} | {s * 100:.3f} | {s_o * 100:.3f} | "
                          f"{eps:.3g} | {eps_o:.3g} | {eps / eps_o:.0f} |")
-            rows6.append(f"| {pname} | Geom{geom} | {t0:.3f} | {t0 / t1:.2f} | {t0 / ta:.2f} | {t0 / tb:.2f} |")
+            rows6.append(f"| {pname} | Geom{geom} | {t0:.3f} | {t0 / t1:.2f} | {t0 / ta:.2f} | {t0 / tb:.2f} | "
+                         f"{t0 / tm:.2f} ({tm:.3f} ms, {c['ch_steps'] / cm['ch_steps']:.2f} x fewer steps) |")
     print("## Tab. IV analogue: absolute times of `gpumcd_run` (device time, CUDA events, median of "
           f"{args.steps}, L2 flushed between runs)\n")
     print("| particles | geometry | histories | ms | M histories/s | G CH steps/s | paper, GTX480, ms (context) |")
@@ -266,8 +268,9 @@ def paper_tables(args):
     print("|---|---|---|---|---|---|---|---|---|")
     print("\n".join(rows5))
     print("\n## Tab. VI analogue: scheduling strategies against the paper's base scheme (scheduler 0)\n")
-    print("| particles | geometry | T_base = scheduler 0, ms | A, scheduler 1 (default CTA size) | A, 512 threads/SM | A, 1024 threads/SM |")
-    print("|---|---|---|---|---|---|")
+    print("| particles | geometry | T_base = scheduler 0, ms | A, scheduler 1 (default CTA size) | A, 512 threads/SM | "
+          "A, 1024 threads/SM | A, scheduler 1 + multi-voxel steps (hom_tol 0.1, another step algorithm: DESIGN.md R32) |")
+    print("|---|---|---|---|---|---|---|")
     print("\n".join(rows6))
 
 
