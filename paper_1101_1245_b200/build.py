@@ -32,6 +32,13 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if force or needs_build():
         cmd = [NVCC, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
                "-shared", "-Xcompiler", "-fPIC", "-I", INCLUDE, "-o", LIB] + sources()
+        # Math policy: single-precision device code is built with --use_fast_math (SFU forms of
+        # division, sqrt, exp, log, sincos; the kernels are issue-bound and 10 % faster for it, parity bars
+        # unchanged).  GPUMCD_IEEE=1 builds the IEEE variant (library forms everywhere).
+        if os.environ.get("GPUMCD_IEEE", "0") == "1":
+            cmd.insert(1, "-DGPUMCD_FAST_MATH=0")
+        else:
+            cmd.insert(1, "--use_fast_math")
         if verbose:
             cmd.insert(1, "-Xptxas=-v")
         extra = os.environ.get("GPUMCD_NVCC_FLAGS", "")      # experiments only, e.g. -DGPUMCD_PTHREADS=768
