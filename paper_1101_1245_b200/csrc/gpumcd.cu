@@ -703,7 +703,22 @@ static int run_persistent(gpumcd_ctx *ctx, uint64_t h_begin, uint64_t n_hist, ui
         // flights end in a fictitious interaction and wait for the phantom fetch), else 512
         int threads = static_cast<int>(ctx->opt.cta_threads);
         if (threads == 0) threads = (ctx->src.particle == 1 || ctx->rho_mean_over_max >= 0.8) ? 512 : 1024;
-        a.high = threads == 512 ? 256u : 512u;
+        // banked particles of the other type that make a warp change to it: photons are cheap to work off
+        // (few per batch keeps the drain short), electrons are worth a fuller batch
+#ifndef GPUMCD_HG512
+#define GPUMCD_HG512 96u
+#endif
+#ifndef GPUMCD_HE512
+#define GPUMCD_HE512 160u
+#endif
+#ifndef GPUMCD_HG1024
+#define GPUMCD_HG1024 512u
+#endif
+#ifndef GPUMCD_HE1024
+#define GPUMCD_HE1024 512u
+#endif
+        a.high_g = threads == 512 ? GPUMCD_HG512 : GPUMCD_HG1024;
+        a.high_e = threads == 512 ? GPUMCD_HE512 : GPUMCD_HE1024;
         void *args[] = {&a};
         // the kernel variant: trace (photon-only replay) x tables in shared memory x CTA size x multi-voxel steps
         const bool multi = ctx->opt.hom_tol > 0.f && !trace; // a trace run tracks no electrons

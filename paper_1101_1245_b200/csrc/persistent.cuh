@@ -132,7 +132,7 @@ struct PersistArgs {
     float4 *stkB;
     uint4 *stkC;
     unsigned cap_r;                // capacity of a ready stack (ES, GS)
-    unsigned high;                 // other-type records that make a warp change type
+    unsigned high_g, high_e;       // banked photons / electrons that make a warp change to that type
     unsigned stride;               // 2 cap_r + 2 kPend
     unsigned long long hist0;      // first history of the launch (low word never wraps inside a launch)
     unsigned n_hist;               // histories of the launch (< 2^32)
@@ -177,7 +177,7 @@ struct Warp {
     float4 *B;
     uint4 *C;
     unsigned cap_r;
-    unsigned high;
+    unsigned high_g, high_e;
     unsigned n[4];
     unsigned lt;   // lanes below this one
     unsigned hw;   // fullest ready stack seen
@@ -284,7 +284,7 @@ __device__ __forceinline__ int electron_mode(const PersistArgs &a, const float *
         const unsigned E = ready + w.n[SK_EH], G = w.n[SK_GS] + w.n[SK_GI];
         const unsigned must = w.cap_r - kMustMargin;
         const bool src_g = !src_is_e && !cl.empty();
-        bool leave = G >= w.high && (E < w.high || (G >= must && E < must));
+        bool leave = G >= w.high_g && (E < w.high_e || (G >= must && E < must));
         if (!src_e) {
             if (ready == 0u) return (G != 0u || src_g) ? 0 : -1; // (EH is empty here)
             leave = leave || (ready < kLow && (src_g || w.n[SK_GS] >= 32u));
@@ -378,7 +378,7 @@ __device__ __forceinline__ int photon_mode(const PersistArgs &a, const float *__
         const unsigned G = ready + w.n[SK_GI], E = w.n[SK_ES] + w.n[SK_EH];
         const unsigned must = w.cap_r - kMustMargin;
         const bool src_e = !src_is_g && !cl.empty();
-        bool leave = E >= w.high && (G < w.high || E >= must);
+        bool leave = E >= w.high_e && (G < w.high_g || E >= must);
         if (!src_g) {
             if (ready == 0u) return (E != 0u || src_e) ? 1 : -1; // (GI is empty here)
             leave = leave || (ready < kLow && (src_e || w.n[SK_ES] >= 32u));
@@ -433,7 +433,8 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(const __grid_consta
     w.B = a.stkB + gwarp * a.stride;
     w.C = a.stkC + gwarp * a.stride;
     w.cap_r = a.cap_r;
-    w.high = a.high;
+    w.high_g = a.high_g;
+    w.high_e = a.high_e;
     w.n[0] = w.n[1] = w.n[2] = w.n[3] = 0u;
     w.lt = (1u << lane) - 1u;
     w.hw = 0u;
