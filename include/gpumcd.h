@@ -86,8 +86,9 @@ typedef struct {
                               0: the paper's scheme (L166): one launch per pass, one thread per
                               particle, the host reads the queue counts between passes            */
     uint32_t warp_stack;   /* scheduler 1: capacity of a warp's electron stack and of its photon
-                              stack, records; default 1024 (smaller values only make sense in
-                              tests of the overflow report; at least 192)                          */
+                              stack, records; default 1024, at least 192 (a warp changes particle
+                              type before a stack fills up, so small stacks cost speed, not
+                              correctness)                                                         */
     uint32_t cta_threads;  /* scheduler 1: threads of the persistent kernel's one CTA per SM, 512 or
                               1024; 0 (default) chooses 1024 for a photon source in a phantom whose
                               mean density is below 0.8 of the largest (most flights end in a

@@ -219,20 +219,30 @@ struct Warp {
         n[s] -= take;
         return got;
     }
-    // Converged code: the lanes with `want` take the next primaries of the source (H0).
-    __device__ __forceinline__ bool primaries(const PersistArgs &a, Claim &cl, bool want, Particle &p)
+    // Converged code: the whole warp makes this warp's next (up to 32) primaries at once and banks them on
+    // ready stack s (SK_ES for an electron source, SK_GS for photons), from where free lanes pop them like
+    // any other ready particle: the source code (H0) then always runs with full lanes.  Returns false if the
+    // source is dry or the stack has no room for them right now.
+    __device__ __forceinline__ bool bank_primaries(const PersistArgs &a, Claim &cl, int s)
     {
         cl.refill(a.head, a.n_hist);
-        const unsigned m = __ballot_sync(kFull, want);
-        const unsigned take = min(static_cast<unsigned>(__popc(m)), cl.end - cl.next);
-        const unsigned rank = __popc(m & lt);
-        const bool got = want && rank < take;
-        if (got) {
-            p = make_primary(a.P, a.S, a.hist0 + (cl.next + rank));
-            *e_inc += static_cast<double>(p.E);
+        const unsigned k = cl.end - cl.next;
+        if (k == 0u || n[s] + k > cap_r) return false;
+        const unsigned lane = threadIdx.x & 31;
+        bool on = lane < k;
+        Particle q;
+        if (on) {
+            q = make_primary(a.P, a.S, a.hist0 + (cl.next + lane));
+            *e_inc += static_cast<double>(q.E);
+            if (s == SK_ES && !electron_tracked(a.P, q.E)) { // below the cutoff (or photon_only): deposited where it is born
+                deposit(a.P, voxel_index(a.P.geo, q), q.E);
+                Acc(a.P).cut(q.E);
+                on = false;
+            }
         }
-        cl.next += take;
-        return got;
+        push(a.P, s, on, q, 0u);
+        cl.next += k;
+        return true;
     }
 };
 
@@ -298,16 +308,8 @@ __device__ __forceinline__ int electron_mode(const PersistArgs &a, const float *
         if (~live) {
             uint32_t extra;
             bool got = w.pop(SK_ES, !alive, p, extra);
-            if (src_e && __any_sync(kFull, !alive && !got)) {
-                if (w.primaries(a, cl, !alive && !got, p)) {
-                    if (electron_tracked(P, p.E)) {
-                        got = true;
-                    } else { // below the cutoff (or photon_only): deposited where it is born
-                        deposit(P, voxel_index(P.geo, p), p.E);
-                        Acc(P).cut(p.E);
-                    }
-                }
-            }
+            if (src_e && __any_sync(kFull, !alive && !got) && w.bank_primaries(a, cl, SK_ES))
+                got = w.pop(SK_ES, !alive && !got, p, extra) || got;
             if (got) {
                 lnT = flog(p.E);
                 alive = true;
@@ -392,7 +394,8 @@ __device__ __forceinline__ int photon_mode(const PersistArgs &a, const float *__
         if (~live) {
             uint32_t extra;
             bool got = w.pop(SK_GS, !alive, p, extra);
-            if (src_g && __any_sync(kFull, !alive && !got)) got = w.primaries(a, cl, !alive && !got, p) || got;
+            if (src_g && __any_sync(kFull, !alive && !got) && w.bank_primaries(a, cl, SK_GS))
+                got = w.pop(SK_GS, !alive && !got, p, extra) || got;
             if (got) alive = true;
         }
         const unsigned fl = __ballot_sync(kFull, alive);
