@@ -89,10 +89,10 @@ typedef struct {
                               stack, records; default 1024, at least 192 (a warp changes particle
                               type before a stack fills up, so small stacks cost speed, not
                               correctness)                                                         */
-    uint32_t cta_threads;  /* scheduler 1: threads of the persistent kernel's one CTA per SM, 512 or
-                              1024; 0 (default) chooses 1024 for a photon source in a phantom whose
-                              mean density is below 0.8 of the largest (most flights end in a
-                              fictitious interaction and wait on memory) and 512 otherwise          */
+    uint32_t cta_threads;  /* scheduler 1: threads of the persistent kernel's one CTA per SM: 0 or 512
+                              (default; 128 registers per thread, short drain phase) or 1024 (64
+                              registers, twice the warps; slower on every workload measured, kept
+                              for the ablation)                                                    */
     float hom_tol;         /* 0 (default): electron steps end at every voxel boundary, Eq. 4 as printed.
                               > 0: multi-voxel steps (the paper's "improvements to the electron-step
                               algorithm", L364-368, are future work there; R32): d_vox of

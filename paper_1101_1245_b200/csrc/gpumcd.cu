@@ -22,12 +22,11 @@ constexpr int kBlock = 256;
 // (H10; positive floats order like their bit patterns, so atomicMax on the bits is a float max).
 __global__ void k_pack_phantom(const float *__restrict__ density, const uint8_t *__restrict__ material,
                                size_t nvox, int n_mat, float2 *__restrict__ out, unsigned *rho_max_bits,
-                               unsigned *n_bad, double *rho_sum)
+                               unsigned *n_bad)
 {
     __shared__ unsigned s_max[8];
     if (threadIdx.x < 8) s_max[threadIdx.x] = 0u;
     __syncthreads();
-    double sum = 0.0;
     for (size_t i = blockIdx.x * static_cast<size_t>(blockDim.x) + threadIdx.x; i < nvox;
          i += static_cast<size_t>(gridDim.x) * blockDim.x) {
         const float d = density[i];
@@ -38,11 +37,8 @@ __global__ void k_pack_phantom(const float *__restrict__ density, const uint8_t 
         } else {
             atomicMax(&s_max[m], __float_as_uint(d));
             out[i] = make_float2(d, __int_as_float(m));
-            sum += static_cast<double>(d);
         }
     }
-    sum = wsum(sum);
-    if ((threadIdx.x & 31) == 0 && sum != 0.0) atomicAdd(rho_sum, sum);
     __syncthreads();
     if (threadIdx.x < 8 && s_max[threadIdx.x]) atomicMax(&rho_max_bits[threadIdx.x], s_max[threadIdx.x]);
 }
@@ -205,8 +201,7 @@ struct gpumcd_ctx {
     float2 *phantom = nullptr;
     float *stage_density = nullptr;   // device staging of host volumes (gpumcd_create_host / set_phantom_host)
     uint8_t *stage_material = nullptr;
-    unsigned *scratch = nullptr;      // 8 rho_max bit patterns + 1 bad-voxel count + (at word 10) the fp64 sum of the densities
-    double rho_mean_over_max = 1.0;   // homogeneity of the phantom: mean density / largest density
+    unsigned *scratch = nullptr;      // 8 rho_max bit patterns + 1 bad-voxel count
     float *dose_stage = nullptr;      // device dose of gpumcd_run_host
     float *table_blob = nullptr;
     std::vector<float> blob_host;     // host copy of the table blob (majorants are rebuilt per phantom)
@@ -350,8 +345,7 @@ static int load_phantom(gpumcd_ctx *ctx, const float *density, const uint8_t *ma
     }
     CK(cudaMemsetAsync(ctx->scratch, 0, 12 * sizeof(unsigned), nullptr));
     const int grid = static_cast<int>(std::min<size_t>((nvox + kBlock - 1) / kBlock, 148 * 8));
-    k_pack_phantom<<<grid, kBlock>>>(d_density, d_material, nvox, ctx->n_mat, ctx->phantom, ctx->scratch, ctx->scratch + 8,
-                                   reinterpret_cast<double *>(ctx->scratch + 10));
+    k_pack_phantom<<<grid, kBlock>>>(d_density, d_material, nvox, ctx->n_mat, ctx->phantom, ctx->scratch, ctx->scratch + 8);
     CK(cudaGetLastError());
     if (ctx->opt.hom_tol > 0.f) {
         const int r_max = std::min(7, static_cast<int>(std::ceil(ctx->opt.es_max_cm / ctx->h)) + 1);
@@ -366,12 +360,6 @@ static int load_phantom(gpumcd_ctx *ctx, const float *density, const uint8_t *ma
     }
     double rho_max[8];
     for (int m = 0; m < 8; ++m) { float f; memcpy(&f, &h_scratch[m], 4); rho_max[m] = f; }
-    {
-        double sum;
-        memcpy(&sum, &h_scratch[10], 8);
-        const double top = *std::max_element(rho_max, rho_max + 8);
-        ctx->rho_mean_over_max = top > 0.0 ? sum / static_cast<double>(nvox) / top : 1.0;
-    }
     const int nE = ctx->n_E, nM = ctx->n_mat;
     const float *ph = ctx->blob_host.data(), *el = ph + ctx->tab.off_el;
     float *mu_max = ctx->blob_host.data() + ctx->tab.off_mu, *m_e = ctx->blob_host.data() + ctx->tab.off_me;
@@ -699,10 +687,8 @@ static int run_persistent(gpumcd_ctx *ctx, uint64_t h_begin, uint64_t n_hist, ui
         a.dose = dose_dev;
         a.nvox = ctx->nvox;
         a.finalize = (h0 + n == h_end) ? 1 : 0;
-        // CTA size (see persistent.cuh): 1024 threads for a photon beam in a heterogeneous phantom (most
-        // flights end in a fictitious interaction and wait for the phantom fetch), else 512
-        int threads = static_cast<int>(ctx->opt.cta_threads);
-        if (threads == 0) threads = (ctx->src.particle == 1 || ctx->rho_mean_over_max >= 0.8) ? 512 : 1024;
+        // CTA size (see persistent.cuh): 512 threads unless the caller asks for 1024
+        const int threads = ctx->opt.cta_threads == 1024 ? 1024 : 512;
         // banked particles of the other type that make a warp change to it: photons are cheap to work off
         // (few per batch keeps the drain short), electrons are worth a fuller batch
 #ifndef GPUMCD_HG512

@@ -32,10 +32,10 @@ namespace cg = cooperative_groups;
 #ifndef GPUMCD_LOW
 #define GPUMCD_LOW 24
 #endif
-// Threads per persistent CTA (one CTA per SM): the kernel is built for 512 (128 registers per
-// thread, no spills, short drain phase: best where flights and steps rarely wait for memory) and
-// for 1024 (64 registers, twice the warps to hide the L2 latency of the phantom fetch: best for
-// photon beams in heterogeneous phantoms, where most flights end in a fictitious interaction).
+// Threads per persistent CTA (one CTA per SM): 512 by default (128 registers per thread, no spills; the
+// per-lane backlog when the source runs dry is half that of 1024 threads).  The 1024-thread build (64
+// registers, spills, twice the warps to hide latency) is kept as an option for the ablation: it was the
+// faster one for photon beams in heterogeneous phantoms until the fast-math build shrank the code.
 constexpr int kPThreadsMax = 1024;
 constexpr unsigned kFull = 0xffffffffu;
 constexpr unsigned kChunk = 32;            // primaries a warp claims per atomic on the source head

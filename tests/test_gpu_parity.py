@@ -151,8 +151,8 @@ def test_schedulers_agree_exactly(workloads):
 
 
 def test_cta_size_does_not_change_the_result(workloads):
-    """Scheduler 1 runs with 512 or 1024 threads per SM (chosen from the phantom's homogeneity unless
-    cta_threads says otherwise): which lane works a particle off does not matter."""
+    """Scheduler 1 runs with 512 (default) or 1024 threads per SM: which lane works a particle off does not
+    matter."""
     for cfg in (2, 4):
         w = workloads[cfg]
         a = run_gpu(w, 60_000, scheduler=1, cta_threads=512)
