@@ -409,6 +409,19 @@ def main():
                 "kernel_share_of_step": ms_e / t_ms if t_ms else None,
                 "alg_inst_per_ch_step": ALG_INST_PER_CH_STEP}
 
+    # ---- secondary rooflines (BASELINE.json north_star): the tally against the measured fp64 atomic rate of the
+    # L2 (gpumcd_probe_tally: the same grid, the field's footprint, nothing but atomic adds), and the DRAM traffic
+    # of the ncu capture against the measured HBM copy bandwidth
+    tally_peak = g.gpumcd_probe_tally(ctx, 200_000_000)
+    tally_rate = local_ch / t_s
+    tally = {"bound": "l2_atomic", "achieved": tally_rate, "peak": tally_peak, "unit": "fp64 atomic adds/s",
+             "frac": tally_rate / tally_peak, "what": "one add per condensed-history step against gpumcd_probe_tally"}
+    hbm = None
+    if roofline["traffic"] and ms_e > 0:
+        gbs = roofline["traffic"] / (ms_e / max(n_e, 1) * 1e-3) / 1e9
+        hbm = {"bound": "hbm", "achieved": gbs, "peak": peaks.get("hbm_gbs"), "unit": "GB/s",
+               "frac": gbs / peaks.get("hbm_gbs"), "what": f"ncu DRAM bytes per launch / kernel time ({peak_kind} copy bandwidth)"}
+
     # ---- end to end through the host entry points: every step copies that step's inputs (the phantom volumes,
     # from pinned host memory) to the device and the resulting dose grid back to the host
     e2e = None
@@ -462,8 +475,8 @@ def main():
             "config": {"workload": w.name, "histories_per_step_per_gpu": n, "scheduler": int(opt.scheduler), "hom_tol": float(opt.hom_tol),
                        "wave_size": int(opt.wave_size), "l2": "flushed between timed steps (512 MiB write)",
                        "tally": "fp64 atomics", "parallelism": f"histories x{world}"},
-            "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu,
-            "wall_s_timed_region": wall,
+            "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "roofline_tally": tally,
+            "roofline_hbm": hbm, "cpu_baseline": cpu, "wall_s_timed_region": wall,
         }
         print(json.dumps(line))
     if dist:

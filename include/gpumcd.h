@@ -213,6 +213,14 @@ typedef struct {
 int gpumcd_set_profiling(gpumcd_ctx *ctx, int enable);
 int gpumcd_get_profile(gpumcd_ctx *ctx, gpumcd_profile *host_out); /* waits for the run's stream */
 
+/* Tally probe: the rate (updates per second, returned in *updates_per_second, a HOST double) at which
+ * this device adds fp64 values into THIS context's energy grid when it does nothing else: about n_updates
+ * atomic adds at pseudo-random voxels under the current source's field (all depths), the address pattern
+ * of the condensed-history deposits (H4/H8).  It is the measured denominator of the tally's roofline
+ * (no vendor figure exists for the L2's fp64 atomic rate).  Synchronous on cuda_stream; the energy tally
+ * of the last run is overwritten (zeroed afterwards); needs a source. */
+int gpumcd_probe_tally(gpumcd_ctx *ctx, uint64_t n_updates, double *updates_per_second, void *cuda_stream);
+
 /* Library-owned, NUL-terminated description of the last error on this context (or of the last
  * failed create when ctx == NULL); valid until the next call on the same context. */
 const char *gpumcd_last_error(gpumcd_ctx *ctx);

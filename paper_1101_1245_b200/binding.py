@@ -26,7 +26,7 @@ GPUMCD_ERR_TABLE_RANGE = -6
 EXPORTS = ("gpumcd_default_options", "gpumcd_create", "gpumcd_create_host", "gpumcd_set_phantom",
            "gpumcd_set_phantom_host", "gpumcd_set_source", "gpumcd_run",
            "gpumcd_run_host", "gpumcd_run_uncertainty", "gpumcd_run_trace", "gpumcd_get_counters", "gpumcd_get_energy_tally",
-           "gpumcd_set_history_offset", "gpumcd_set_profiling", "gpumcd_get_profile",
+           "gpumcd_set_history_offset", "gpumcd_set_profiling", "gpumcd_get_profile", "gpumcd_probe_tally",
            "gpumcd_last_error", "gpumcd_destroy")
 
 
@@ -103,6 +103,7 @@ def load_library():
         lib.gpumcd_set_history_offset.argtypes = [vp, C.c_uint64]
         lib.gpumcd_set_profiling.argtypes = [vp, C.c_int]
         lib.gpumcd_get_profile.argtypes = [vp, C.POINTER(gpumcd_profile)]
+        lib.gpumcd_probe_tally.argtypes = [vp, C.c_uint64, C.POINTER(C.c_double), vp]
         lib.gpumcd_last_error.argtypes = [vp]
         lib.gpumcd_last_error.restype = C.c_char_p
         lib.gpumcd_destroy.argtypes = [vp]
@@ -291,6 +292,13 @@ def gpumcd_get_profile(ctx: Context) -> dict:
     p = gpumcd_profile()
     ctx._check(load_library().gpumcd_get_profile(ctx._h, C.byref(p)))
     return p.as_dict()
+
+
+def gpumcd_probe_tally(ctx: Context, n_updates: int, stream=None) -> float:
+    """fp64 atomic adds per second into the context's energy grid under the source's field (include/gpumcd.h)."""
+    r = C.c_double(0.0)
+    ctx._check(load_library().gpumcd_probe_tally(ctx._h, int(n_updates), C.byref(r), _stream_ptr(stream)))
+    return r.value
 
 
 def gpumcd_last_error(ctx: Optional[Context]) -> str:

@@ -182,6 +182,27 @@ __global__ void k_finalize_uncertainty(const double *__restrict__ s1, const doub
     }
 }
 
+// Tally probe (the denominator of the tally's roofline, since no vendor figure exists for
+// the fp64 atomic rate of the L2): every thread adds `per_thread` values into the context's own energy grid
+// at pseudo-random voxels of the beam-shaped region x in [x0, x0+wx), y in [y0, y0+wy), all depths, the
+// address pattern of the condensed-history deposits, and nothing else.
+__global__ void k_tally_probe(double *__restrict__ edep, int nx, int ny, int nz, int x0, int y0, int wx, int wy,
+                              unsigned per_thread, unsigned seed)
+{
+    const unsigned tid = blockIdx.x * blockDim.x + threadIdx.x;
+    uint4 r = philox4x32_10(tid, 0u, 0u, 0u, seed, 0x5eedu);
+    for (unsigned k = 0; k < per_thread; ++k) {
+        // a cheap generator inside the loop (the probe must be bound by the atomics, not by Philox)
+        r.x = r.x * 1664525u + 1013904223u;
+        r.y = r.y * 22695477u + 1u;
+        r.z = r.z * 1103515245u + 12345u;
+        const unsigned ix = x0 + __umulhi(r.x, static_cast<unsigned>(wx));
+        const unsigned iy = y0 + __umulhi(r.y, static_cast<unsigned>(wy));
+        const unsigned iz = __umulhi(r.z, static_cast<unsigned>(nz));
+        atomicAdd(&edep[ix + static_cast<size_t>(nx) * (iy + static_cast<size_t>(ny) * iz)], 1.0);
+    }
+}
+
 } // namespace gpumcd
 
 // =============================================================================================
@@ -896,6 +917,42 @@ extern "C" int gpumcd_get_profile(gpumcd_ctx *ctx, gpumcd_profile *out)
         (&p.ms_source)[e.cls] += ms;
     }
     *out = p;
+    return GPUMCD_OK;
+}
+
+extern "C" int gpumcd_probe_tally(gpumcd_ctx *ctx, uint64_t n_updates, double *updates_per_second, void *cuda_stream)
+{
+    if (!ctx || !updates_per_second || n_updates == 0) return GPUMCD_ERR_INVALID_ARG;
+    if (!ctx->have_source) { set_error(ctx, "gpumcd_probe_tally called before gpumcd_set_source"); return GPUMCD_ERR_NO_SOURCE; }
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    // the field's footprint on the grid (a pencil beam: a 3 x 3 voxel column)
+    const double h = ctx->h;
+    int x0 = static_cast<int>(std::floor((ctx->src.cx - 0.5 * ctx->src.wx) / h)) - (ctx->src.shape == 0 ? 1 : 0);
+    int y0 = static_cast<int>(std::floor((ctx->src.cy - 0.5 * ctx->src.wy) / h)) - (ctx->src.shape == 0 ? 1 : 0);
+    int x1 = static_cast<int>(std::floor((ctx->src.cx + 0.5 * ctx->src.wx) / h)) + (ctx->src.shape == 0 ? 1 : 0);
+    int y1 = static_cast<int>(std::floor((ctx->src.cy + 0.5 * ctx->src.wy) / h)) + (ctx->src.shape == 0 ? 1 : 0);
+    x0 = std::max(x0, 0); y0 = std::max(y0, 0);
+    x1 = std::min(x1, ctx->nx - 1); y1 = std::min(y1, ctx->ny - 1);
+    const int threads = 512, blocks = 148 * 2;
+    const uint64_t per_thread = (n_updates + static_cast<uint64_t>(threads) * blocks - 1) / (static_cast<uint64_t>(threads) * blocks);
+    if (per_thread > 0xffffffffull) { set_error(ctx, "n_updates too large"); return GPUMCD_ERR_INVALID_ARG; }
+    cudaEvent_t a, b;
+    CK(cudaEventCreate(&a)); CK(cudaEventCreate(&b));
+    CK(cudaMemsetAsync(ctx->edep, 0, ctx->nvox * sizeof(double), st));
+    // once untimed (first touch of the grid), once timed
+    k_tally_probe<<<blocks, threads, 0, st>>>(ctx->edep, ctx->nx, ctx->ny, ctx->nz, x0, y0, x1 - x0 + 1, y1 - y0 + 1,
+                                              static_cast<unsigned>(per_thread), 1u);
+    CK(cudaEventRecord(a, st));
+    k_tally_probe<<<blocks, threads, 0, st>>>(ctx->edep, ctx->nx, ctx->ny, ctx->nz, x0, y0, x1 - x0 + 1, y1 - y0 + 1,
+                                              static_cast<unsigned>(per_thread), 2u);
+    CK(cudaEventRecord(b, st));
+    CK(cudaGetLastError());
+    CK(cudaEventSynchronize(b));
+    float ms = 0.f;
+    CK(cudaEventElapsedTime(&ms, a, b));
+    cudaEventDestroy(a); cudaEventDestroy(b);
+    CK(cudaMemsetAsync(ctx->edep, 0, ctx->nvox * sizeof(double), st)); // the tally of the last run is gone
+    *updates_per_second = static_cast<double>(per_thread) * threads * blocks / (static_cast<double>(ms) * 1e-3);
     return GPUMCD_OK;
 }
 

@@ -333,3 +333,27 @@ def test_error_paths(workloads):
     assert small["counters"]["overflow_count"] == 0 and small["counters"]["bank_high_water"] <= 192
     for k in INT_KEYS:
         assert small["counters"][k] == ref["counters"][k], k
+
+
+def test_tally_probe(workloads):
+    """gpumcd_probe_tally: a plausible fp64 atomic rate, and the context still works afterwards."""
+    import torch
+
+    import paper_1101_1245_b200 as g
+    w = workloads[1]
+    dev = torch.device("cuda:0")
+    rho = torch.from_numpy(w.density).to(dev)
+    mat = torch.from_numpy(w.material).to(dev)
+    dose = torch.empty(rho.shape, dtype=torch.float32, device=dev)
+    with g.gpumcd_create(rho, mat, w.voxel_cm, w.tables) as ctx:
+        with pytest.raises(g.GpumcdError):
+            g.gpumcd_probe_tally(ctx, 1000)                 # no source yet
+        g.gpumcd_set_source(ctx, w.source)
+        g.gpumcd_run(ctx, 20_000, 1, dose)
+        before = g.gpumcd_get_counters(ctx)
+        rate = g.gpumcd_probe_tally(ctx, 20_000_000)
+        assert 1e9 < rate < 1e13
+        g.gpumcd_run(ctx, 20_000, 1, dose)
+        after = g.gpumcd_get_counters(ctx)
+        assert after["ch_steps"] == before["ch_steps"]
+        assert after["e_dep_continuous"] == pytest.approx(before["e_dep_continuous"], rel=1e-12)
