@@ -94,3 +94,28 @@ def test_multi_voxel_dose_is_the_dose_of_the_eq4_transport(cfg, n):
     ca, cb = a["edep"][col].sum(axis=(1, 2)), b["edep"][col].sum(axis=(1, 2))
     assert np.abs(ca - cb).max() <= 0.015 * ca.max()
     assert total(b["counters"]) == pytest.approx(total(a["counters"]), rel=2e-3)
+
+
+def test_set_phantom_rebuilds_the_uniform_radius_field():
+    """The look-ahead shortcut (uniform radius per voxel) belongs to the phantom: a context re-targeted at
+    another phantom must give what a fresh context gives, event for event."""
+    import torch
+
+    import paper_1101_1245_b200 as g
+    w = make_paper_geometry(3, ELECTRON)
+    n = 40_000
+    ref = run_gpu(w, n, hom_tol=TOL)
+    water = np.ones_like(w.density)
+    zeros = np.zeros_like(w.material)
+    dose = np.empty(w.density.shape, np.float32)
+    with g.gpumcd_create_host(water, zeros, w.voxel_cm, w.tables, g.gpumcd_default_options(hom_tol=TOL)) as ctx:
+        g.gpumcd_set_source(ctx, w.source)
+        g.gpumcd_run_host(ctx, n, w.seed, dose)              # uniform water: every voxel has the largest radius
+        c_water = g.gpumcd_get_counters(ctx)
+        g.gpumcd_set_phantom_host(ctx, w.density, w.material)
+        g.gpumcd_run_host(ctx, n, w.seed, dose)
+        c = g.gpumcd_get_counters(ctx)
+    for k in INT_KEYS:
+        assert c[k] == ref["counters"][k], k
+    np.testing.assert_allclose(dose, ref["dose"], rtol=1e-6, atol=0)
+    assert c_water["ch_steps"] != c["ch_steps"]
