@@ -509,7 +509,7 @@ static int create_impl(gpumcd_ctx **out, const float *density, const uint8_t *ma
         if (per_sm < 1) { set_error(ctx, "persistent kernel does not fit on an SM"); return GPUMCD_ERR_CUDA; }
         ctx->p_grid = n_sm; // one CTA per SM
         ctx->cap_r = std::max(opt.warp_stack, kMustMargin + 32u);
-        ctx->stride = 2 * ctx->cap_r + 2 * kPend;
+        ctx->stride = 2 * ctx->cap_r + 3 * kPend;
         const size_t n_warps = static_cast<size_t>(ctx->p_grid) * (kPThreadsMax / 32);
         const size_t recs = n_warps * ctx->stride;
         CK(cudaMalloc(&ctx->stkA, recs * sizeof(float4)));

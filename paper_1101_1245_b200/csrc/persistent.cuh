@@ -39,7 +39,7 @@ namespace cg = cooperative_groups;
 constexpr int kPThreadsMax = 1024;
 constexpr unsigned kFull = 0xffffffffu;
 constexpr unsigned kChunk = 32;            // primaries a warp claims per atomic on the source head
-constexpr unsigned kPend = 64;             // capacity of a waiting stack (EH, GI): < 32 before a move, + 32 after
+constexpr unsigned kPend = 64;             // capacity of a waiting stack (EH, GI, GR): < 32 before a move, + 32 after
 constexpr unsigned kLow = GPUMCD_LOW;      // own-type particles below which a warp with no source changes type
 constexpr unsigned kMustMargin = 160;      // a ready stack within this many records of its capacity forces the change
 
@@ -128,12 +128,12 @@ struct PersistArgs {
     Params P;
     SourceDev S;
     unsigned *head;    // next primary of this launch to be claimed (the only counter the warps share)
-    float4 *stkA;      // per-warp stacks, `stride` records per warp: [ES cap_r | GS cap_r | EH kPend | GI kPend]
+    float4 *stkA;      // per-warp stacks, `stride` records per warp: [ES cap_r | GS cap_r | EH kPend | GI kPend | GR kPend]
     float4 *stkB;
     uint4 *stkC;
     unsigned cap_r;                // capacity of a ready stack (ES, GS)
     unsigned high_g, high_e;       // banked photons / electrons that make a warp change to that type
-    unsigned stride;               // 2 cap_r + 2 kPend
+    unsigned stride;               // 2 cap_r + 3 kPend
     unsigned long long hist0;      // first history of the launch (low word never wraps inside a launch)
     unsigned n_hist;               // histories of the launch (< 2^32)
     unsigned table_floats;         // length of the table blob, padded to a multiple of 4 floats
@@ -147,7 +147,7 @@ struct PersistArgs {
 // DevCounters lists its first eleven members in this order.
 enum : int { WC_FLIGHT = 0, WC_COMPTON, WC_PHOTO, WC_PAIR, WC_FICT, WC_STEP, WC_MOLLER, WC_BREMS, WC_HFICT,
              WC_PUSH_E, WC_PUSH_G, WC_N };
-enum : int { SK_ES = 0, SK_GS = 1, SK_EH = 2, SK_GI = 3 };
+enum : int { SK_ES = 0, SK_GS = 1, SK_EH = 2, SK_GI = 3, SK_GR = 4 };
 
 struct WarpCtl {          // one per warp, shared memory
     unsigned n_es, n_gs;  // stack counts while divergent code pushes (photon_interact); else in registers
@@ -178,7 +178,7 @@ struct Warp {
     uint4 *C;
     unsigned cap_r;
     unsigned high_g, high_e;
-    unsigned n[4];
+    unsigned n[5];
     unsigned lt;   // lanes below this one
     unsigned hw;   // fullest ready stack seen
     WarpCtl *ctl;
@@ -186,7 +186,7 @@ struct Warp {
 
     __device__ __forceinline__ unsigned off(int s) const
     {
-        return s == SK_ES ? 0u : (s == SK_GS ? cap_r : (s == SK_EH ? 2u * cap_r : 2u * cap_r + kPend));
+        return s == SK_ES ? 0u : (s == SK_GS ? cap_r : 2u * cap_r + static_cast<unsigned>(s - SK_EH) * kPend);
     }
     __device__ __forceinline__ unsigned cap(int s) const { return s < 2 ? cap_r : kPend; }
     __device__ __forceinline__ void count(int k, unsigned mask) const
@@ -291,7 +291,7 @@ __device__ __forceinline__ int electron_mode(const PersistArgs &a, const float *
         // unchanged by parking, and the two modes' rules exclude each other, so a change is never
         // undone before some work has been done)
         const unsigned ready = static_cast<unsigned>(__popc(live)) + w.n[SK_ES];
-        const unsigned E = ready + w.n[SK_EH], G = w.n[SK_GS] + w.n[SK_GI];
+        const unsigned E = ready + w.n[SK_EH], G = w.n[SK_GS] + w.n[SK_GI] + w.n[SK_GR];
         const unsigned must = w.cap_r - kMustMargin;
         const bool src_g = !src_is_e && !cl.empty();
         bool leave = G >= w.high_g && (E < w.high_e || (G >= must && E < must));
@@ -326,6 +326,47 @@ __device__ __forceinline__ int electron_mode(const PersistArgs &a, const float *
     }
 }
 
+// Photon mode, interactions of up to 32 photons waiting in stack sk (H2).  KIND != 0: all of them are of
+// that kind (the compiler drops the other branches of photon_interact); else the kind is in the record.
+template <bool TRACE, int KIND>
+__device__ __forceinline__ void interact_batch(const Params &P, Warp &w, int sk, Particle &p, bool &alive)
+{
+    const unsigned lane = threadIdx.x & 31;
+    w.push(P, SK_GS, alive, p, 0u); // park the photons in flight
+    alive = false;
+    const unsigned nb = min(32u, w.n[sk]);
+    // the interaction code pushes from divergent branches: the two ready stacks' counts go through shared
+    // memory for its duration
+    if (lane == 0) {
+        w.ctl->n_es = w.n[SK_ES];
+        w.ctl->n_gs = w.n[SK_GS];
+    }
+    __syncwarp();
+    int kind = 0;
+    if (lane < nb) {
+        uint32_t kbits;
+        p = load_rec(w.A, w.B, w.C, w.off(sk) + w.n[sk] - 1u - lane, kbits);
+        kind = KIND ? KIND : static_cast<int>(kbits);
+        const WarpStack qE{w.A + w.off(SK_ES), w.B + w.off(SK_ES), w.C + w.off(SK_ES), &w.ctl->n_es,
+                           &w.ctl->wc[WC_PUSH_E], w.cap_r};
+        const WarpStack qG{w.A + w.off(SK_GS), w.B + w.off(SK_GS), w.C + w.off(SK_GS), &w.ctl->n_gs,
+                           &w.ctl->wc[WC_PUSH_G], w.cap_r};
+        alive = photon_interact<TRACE>(P, p, kind, qE, qG) == PM_FLIGHT;
+    }
+    __syncwarp();
+    w.n[SK_ES] = w.ctl->n_es;
+    w.n[SK_GS] = w.ctl->n_gs;
+    w.n[sk] -= nb;
+    w.hw = max(w.hw, max(w.n[SK_ES], w.n[SK_GS]));
+    if (KIND == PM_COMPTON) {
+        w.count(WC_COMPTON, __ballot_sync(kFull, kind == PM_COMPTON));
+    } else {
+        w.count(WC_PHOTO, __ballot_sync(kFull, kind == PM_PHOTO));
+        w.count(WC_PAIR, __ballot_sync(kFull, kind == PM_PAIR));
+    }
+    __syncwarp();
+}
+
 // ---------------------------------------------------------------------------------------------
 // Photon mode: the lanes hold photons due a flight.  Returns the type to go on with (1 electrons,
 // -1 nothing left); on return no lane holds a particle.
@@ -341,43 +382,21 @@ __device__ __forceinline__ int photon_mode(const PersistArgs &a, const float *__
     for (;;) {
         const unsigned live = __ballot_sync(kFull, alive);
         const bool src_g = src_is_g && !cl.empty();
-        // ---- interactions of 32 waiting photons (or of what is left when nothing else can move)
-        if (w.n[SK_GI] >= 32u || (w.n[SK_GI] != 0u && live == 0u && w.n[SK_GS] == 0u && !src_g)) {
-            w.push(P, SK_GS, alive, p, 0u); // park the photons in flight
-            alive = false;
-            const unsigned nb = min(32u, w.n[SK_GI]);
-            // the interaction code pushes from divergent branches: the two ready stacks' counts go
-            // through shared memory for its duration
-            if (lane == 0) {
-                w.ctl->n_es = w.n[SK_ES];
-                w.ctl->n_gs = w.n[SK_GS];
-            }
-            __syncwarp();
-            int kind = 0;
-            if (lane < nb) {
-                uint32_t kbits;
-                p = load_rec(w.A, w.B, w.C, w.off(SK_GI) + w.n[SK_GI] - 1u - lane, kbits);
-                kind = static_cast<int>(kbits);
-                const WarpStack qE{w.A + w.off(SK_ES), w.B + w.off(SK_ES), w.C + w.off(SK_ES), &w.ctl->n_es,
-                                   &w.ctl->wc[WC_PUSH_E], w.cap_r};
-                const WarpStack qG{w.A + w.off(SK_GS), w.B + w.off(SK_GS), w.C + w.off(SK_GS), &w.ctl->n_gs,
-                                   &w.ctl->wc[WC_PUSH_G], w.cap_r};
-                alive = photon_interact<TRACE>(P, p, kind, qE, qG) == PM_FLIGHT;
-            }
-            __syncwarp();
-            w.n[SK_ES] = w.ctl->n_es;
-            w.n[SK_GS] = w.ctl->n_gs;
-            w.n[SK_GI] -= nb;
-            w.hw = max(w.hw, max(w.n[SK_ES], w.n[SK_GS]));
-            w.count(WC_COMPTON, __ballot_sync(kFull, kind == PM_COMPTON));
-            w.count(WC_PHOTO, __ballot_sync(kFull, kind == PM_PHOTO));
-            w.count(WC_PAIR, __ballot_sync(kFull, kind == PM_PAIR));
-            __syncwarp();
+        // ---- interactions of 32 waiting photons (or of what is left when nothing else can move): Compton
+        // events wait in GI, the rare photoelectric and pair events in GR, so that a batch of Compton events
+        // does not drag the long pair code along for one or two lanes
+        const bool stuck = live == 0u && w.n[SK_GS] == 0u && !src_g;
+        if (w.n[SK_GI] >= 32u || (w.n[SK_GI] != 0u && stuck)) {
+            interact_batch<TRACE, PM_COMPTON>(P, w, SK_GI, p, alive);
+            continue;
+        }
+        if (w.n[SK_GR] >= 32u || (w.n[SK_GR] != 0u && stuck)) {
+            interact_batch<TRACE, 0>(P, w, SK_GR, p, alive);
             continue;
         }
         // ---- change of particle type?  (see electron_mode)
         const unsigned ready = static_cast<unsigned>(__popc(live)) + w.n[SK_GS];
-        const unsigned G = ready + w.n[SK_GI], E = w.n[SK_ES] + w.n[SK_EH];
+        const unsigned G = ready + w.n[SK_GI] + w.n[SK_GR], E = w.n[SK_ES] + w.n[SK_EH];
         const unsigned must = w.cap_r - kMustMargin;
         const bool src_e = !src_is_g && !cl.empty();
         bool leave = E >= w.high_e && (G < w.high_g || E >= must);
@@ -405,7 +424,8 @@ __device__ __forceinline__ int photon_mode(const PersistArgs &a, const float *__
         if (alive) mode = photon_flight<TRACE>(P, TB, p);
         w.count(WC_FLIGHT, fl);
         w.count(WC_FICT, __ballot_sync(kFull, mode == PM_FLIGHT));
-        w.push(P, SK_GI, mode >= PM_COMPTON, p, static_cast<uint32_t>(mode));
+        w.push(P, SK_GI, mode == PM_COMPTON, p, static_cast<uint32_t>(mode));
+        w.push(P, SK_GR, mode > PM_COMPTON, p, static_cast<uint32_t>(mode)); // photoelectric and pair events: rare
         alive = mode == PM_FLIGHT;
     }
 }
@@ -438,7 +458,7 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(const __grid_consta
     w.cap_r = a.cap_r;
     w.high_g = a.high_g;
     w.high_e = a.high_e;
-    w.n[0] = w.n[1] = w.n[2] = w.n[3] = 0u;
+    w.n[0] = w.n[1] = w.n[2] = w.n[3] = w.n[4] = 0u;
     w.lt = (1u << lane) - 1u;
     w.hw = 0u;
     w.ctl = &s_ctl[threadIdx.x >> 5];
