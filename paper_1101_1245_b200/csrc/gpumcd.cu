@@ -713,7 +713,7 @@ static int run_persistent(gpumcd_ctx *ctx, uint64_t h_begin, uint64_t n_hist, ui
         // banked particles of the other type that make a warp change to it: photons are cheap to work off
         // (few per batch keeps the drain short), electrons are worth a fuller batch
 #ifndef GPUMCD_HG512
-#define GPUMCD_HG512 96u
+#define GPUMCD_HG512 80u
 #endif
 #ifndef GPUMCD_HE512
 #define GPUMCD_HE512 160u

@@ -294,7 +294,10 @@ __device__ __forceinline__ int electron_mode(const PersistArgs &a, const float *
         const unsigned E = ready + w.n[SK_EH], G = w.n[SK_GS] + w.n[SK_GI] + w.n[SK_GR];
         const unsigned must = w.cap_r - kMustMargin;
         const bool src_g = !src_is_e && !cl.empty();
-        bool leave = G >= w.high_g && (E < w.high_e || (G >= must && E < must));
+        // (only READY photons count towards the high-water mark: photon mode stays while it has kLow of them,
+        // so a change made here is never undone before some work has been done)
+        const unsigned Gr = w.n[SK_GS];
+        bool leave = Gr >= w.high_g && (E < w.high_e || (Gr >= must && E < must));
         if (!src_e) {
             if (ready == 0u) return (G != 0u || src_g) ? 0 : -1; // (EH is empty here)
             leave = leave || (ready < kLow && (src_g || w.n[SK_GS] >= 32u));
@@ -399,7 +402,8 @@ __device__ __forceinline__ int photon_mode(const PersistArgs &a, const float *__
         const unsigned G = ready + w.n[SK_GI] + w.n[SK_GR], E = w.n[SK_ES] + w.n[SK_EH];
         const unsigned must = w.cap_r - kMustMargin;
         const bool src_e = !src_is_g && !cl.empty();
-        bool leave = E >= w.high_e && (G < w.high_g || E >= must);
+        const unsigned Er = w.n[SK_ES];
+        bool leave = Er >= w.high_e && (G < w.high_g || Er >= must);
         if (!src_g) {
             if (ready == 0u) return (E != 0u || src_e) ? 1 : -1; // (GI is empty here)
             leave = leave || (ready < kLow && (src_e || w.n[SK_ES] >= 32u));
