@@ -34,9 +34,9 @@ if ROOT not in sys.path:
 # issue peak = 148 SMs x 4 schedulers x 32 lanes x 1 inst/clk x max SM clock.
 ALG_INST_PER_CH_STEP = 330.0
 # dram__bytes_read.sum + dram__bytes_write.sum of k_persistent per launch, from the `ncu --set full` capture
-# summarised in profiles/r01d_ncu_k_persistent_final.md (a profiler figure, per workload; None = not captured).
+# summarised in profiles/r01e_ncu_k_persistent_last.md (a profiler figure, per workload; None = not captured).
 # The algorithmic DRAM bytes are the first touch of phantom + tally + dose (42 MB for config 2).
-NCU_DRAM_BYTES_PER_LAUNCH = {"cfg2_15MeV_electron_10x10_water128": 39.5e6 + 72.4e6}
+NCU_DRAM_BYTES_PER_LAUNCH = {"cfg2_15MeV_electron_10x10_water128": 42.8e6 + 102.3e6}
 N_SM, N_SCHED, LANES = 148, 4, 32
 
 
