@@ -357,3 +357,34 @@ def test_tally_probe(workloads):
         after = g.gpumcd_get_counters(ctx)
         assert after["ch_steps"] == before["ch_steps"]
         assert after["e_dep_continuous"] == pytest.approx(before["e_dep_continuous"], rel=1e-12)
+
+
+@pytest.mark.parametrize("cfg,n_oracle", [(4, 1_000_000), (5, 1_000_000)])
+def test_full_size_properties(cfg, n_oracle, workloads):
+    """Configs 4 and 5 at BASELINE.json's full history counts (2e7, 1e8), default options = the launch
+    configuration bench.py times.  The oracle cannot run these sizes in seconds, so what is checked is what
+    holds at any size: the energy audit, the tally against its own total, and per-history averages and the
+    laterally integrated depth dose against the oracle's bounded sample of the same stream family."""
+    w = workloads[cfg]
+    n = w.n_histories
+    g = run_gpu(w, n)
+    c = g["counters"]
+    assert c["n_histories"] == n and c["overflow_count"] == 0
+    out = total_deposit(c) + c["e_escaped"]
+    assert abs(out / c["e_incident"] - 1.0) <= 1e-6                       # BASELINE.json: energy conservation
+    assert g["edep"].sum() == pytest.approx(total_deposit(c), rel=1e-9)
+    assert np.isfinite(g["dose"]).all() and (g["dose"] >= 0).all() and (g["edep"] >= 0).all()
+    mass = w.density.astype(np.float64) * w.voxel_cm ** 3
+    np.testing.assert_allclose(g["dose"], g["edep"] / mass / n, rtol=2e-6, atol=0)      # H8
+    o = oracle.run_workload(w, n_oracle)
+    if w.source.spec_edges is None:
+        assert c["e_incident"] == pytest.approx(n * w.source.energy, rel=1e-7)
+    else:
+        assert c["e_incident"] / n == pytest.approx(o.counters["e_incident"] / n_oracle, rel=5e-3)
+    # per-history averages: the oracle's sample is the first n_oracle histories of the same streams
+    for k in INT_KEYS:
+        assert c[k] / n == pytest.approx(o.counters[k] / n_oracle, rel=0.02), k
+    assert total_deposit(c) / n == pytest.approx(total_deposit(o.counters) / n_oracle, rel=0.01)
+    dg = g["edep"].sum(axis=(1, 2)) / n
+    do = o.edep.sum(axis=(1, 2)) / n_oracle
+    assert np.abs(dg - do).max() <= 0.03 * do.max()      # the oracle sample's noise per depth bin is ~1 %
