@@ -264,3 +264,61 @@ def run_pathlen(density, material, voxel_cm, tables, source, n_histories, seed, 
         raise RuntimeError(f"orc_run_pathlen failed with code {rc}")
     del keep_t, keep_s
     return out
+
+
+VLOG_COLS = 24
+VLOG = {"hist": 0, "kind": 1, "parent_track": 2, "parent_ctr": 3, "E0": 4, "d0": slice(5, 8), "E1": 8,
+        "d1": slice(9, 12), "child_type": 12, "child_track": 13, "child_E": 14, "child_d": slice(15, 18),
+        "x": slice(18, 21)}
+COMPTON, PHOTO, PAIR, MOLLER, BREMS = 1, 2, 3, 4, 5
+
+
+def run_endstate(density, material, voxel_cm, tables, source, n_histories, seed, options: Options = None,
+                 max_steps: int = 0):
+    """End state of every history's primary track: (end[n, 8] = x, y, z, u, v, w, E, steps taken;
+    pathmat[n, n_materials] = the primary electron's path length per material)."""
+    options = options or Options()
+    density = np.ascontiguousarray(density, np.float32)
+    material = np.ascontiguousarray(material, np.uint8)
+    nz, ny, nx = density.shape
+    t, keep_t = _tables_c(tables)
+    s, keep_s = _source_c(source)
+    o = options.c()
+    end = np.zeros((int(n_histories), 8))
+    pathmat = np.zeros((int(n_histories), tables.n_materials))
+    f = lib().orc_run_endstate
+    f.restype = C.c_int
+    rc = f(_p(density), _p(material), C.c_int32(nx), C.c_int32(ny), C.c_int32(nz),
+           C.c_double(float(np.float32(voxel_cm))), C.byref(t), C.byref(o), C.byref(s),
+           C.c_uint64(int(n_histories)), C.c_uint64(seed), C.c_int64(int(max_steps)), _p(end), _p(pathmat))
+    if rc != 0:
+        raise RuntimeError(f"orc_run_endstate failed with code {rc}")
+    del keep_t, keep_s
+    return end, pathmat
+
+
+def run_vertices(density, material, voxel_cm, tables, source, n_histories, seed, options: Options = None,
+                 cap: int = 4_000_000):
+    """Log of every pushed secondary with its vertex: (rows[n_pushed, VLOG_COLS], counters); columns in VLOG."""
+    options = options or Options()
+    density = np.ascontiguousarray(density, np.float32)
+    material = np.ascontiguousarray(material, np.uint8)
+    nz, ny, nx = density.shape
+    t, keep_t = _tables_c(tables)
+    s, keep_s = _source_c(source)
+    o = options.c()
+    rows = np.zeros((int(cap), VLOG_COLS))
+    n_out = C.c_int64(0)
+    cnt = Counters()
+    f = lib().orc_run_vertices
+    f.restype = C.c_int
+    rc = f(_p(density), _p(material), C.c_int32(nx), C.c_int32(ny), C.c_int32(nz),
+           C.c_double(float(np.float32(voxel_cm))), C.byref(t), C.byref(o), C.byref(s),
+           C.c_uint64(int(n_histories)), C.c_uint64(seed), _p(rows), C.c_int64(int(cap)), C.byref(n_out),
+           C.byref(cnt))
+    if rc != 0:
+        raise RuntimeError(f"orc_run_vertices failed with code {rc}")
+    if n_out.value > cap:
+        raise RuntimeError(f"vertex log too small: {n_out.value} secondaries, capacity {cap}")
+    del keep_t, keep_s
+    return rows[:n_out.value].copy(), cnt.as_dict()

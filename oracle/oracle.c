@@ -367,6 +367,13 @@ typedef struct {
     int trace_n;
     int want_trace;
     double *pathlen; /* NULL, or where to accumulate the primary electron's path length */
+    /* pins of the transport loop itself (orc_run_endstate, orc_run_vertices): NULL / 0 unless asked for */
+    double *end;      /* 8 doubles: where and how the primary track ended (x, d, E, steps taken) */
+    double *pathmat;  /* n_materials doubles: the primary electron's path length per material */
+    int64_t max_steps; /* > 0: the primary electron is stopped after this many condensed-history steps */
+    double *vlog;     /* ORC_VLOG_COLS doubles per pushed secondary */
+    int64_t vlog_cap, vlog_n;
+    double vtx[12];   /* the vertex being processed: kind, parent track, parent ctr, E0, d0, E1, d1, (pad) */
     /* history-by-history second moment (Eq. 13): NULL unless asked for */
     double *esq;     /* sum over histories of (energy the history left in the voxel)^2 */
     double *etmp;    /* energy the current history has left in each voxel so far */
@@ -442,6 +449,19 @@ static void push(world_t *W, int type, const double x[3], const double d[3], dou
     p->track = track;
     p->ctr = 0;
     p->primary = 0;
+    if (W->vlog) {
+        /* one row per pushed secondary: the vertex (set by the caller) and the child as pushed */
+        if (W->vlog_n < W->vlog_cap) {
+            double *r = W->vlog + (size_t)W->vlog_n * ORC_VLOG_COLS;
+            r[0] = (double)W->hist;
+            memcpy(r + 1, W->vtx, sizeof(double) * 11);
+            r[12] = (double)type; r[13] = (double)track; r[14] = E;
+            r[15] = d[0]; r[16] = d[1]; r[17] = d[2];
+            r[18] = x[0]; r[19] = x[1]; r[20] = x[2];
+            r[21] = r[22] = r[23] = 0.0;
+        }
+        W->vlog_n++;
+    }
     if (type == 0) W->c.pushes_g++; else W->c.pushes_e++;
     if ((uint64_t)W->sp > W->c.stack_high_water) W->c.stack_high_water = (uint64_t)W->sp;
 }
@@ -452,6 +472,27 @@ static void trace_event(world_t *W, const particle_t *p, int code)
         W->trace |= (uint64_t)code << (3 * W->trace_n);
         W->trace_n++;
     }
+}
+
+/* orc_run_vertices: describe the vertex whose secondaries are about to be pushed.  kind: 1 Compton,
+ * 2 photoelectric, 3 pair, 4 Moller, 5 bremsstrahlung.  (E0, d0): the parent before the event,
+ * (E1, d1): after it (E1 = 0 if it is absorbed). */
+static void vertex(world_t *W, int kind, const stream_t *s, double E0, const double d0[3], double E1,
+                   const double d1[3])
+{
+    if (!W->vlog) return;
+    W->vtx[0] = (double)kind; W->vtx[1] = (double)s->track; W->vtx[2] = (double)s->ctr;
+    W->vtx[3] = E0; W->vtx[4] = d0[0]; W->vtx[5] = d0[1]; W->vtx[6] = d0[2];
+    W->vtx[7] = E1; W->vtx[8] = d1[0]; W->vtx[9] = d1[1]; W->vtx[10] = d1[2];
+}
+
+/* orc_run_endstate: where and how the primary track ended */
+static void end_state(world_t *W, const particle_t *p, int64_t steps)
+{
+    if (!W->end || !p->primary) return;
+    W->end[0] = p->x[0]; W->end[1] = p->x[1]; W->end[2] = p->x[2];
+    W->end[3] = p->d[0]; W->end[4] = p->d[1]; W->end[5] = p->d[2];
+    W->end[6] = p->E; W->end[7] = (double)steps;
 }
 
 /* An electron is born with kinetic energy T at x: transported if T >= E_cut and electrons
@@ -488,7 +529,9 @@ static void photon_history(world_t *W, particle_t p)
         double r = U(w[1]) * mu_max;
         double c1 = rho * tab_photon(W, m, 0, lnE);
         double c2 = c1 + rho * tab_photon(W, m, 1, lnE);
-        double c3 = c2 + rho * tab_photon(W, m, 2, lnE);
+        /* pair production needs E > 2 m (L74): the column interpolated between the nodes around the
+         * threshold is not zero just below it (R33) */
+        double c3 = c2 + (p.E > 2.0 * M_E ? rho * tab_photon(W, m, 2, lnE) : 0.0);
         if (r < c1) {
             /* ---- Compton (L65) ---- */
             W->c.photon_compton++;
@@ -506,6 +549,7 @@ static void photon_history(world_t *W, particle_t p)
                 for (int a = 0; a < 3; ++a) q[a] /= n;
                 uint32_t id[4];
                 lineage(&s, id);
+                vertex(W, 1, &s, p.E, p.d, E1, dnew);
                 push(W, 1, p.x, q, Te, id[0]);
             } else {
                 deposit(W, v, Te, DEP_CUTOFF);
@@ -528,6 +572,7 @@ static void photon_history(world_t *W, particle_t p)
                 rotate(p.d, 1.0 - nu, s2 > 0.0 ? sqrt(s2) : 0.0, phi, q);
                 uint32_t id[4];
                 lineage(&s, id);
+                vertex(W, 2, &s, p.E, p.d, 0.0, p.d);
                 push(W, 1, p.x, q, p.E, id[0]);
             } else {
                 deposit(W, v, p.E, DEP_CUTOFF);
@@ -557,6 +602,7 @@ static void photon_history(world_t *W, particle_t p)
             int t1 = electron_is_tracked(W, T1), t2 = electron_is_tracked(W, T2);
             uint32_t id[4] = { 0, 0, 0, 0 };
             if (t1 || t2 || W->opt.pair_mode == 1) lineage(&s, id);
+            vertex(W, 3, &s, p.E, p.d, 0.0, p.d);
             if (t1) push(W, 1, p.x, q1, T1, id[0]); else deposit(W, v, T1, DEP_CUTOFF);
             if (t2) push(W, 1, p.x, q2, T2, id[1]); else deposit(W, v, T2, DEP_CUTOFF);
             W->c.e_pair_rest += 2.0 * M_E;
@@ -630,9 +676,16 @@ static void electron_history(world_t *W, particle_t p)
     const orc_tables *t = W->t;
     const double e_cut = t->e_cut, h = W->h;
     int v[3];
-    if (!locate(W, p.x, v)) { W->c.e_escaped += p.E; return; }
-    if (!electron_is_tracked(W, p.E)) { deposit(W, v, p.E, DEP_CUTOFF); return; }
+    int64_t steps = 0;
+    if (!locate(W, p.x, v)) { W->c.e_escaped += p.E; end_state(W, &p, steps); return; }
+    if (!electron_is_tracked(W, p.E)) { deposit(W, v, p.E, DEP_CUTOFF); end_state(W, &p, steps); return; }
     for (;;) {
+        if (W->max_steps > 0 && p.primary && steps == W->max_steps) {
+            /* orc_run_endstate: the primary is taken out of the run here (audited as escaped) */
+            W->c.e_escaped += p.E;
+            end_state(W, &p, steps);
+            return;
+        }
         size_t iv = vindex(W, v);
         int m = W->material[iv];
         double rho = (double)W->density[iv];
@@ -668,13 +721,16 @@ static void electron_history(world_t *W, particle_t p)
         if (Tmid < t->e_min) Tmid = t->e_min;
         double dE = es * rho * tab_electron(W, m, 0, log(Tmid));
         W->c.ch_steps++;
+        steps++;
         if (T - dE < e_cut) {
             /* end of range: everything left is deposited in the current voxel (R8) */
             if (W->pathlen && p.primary) *W->pathlen += es * (T - e_cut) / dE;
             deposit(W, v, T, DEP_CUTOFF);
+            end_state(W, &p, steps);
             return;
         }
         if (W->pathlen && p.primary) *W->pathlen += es;
+        if (W->pathmat && p.primary) W->pathmat[m] += es;
         double zeta = U(a[1]);
         /* R32: the loss of a multi-voxel step goes to the voxel of a point drawn uniformly along the
          * step's path (first leg, then second leg): the path-length share of every voxel in expectation */
@@ -710,7 +766,7 @@ static void electron_history(world_t *W, particle_t p)
         }
         for (int k = 0; k < 3; ++k) p.x[k] += (1.0 - zeta) * es * p.d[k];
         p.E = T - dE;
-        if (!locate(W, p.x, v)) { W->c.e_escaped += p.E; return; }
+        if (!locate(W, p.x, v)) { W->c.e_escaped += p.E; end_state(W, &p, steps); return; }
         if (!hard) continue;
         /* ---- hard event: real or fictitious (L110-113), at the post-step energy ---- */
         uint32_t b[4];
@@ -719,7 +775,9 @@ static void electron_history(world_t *W, particle_t p)
         int m1 = W->material[iv];
         double rho1 = (double)W->density[iv];
         double lnT1 = log(p.E);
-        double sM = rho1 * tab_electron(W, m1, 1, lnT1);
+        /* a Moller event transfers W in [K_cut, T/2] (L90): none is possible for T <= 2 K_cut, where the
+         * column interpolated between the nodes around the threshold is not zero (R33) */
+        double sM = p.E > 2.0 * e_cut ? rho1 * tab_electron(W, m1, 1, lnT1) : 0.0;
         double sB = rho1 * tab_electron(W, m1, 2, lnT1);
         double r = U(b[0]) * M;
         if (r < sM) {
@@ -735,6 +793,7 @@ static void electron_history(world_t *W, particle_t p)
             rotate(p.d, sqrt(c2d), sqrt(1.0 - c2d > 0.0 ? 1.0 - c2d : 0.0), phi + 0.5 * TWO_PI, dd);
             uint32_t id[4];
             lineage(&s, id);
+            vertex(W, 4, &s, T1, p.d, T1 - Wd, dp);
             push(W, 1, p.x, dd, Wd, id[0]); /* Wd >= K_cut = E_cut: always tracked */
             p.E = T1 - Wd;
             memcpy(p.d, dp, sizeof dp);
@@ -748,9 +807,10 @@ static void electron_history(world_t *W, particle_t p)
             rotate(p.d, cos(th), sin(th), phi, dg);
             uint32_t id[4];
             lineage(&s, id);
+            vertex(W, 5, &s, T1, p.d, T1 - k, p.d);
             push(W, 0, p.x, dg, k, id[0]); /* k >= k_c = P_cut: always tracked */
             p.E = T1 - k;
-            if (p.E < e_cut) { deposit(W, v, p.E, DEP_CUTOFF); return; }
+            if (p.E < e_cut) { deposit(W, v, p.E, DEP_CUTOFF); end_state(W, &p, steps); return; }
         } else {
             W->c.hard_fict++;
         }
@@ -784,11 +844,21 @@ static int make_primary(world_t *W, const orc_source *src, const double *cdf, pa
     return 0;
 }
 
+/* outputs of the transport-loop pins (single worker; all NULL / 0 in a plain run) */
+typedef struct {
+    double *end;      /* [n_hist][8] */
+    double *pathmat;  /* [n_hist][n_materials] */
+    int64_t max_steps;
+    double *vlog;     /* [vlog_cap][ORC_VLOG_COLS] */
+    int64_t vlog_cap;
+    int64_t *vlog_n;
+} pins_t;
+
 static int run_impl(const float *density, const uint8_t *material, int32_t nx, int32_t ny,
                     int32_t nz, double voxel_cm, const orc_tables *t, const orc_options *opt,
                     const orc_source *src, uint64_t hist_begin, uint64_t n_hist, uint64_t seed,
                     double *edep_out, float *dose_out, uint64_t *trace_out, orc_counters *counters,
-                    int32_t n_threads, double *pathlen_out, double *edep_sq_out)
+                    int32_t n_threads, double *pathlen_out, double *edep_sq_out, const pins_t *pins)
 {
     if (!density || !material || !t || !opt || !src || !edep_out) return -1;
     if (nx <= 0 || ny <= 0 || nz <= 0 || voxel_cm <= 0.0) return -1;
@@ -848,6 +918,7 @@ static int run_impl(const float *density, const uint8_t *material, int32_t nx, i
         }
         W->seed = seed;
         W->want_trace = trace_out != NULL;
+        if (pins) { W->max_steps = pins->max_steps; W->vlog = pins->vlog; W->vlog_cap = pins->vlog_cap; }
 #ifdef _OPENMP
 #pragma omp for schedule(static)
 #endif
@@ -857,6 +928,11 @@ static int run_impl(const float *density, const uint8_t *material, int32_t nx, i
             W->sp = 0; W->trace = 0; W->trace_n = 0;
             W->pathlen = pathlen_out ? &pathlen_out[ih] : NULL;
             if (W->pathlen) *W->pathlen = 0.0;
+            if (pins && pins->end) { W->end = pins->end + 8 * ih; memset(W->end, 0, 8 * sizeof(double)); }
+            if (pins && pins->pathmat) {
+                W->pathmat = pins->pathmat + (size_t)t->n_materials * ih;
+                memset(W->pathmat, 0, sizeof(double) * (size_t)t->n_materials);
+            }
             particle_t p;
             make_primary(W, src, cdf, &p);
             W->c.e_incident += p.E;
@@ -884,6 +960,7 @@ static int run_impl(const float *density, const uint8_t *material, int32_t nx, i
         world_t *W = workers[k];
         if (!W) continue;
         if (W->overflow) failed = 1;
+        if (pins && pins->vlog_n) *pins->vlog_n = W->vlog_n;
         if (k > 0) {
             for (size_t i = 0; i < nvox; ++i) edep_out[i] += W->edep[i];
             free(W->edep);
@@ -924,7 +1001,7 @@ int orc_run(const float *density, const uint8_t *material, int32_t nx, int32_t n
             uint64_t *trace_out, orc_counters *counters, int32_t n_threads)
 {
     return run_impl(density, material, nx, ny, nz, voxel_cm, t, opt, src, hist_begin, n_hist, seed,
-                    edep_out, dose_out, trace_out, counters, n_threads, NULL, NULL);
+                    edep_out, dose_out, trace_out, counters, n_threads, NULL, NULL, NULL);
 }
 
 /* As orc_run, and also the per-voxel sum over histories of the squared energy a history deposits
@@ -937,7 +1014,7 @@ int orc_run_moments(const float *density, const uint8_t *material, int32_t nx, i
 {
     if (!edep_sq_out) return -1;
     return run_impl(density, material, nx, ny, nz, voxel_cm, t, opt, src, hist_begin, n_hist, seed,
-                    edep_out, NULL, NULL, counters, n_threads, NULL, edep_sq_out);
+                    edep_out, NULL, NULL, counters, n_threads, NULL, edep_sq_out, NULL);
 }
 
 int orc_run_pathlen(const float *density, const uint8_t *material, int32_t nx, int32_t ny,
@@ -948,7 +1025,49 @@ int orc_run_pathlen(const float *density, const uint8_t *material, int32_t nx, i
     double *edep = (double *)malloc(sizeof(double) * nvox);
     if (!edep) return -3;
     int rc = run_impl(density, material, nx, ny, nz, voxel_cm, t, opt, src, 0, n_hist, seed, edep,
-                      NULL, NULL, NULL, 1, pathlen_out, NULL);
+                      NULL, NULL, NULL, 1, pathlen_out, NULL, NULL);
+    free(edep);
+    return rc;
+}
+
+/* Transport-loop pin: the state in which each history's PRIMARY track ended (end_out[n_hist][8] = position,
+ * direction, energy, condensed-history steps taken) and, for an electron primary, its path length per material
+ * (pathmat_out[n_hist][n_materials], step lengths booked on the step-start voxel's material; may be NULL).
+ * max_steps > 0 takes the primary electron out of the run after that many steps.  One worker. */
+int orc_run_endstate(const float *density, const uint8_t *material, int32_t nx, int32_t ny, int32_t nz,
+                     double voxel_cm, const orc_tables *t, const orc_options *opt, const orc_source *src,
+                     uint64_t n_hist, uint64_t seed, int64_t max_steps, double *end_out, double *pathmat_out)
+{
+    if (!end_out || max_steps < 0) return -1;
+    size_t nvox = (size_t)nx * ny * nz;
+    double *edep = (double *)malloc(sizeof(double) * nvox);
+    if (!edep) return -3;
+    pins_t pins = { end_out, pathmat_out, max_steps, NULL, 0, NULL };
+    int rc = run_impl(density, material, nx, ny, nz, voxel_cm, t, opt, src, 0, n_hist, seed, edep, NULL, NULL,
+                      NULL, 1, NULL, NULL, &pins);
+    free(edep);
+    return rc;
+}
+
+/* Transport-loop pin: one row of ORC_VLOG_COLS doubles per secondary, in the order they are pushed, as they
+ * are pushed (the in-situ kinematics, not a re-typed copy).  Columns: 0 history, 1 vertex kind (1 Compton,
+ * 2 photoelectric, 3 pair, 4 Moller, 5 bremsstrahlung), 2 parent track id, 3 parent draw counter at the
+ * vertex, 4 parent energy before, 5-7 parent direction before, 8 parent energy after (0: absorbed), 9-11
+ * parent direction after, 12 child type (0 photon, 1 electron), 13 child track id, 14 child energy, 15-17
+ * child direction, 18-20 vertex position.  At most cap rows are written; *n_out receives the number of
+ * secondaries pushed.  One worker. */
+int orc_run_vertices(const float *density, const uint8_t *material, int32_t nx, int32_t ny, int32_t nz,
+                     double voxel_cm, const orc_tables *t, const orc_options *opt, const orc_source *src,
+                     uint64_t n_hist, uint64_t seed, double *vlog_out, int64_t cap, int64_t *n_out,
+                     orc_counters *counters)
+{
+    if (!vlog_out || cap <= 0 || !n_out) return -1;
+    size_t nvox = (size_t)nx * ny * nz;
+    double *edep = (double *)malloc(sizeof(double) * nvox);
+    if (!edep) return -3;
+    pins_t pins = { NULL, NULL, 0, vlog_out, cap, n_out };
+    int rc = run_impl(density, material, nx, ny, nz, voxel_cm, t, opt, src, 0, n_hist, seed, edep, NULL, NULL,
+                      counters, 1, NULL, NULL, &pins);
     free(edep);
     return rc;
 }

@@ -18,7 +18,12 @@
  * samplers against the analytic densities; narrow-beam attenuation exp(-mu x);
  * Woodcock invariance under an inflated majorant; CSDA range against
  * numerical integration of the stopping-power table; exact energy conservation;
- * brute-force expectation on a one-voxel phantom.
+ * brute-force expectation on a one-voxel phantom; and, for the transport loop itself
+ * (tests/test_oracle_pins.py): <cos theta> = exp(-int rho/lambda_1 ds) in uniform media and
+ * across a slab stack (martingale identity), the alternate hinge's two energies, momentum
+ * and energy conservation of every Compton / Moller / pair / bremsstrahlung vertex as it is
+ * pushed, Sauter angles of photo-electrons, distinct track ids within a history, and the
+ * kinematic thresholds of Moller and pair events.
  * PARITY UNPINNED: the dose grid as a whole has no external truth here (EGSnrc and
  * its data files are absent); it is pinned only through the pieces above.
  *
@@ -129,6 +134,18 @@ int orc_run_moments(const float *density, const uint8_t *material, int32_t nx, i
 int orc_run_pathlen(const float *density, const uint8_t *material, int32_t nx, int32_t ny,
                     int32_t nz, double voxel_cm, const orc_tables *t, const orc_options *opt,
                     const orc_source *src, uint64_t n_hist, uint64_t seed, double *pathlen_out);
+
+/* ---- pins of the transport loop itself (tests/test_oracle_pins.py) ---- */
+#define ORC_VLOG_COLS 24
+/* End state of every history's primary track, and the primary electron's path length per material. */
+int orc_run_endstate(const float *density, const uint8_t *material, int32_t nx, int32_t ny, int32_t nz,
+                     double voxel_cm, const orc_tables *t, const orc_options *opt, const orc_source *src,
+                     uint64_t n_hist, uint64_t seed, int64_t max_steps, double *end_out, double *pathmat_out);
+/* Log of every pushed secondary with its vertex (columns: see oracle.c). */
+int orc_run_vertices(const float *density, const uint8_t *material, int32_t nx, int32_t ny, int32_t nz,
+                     double voxel_cm, const orc_tables *t, const orc_options *opt, const orc_source *src,
+                     uint64_t n_hist, uint64_t seed, double *vlog_out, int64_t cap, int64_t *n_out,
+                     orc_counters *counters);
 
 #ifdef __cplusplus
 }
