@@ -4,11 +4,13 @@
     python bench.py --gpus N --steps K --warmup W            # the CUDA library (this repo)
     python bench.py --impl reference --steps K --warmup W    # the CPU oracle, timed as it stands
     python bench.py --paper-tables [--steps K]               # PAPER.md Tab. IV-VI measured here (markdown)
+    python bench.py --ablation [--steps K]                   # Tab. VI / L180 / L352 ablation on configs 2-5 (JSON)
 
 A "step" is one gpumcd_run of the whole hot path (source, photon and electron transport with all
-secondaries, tally, finalize) over one batch of synthetic histories.  Workload at N = 1: config 2 of
-BASELINE.json (15 MeV electrons, 10x10 cm^2 field, 1e6 histories, 128^3 water at 0.25 cm), the
-configuration the metric is quoted on.  --config selects another one.
+secondaries, tally, finalize) over one batch of synthetic histories.  BASELINE.json quotes its metric on
+no single configuration, so the workload at N = 1 is the largest single-GPU one, config 5 (18 MV spectrum,
+10x10 cm^2 field, 1e8 histories, 256x256x128 CT-like phantom at 0.2 cm); the same figures for all five
+configurations are in the line's `per_config` block.  --config selects another headline.
 
 Metric: coupled photon-electron histories/s (value) and condensed-history steps/s (ch_steps_per_s).
 Multi-GPU (--gpus N under torchrun): every rank simulates its own disjoint history range (weak
@@ -33,10 +35,6 @@ if ROOT not in sys.path:
 # thread-instructions one condensed-history step needs at minimum, and the
 # issue peak = 148 SMs x 4 schedulers x 32 lanes x 1 inst/clk x max SM clock.
 ALG_INST_PER_CH_STEP = 330.0
-# dram__bytes_read.sum + dram__bytes_write.sum of k_persistent per launch, from the `ncu --set full` capture
-# summarised in profiles/r01e_ncu_k_persistent_last.md (a profiler figure, per workload; None = not captured).
-# The algorithmic DRAM bytes are the first touch of phantom + tally + dose (42 MB for config 2).
-NCU_DRAM_BYTES_PER_LAUNCH = {"cfg2_15MeV_electron_10x10_water128": 42.8e6 + 102.3e6}
 N_SM, N_SCHED, LANES = 148, 4, 32
 
 
@@ -275,24 +273,221 @@ def paper_tables(args):
 
 
 
+def ablation(args):
+    """--ablation: the paper's divergence-reduction ablation (Tab. VI; compaction interval N, L180; pool, L182;
+    "grouping particles", L352) restated for this scheduler, on configs 2-5 at full size: scheduler 0 (the paper's
+    base scheme, with its wave size and bank factor d, L166) against scheduler 1, CTA size, tally mode, the
+    high-water marks that set how much work of one type a warp does before it picks up the other type, the
+    drain threshold, the stack capacity, and multi-voxel steps.  One JSON object on stdout; ms = median device
+    time of gpumcd_run over --steps runs after 3 warm-up runs, L2 flushed in between."""
+    import torch
+
+    import paper_1101_1245_b200 as g
+    from paper_1101_1245_b200.inputs import make_config
+    assert torch.cuda.is_available(), "needs a CUDA device"
+    variants = [("default", {}),
+                ("scheduler0", {"scheduler": 0}), ("scheduler0_wave2^18", {"scheduler": 0, "wave_size": 1 << 18}),
+                ("scheduler0_wave2^22_d4", {"scheduler": 0, "wave_size": 1 << 22, "bank_factor": 4}),
+                ("cta1024", {"cta_threads": 1024}),
+                ("tally_warp", {"tally_mode": 1}), ("tally_fixed", {"tally_mode": 2}),
+                ("high_g40", {"bank_high_g": 40}), ("high_g160", {"bank_high_g": 160}), ("high_g320", {"bank_high_g": 320}),
+                ("high_e80", {"bank_high_e": 80}), ("high_e320", {"bank_high_e": 320}), ("high_e640", {"bank_high_e": 640}),
+                ("low8", {"bank_low": 8}), ("low48", {"bank_low": 48}),
+                ("stack256", {"warp_stack": 256}), ("stack512", {"warp_stack": 512}),
+                ("hom_tol0.1", {"hom_tol": 0.1})]
+    out = {"what": "ms per gpumcd_run (median of %d, device time), full history counts" % args.steps, "configs": {}}
+    for c in (2, 3, 4, 5):
+        w = make_config(c)
+        row = {}
+        for name, o in variants:
+            if c == 5 and o.get("scheduler") == 0 and o.get("wave_size", 1 << 20) > (1 << 20):
+                continue                      # 4 queues x 2^22 x 4 x 48 B does not leave room for the rest
+            t, cnt = time_gpu(g, torch, w, w.n_histories, args.steps, **o)
+            row[name] = {"ms": round(t, 4), "ch_steps": cnt["ch_steps"], "bank_high_water": cnt["bank_high_water"]}
+        out["configs"][w.name] = row
+    print(json.dumps(out))
+    return 0
+
+
+def load_traffic_table():
+    """profiles/ncu_traffic.csv: DRAM bytes per launch of k_persistent from the kept `ncu --set full` captures
+    (dram__bytes_read.sum + dram__bytes_write.sum), one row per workload, written next to each ncu summary."""
+    out = {}
+    path = os.path.join(ROOT, "profiles", "ncu_traffic.csv")
+    if os.path.exists(path):
+        for line in open(path):
+            f = [x.strip() for x in line.split(",")]
+            if len(f) >= 4 and not line.startswith("#") and f[0] != "workload":
+                out[f[0]] = {"read": float(f[1]), "write": float(f[2]), "capture": f[3]}
+    return out
+
+
+# algorithmic DRAM bytes of one run: first touch of the phantom (8 B / voxel), the tally read + written back
+# (2 x 8 B / voxel) and the dose written (4 B / voxel); DESIGN.md 7 "Rooflines"
+def algorithmic_dram_bytes(w):
+    return int(w.density.size) * (8 + 16 + 4)
+
+
+def measure(g, torch, dist, w, n, opts, steps, warmup, dev, rank, world, flush, e2e=True, probe=True):
+    """Time `steps` runs of workload `w` (device time by CUDA events on the launching stream, L2 flushed in between),
+    then the same through the host entry points.  Returns the figures of one bench line."""
+    from paper_1101_1245_b200.sharding import combine_dose
+    rho = torch.from_numpy(w.density).to(dev)
+    mat = torch.from_numpy(w.material).to(dev)
+    dose = torch.empty(rho.shape, dtype=torch.float32, device=dev)
+    opt = g.gpumcd_default_options(**opts)
+    ctx = g.gpumcd_create(rho, mat, w.voxel_cm, w.tables, opt)
+    g.gpumcd_set_source(ctx, w.source)
+    g.gpumcd_set_history_offset(ctx, rank * n)       # disjoint history ranges per rank (PAPER.md L188)
+    g.gpumcd_set_profiling(ctx, True)
+
+    def step(seed):
+        g.gpumcd_run(ctx, n, seed, dose)
+        if dist:
+            combine_dose(dose, n, world * n, dist)    # "the resulting dose arrays are summed" (L188)
+
+    for k in range(warmup):
+        step(w.seed + k)
+    torch.cuda.synchronize()
+    if dist:
+        dist.barrier()
+    torch.cuda.synchronize()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    ch_steps = flights = launches = 0
+    ms_e = 0.0
+    n_e = 0
+    wall0 = time.perf_counter()
+    for k in range(steps):
+        flush.fill_(k & 0xFF)                          # evict the phantom / tally / tables from L2
+        torch.cuda.synchronize()
+        ev[k][0].record()
+        step(w.seed + 100 + k)
+        ev[k][1].record()
+        torch.cuda.synchronize()
+        c = g.gpumcd_get_counters(ctx)
+        p = g.gpumcd_get_profile(ctx)
+        ch_steps += c["ch_steps"]
+        flights += c["photon_flights"]
+        launches += p["launches"]
+        ms_e += p["ms_electron"] + p["ms_photon"]
+        n_e += p["n_electron"] + p["n_photon"]
+    if dist:
+        dist.barrier()
+    torch.cuda.synchronize()
+    wall = time.perf_counter() - wall0
+    t_ms = sum(a.elapsed_time(b) for a, b in ev)
+    if dist:
+        tt = torch.tensor([t_ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        t_ms = float(tt.item())
+        agg = torch.tensor([ch_steps, flights], dtype=torch.float64, device=dev)
+        dist.all_reduce(agg)
+        ch_steps, flights = (float(x) for x in agg.tolist())
+    t_s = t_ms * 1e-3
+    out = {"workload": w.name, "histories_per_step_per_gpu": n, "ms_per_step": t_ms / steps,
+           "value": world * steps * n / t_s, "ch_steps_per_s": ch_steps / t_s, "photon_flights_per_s": flights / t_s,
+           "gpu_launches": int(launches), "wall_s_timed_region": wall,
+           "bank_high_water": int(c["bank_high_water"])}
+
+    # ---- roofline of the dominant kernel (the transport kernel): issue-rate bound
+    peaks, peak_kind = measured_peaks()
+    peak_inst = N_SM * N_SCHED * LANES * peaks.get("sm_max_mhz", 1965.0) * 1e6
+    local_ch = ch_steps / world
+    achieved = ALG_INST_PER_CH_STEP * local_ch / (ms_e * 1e-3) if ms_e > 0 else None
+    traffic = load_traffic_table().get(w.name) if n == w.n_histories else None
+    out["roofline"] = {"bound": "alu", "kernel": "k_persistent (transport + tally + finalize)" if opt.scheduler == 1 else "transport passes",
+                       "achieved": achieved, "peak": peak_inst,
+                       "unit": "thread-inst/s", "frac": (achieved / peak_inst) if achieved else None,
+                       "traffic": (traffic["read"] + traffic["write"]) if traffic else None,
+                       "traffic_source": traffic["capture"] if traffic else None,
+                       "algorithmic_dram_bytes": algorithmic_dram_bytes(w),
+                       "peak_source": f"148 SMs x 4 x 32 x sm_max_mhz ({peak_kind})",
+                       "kernel_ms_per_step": ms_e / steps, "kernel_launches_per_step": n_e / steps,
+                       "kernel_share_of_step": ms_e / t_ms if t_ms else None,
+                       "alg_inst_per_ch_step": ALG_INST_PER_CH_STEP}
+
+    # ---- secondary rooflines (BASELINE.json north_star): the tally against the measured atomic rate of the L2
+    # (gpumcd_probe_tally: the same grid, the field's footprint, nothing but atomic adds of the tally's type), and the
+    # DRAM traffic of the ncu capture against the measured HBM copy bandwidth
+    if probe:
+        tally_peak = g.gpumcd_probe_tally(ctx, 200_000_000)
+        tally_rate = local_ch / t_s
+        out["roofline_tally"] = {"bound": "l2_atomic", "achieved": tally_rate, "peak": tally_peak,
+                                 "unit": ("u64" if opt.tally_mode == 2 else "fp64") + " atomic adds/s",
+                                 "frac": tally_rate / tally_peak, "tally_mode": int(opt.tally_mode),
+                                 "what": "one add per condensed-history step against gpumcd_probe_tally under this field"}
+    out["roofline_hbm"] = None
+    if traffic and ms_e > 0:
+        gbs = (traffic["read"] + traffic["write"]) / (ms_e / max(n_e, 1) * 1e-3) / 1e9
+        out["roofline_hbm"] = {"bound": "hbm", "achieved": gbs, "peak": peaks.get("hbm_gbs"), "unit": "GB/s",
+                               "frac": gbs / peaks.get("hbm_gbs"),
+                               "what": f"ncu DRAM bytes per launch / kernel time ({peak_kind} copy bandwidth)"}
+
+    # ---- end to end through the host entry points: every step copies that step's inputs (the phantom volumes,
+    # from pinned host memory) to the device and the resulting dose grid back to the host
+    out["e2e"] = None
+    if e2e:
+        rho_h = torch.from_numpy(w.density).pin_memory()
+        mat_h = torch.from_numpy(w.material).pin_memory()
+        dose_h = torch.empty(rho.shape, dtype=torch.float32).pin_memory()
+        rho_np, mat_np, dose_np = rho_h.numpy(), mat_h.numpy(), dose_h.numpy()
+
+        def e2e_step(seed):
+            g.gpumcd_set_phantom_host(ctx, rho_np, mat_np)
+            g.gpumcd_set_source(ctx, w.source)
+            g.gpumcd_run_host(ctx, n, seed, dose_np)          # returns after the device-to-host copy
+
+        g.gpumcd_set_profiling(ctx, False)
+        for k in range(warmup):
+            e2e_step(w.seed + 300 + k)
+        if dist:
+            dist.barrier()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for k in range(steps):
+            e2e_step(w.seed + 400 + k)
+        torch.cuda.synchronize()
+        e2e_t = (time.perf_counter() - t0) / steps
+        if dist:
+            tt = torch.tensor([e2e_t], dtype=torch.float64, device=dev)
+            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+            e2e_t = float(tt.item())
+        blob_bytes = 4 * (w.tables.photon.size + w.tables.electron.size + w.tables.ms_a.size + 2 * w.tables.n_energy)
+        out["e2e"] = {"value": world * n / e2e_t, "unit": "histories/s",
+                      "h2d_bytes_per_step": int(rho.numel() * 5 + blob_bytes), "d2h_bytes_per_step": int(rho.numel() * 4),
+                      "ms_per_step": e2e_t * 1e3,
+                      "what": "gpumcd_set_phantom_host + gpumcd_set_source + gpumcd_run_host per step, wall clock, pinned host buffers"}
+    out["options"] = {"scheduler": int(opt.scheduler), "hom_tol": float(opt.hom_tol), "wave_size": int(opt.wave_size),
+                      "tally_mode": int(opt.tally_mode), "cta_threads": int(opt.cta_threads) or 512}
+    g.gpumcd_destroy(ctx)
+    return out
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", type=int, default=2)
+    ap.add_argument("--config", type=int, default=5,
+                    help="the headline workload (default 5: the largest single-GPU configuration of BASELINE.json)")
+    ap.add_argument("--no-per-config", action="store_true",
+                    help="skip the per_config block (the other four configurations, measured the same way)")
     ap.add_argument("--histories", type=int, default=0, help="override histories per step (0 = the config's)")
     ap.add_argument("--scheduler", type=int, default=-1)
     ap.add_argument("--wave", type=int, default=0, help="override wave_size (0 = library default)")
     ap.add_argument("--cta-threads", type=int, default=0, help="override cta_threads (0 = the library's choice)")
+    ap.add_argument("--tally-mode", type=int, default=-1, help="override tally_mode (-1 = the library's default)")
+    ap.add_argument("--warp-stack", type=int, default=0, help="override warp_stack (0 = library default)")
     ap.add_argument("--hom-tol", type=float, default=0.0,
                     help="multi-voxel electron steps (gpumcd_options.hom_tol; 0 = Eq. 4 as printed, the default)")
-    ap.add_argument("--ref-histories", type=int, default=50_000)
+    ap.add_argument("--ref-histories", type=int, default=200_000)
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--paper-tables", action="store_true", help="print PAPER.md Tab. IV-VI measured here (markdown)")
+    ap.add_argument("--ablation", action="store_true",
+                    help="scheduling / tally ablation of PAPER.md Tab. VI and L180, L352 on configs 2-5 (JSON on stdout)")
     ap.add_argument("--oracle-fraction", type=float, default=0.02,
                     help="--paper-tables: share of the histories the oracle is timed on")
     args = ap.parse_args()
@@ -301,13 +496,14 @@ def main():
         return reference_arm(args)
     if args.paper_tables:
         return paper_tables(args)
+    if args.ablation:
+        return ablation(args)
 
     import torch
 
     import paper_1101_1245_b200 as g
     from paper_1101_1245_b200 import build as cuda_build
     from paper_1101_1245_b200.inputs import make_config
-    from paper_1101_1245_b200.sharding import combine_dose
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -326,11 +522,6 @@ def main():
         dist.barrier()
     g.load_library()
 
-    w = make_config(args.config)
-    n = args.histories or w.n_histories
-    rho = torch.from_numpy(w.density).to(dev)
-    mat = torch.from_numpy(w.material).to(dev)
-    dose = torch.empty(rho.shape, dtype=torch.float32, device=dev)
     opts = {}
     if args.scheduler >= 0:
         opts["scheduler"] = args.scheduler
@@ -340,124 +531,31 @@ def main():
         opts["cta_threads"] = args.cta_threads
     if args.hom_tol > 0:
         opts["hom_tol"] = args.hom_tol
-    opt = g.gpumcd_default_options(**opts)
-    ctx = g.gpumcd_create(rho, mat, w.voxel_cm, w.tables, opt)
-    g.gpumcd_set_source(ctx, w.source)
-    g.gpumcd_set_history_offset(ctx, rank * n)       # disjoint history ranges per rank
-    g.gpumcd_set_profiling(ctx, True)
+    if args.tally_mode >= 0:
+        opts["tally_mode"] = args.tally_mode
+    if args.warp_stack > 0:
+        opts["warp_stack"] = args.warp_stack
     flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev)   # > 126 MB L2
 
-    def step(seed):
-        g.gpumcd_run(ctx, n, seed, dose)
-        if dist:
-            combine_dose(dose, n, world * n, dist)    # "the resulting dose arrays are summed" (L188)
-
-    for k in range(args.warmup):
-        step(w.seed + k)
-    torch.cuda.synchronize()
-
+    w = make_config(args.config)
+    n = args.histories or w.n_histories
     sampler = ClockSampler(local)
     sampler.start()
-    if dist:
-        dist.barrier()
-    torch.cuda.synchronize()
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    ch_steps = flights = launches = 0
-    ms_e = ms_p = 0.0
-    n_e = n_p = 0
-    wall0 = time.perf_counter()
-    for k in range(args.steps):
-        flush.fill_(k & 0xFF)                          # evict the phantom / tally / tables from L2
-        torch.cuda.synchronize()
-        ev[k][0].record()
-        step(w.seed + 100 + k)
-        ev[k][1].record()
-        torch.cuda.synchronize()
-        c = g.gpumcd_get_counters(ctx)
-        p = g.gpumcd_get_profile(ctx)
-        ch_steps += c["ch_steps"]
-        flights += c["photon_flights"]
-        launches += p["launches"]
-        ms_e += p["ms_electron"]; ms_p += p["ms_photon"]
-        n_e += p["n_electron"]; n_p += p["n_photon"]
-    if dist:
-        dist.barrier()
-    torch.cuda.synchronize()
-    wall = time.perf_counter() - wall0
+    head = measure(g, torch, dist, w, n, opts, args.steps, args.warmup, dev, rank, world, flush, e2e=not args.no_e2e)
+    per_config = {}
+    if not args.no_per_config and not args.histories:
+        for c in (1, 2, 3, 4, 5):
+            if c == args.config:
+                per_config[f"cfg{c}"] = {k: head[k] for k in ("workload", "ms_per_step", "value", "ch_steps_per_s",
+                                                               "photon_flights_per_s", "roofline", "roofline_tally", "e2e")}
+                continue
+            wc = make_config(c)
+            m = measure(g, torch, dist, wc, wc.n_histories, opts, args.steps, args.warmup, dev, rank, world, flush,
+                        e2e=not args.no_e2e)
+            per_config[f"cfg{c}"] = {k: m[k] for k in ("workload", "ms_per_step", "value", "ch_steps_per_s",
+                                                        "photon_flights_per_s", "roofline", "roofline_tally", "e2e")}
+            del wc
     clocks = sampler.stop()
-    t_ms = sum(a.elapsed_time(b) for a, b in ev)
-    if dist:
-        tt = torch.tensor([t_ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        t_ms = float(tt.item())
-        agg = torch.tensor([ch_steps, flights], dtype=torch.float64, device=dev)
-        dist.all_reduce(agg)
-        ch_steps, flights = (float(x) for x in agg.tolist())
-    t_s = t_ms * 1e-3
-    value = world * args.steps * n / t_s
-
-    # ---- roofline of the dominant kernel (electron transport): issue-rate bound
-    peaks, peak_kind = measured_peaks()
-    peak_inst = N_SM * N_SCHED * LANES * peaks.get("sm_max_mhz", 1965.0) * 1e6
-    local_ch = ch_steps / world
-    achieved = ALG_INST_PER_CH_STEP * local_ch / (ms_e * 1e-3) if ms_e > 0 else None
-    roofline = {"bound": "alu", "kernel": "electron transport", "achieved": achieved, "peak": peak_inst,
-                "unit": "thread-inst/s", "frac": (achieved / peak_inst) if achieved else None,
-                "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(w.name) if n == w.n_histories else None,
-                "peak_source": f"148 SMs x 4 x 32 x sm_max_mhz ({peak_kind})",
-                "kernel_ms_per_step": ms_e / args.steps, "kernel_launches_per_step": n_e / args.steps,
-                "kernel_share_of_step": ms_e / t_ms if t_ms else None,
-                "alg_inst_per_ch_step": ALG_INST_PER_CH_STEP}
-
-    # ---- secondary rooflines (BASELINE.json north_star): the tally against the measured fp64 atomic rate of the
-    # L2 (gpumcd_probe_tally: the same grid, the field's footprint, nothing but atomic adds), and the DRAM traffic
-    # of the ncu capture against the measured HBM copy bandwidth
-    tally_peak = g.gpumcd_probe_tally(ctx, 200_000_000)
-    tally_rate = local_ch / t_s
-    tally = {"bound": "l2_atomic", "achieved": tally_rate, "peak": tally_peak, "unit": "fp64 atomic adds/s",
-             "frac": tally_rate / tally_peak, "what": "one add per condensed-history step against gpumcd_probe_tally"}
-    hbm = None
-    if roofline["traffic"] and ms_e > 0:
-        gbs = roofline["traffic"] / (ms_e / max(n_e, 1) * 1e-3) / 1e9
-        hbm = {"bound": "hbm", "achieved": gbs, "peak": peaks.get("hbm_gbs"), "unit": "GB/s",
-               "frac": gbs / peaks.get("hbm_gbs"), "what": f"ncu DRAM bytes per launch / kernel time ({peak_kind} copy bandwidth)"}
-
-    # ---- end to end through the host entry points: every step copies that step's inputs (the phantom volumes,
-    # from pinned host memory) to the device and the resulting dose grid back to the host
-    e2e = None
-    if not args.no_e2e:
-        rho_h = torch.from_numpy(w.density).pin_memory()
-        mat_h = torch.from_numpy(w.material).pin_memory()
-        dose_h = torch.empty(rho.shape, dtype=torch.float32).pin_memory()
-        rho_np, mat_np, dose_np = rho_h.numpy(), mat_h.numpy(), dose_h.numpy()
-
-        def e2e_step(seed):
-            g.gpumcd_set_phantom_host(ctx, rho_np, mat_np)
-            g.gpumcd_set_source(ctx, w.source)
-            g.gpumcd_run_host(ctx, n, seed, dose_np)          # returns after the device-to-host copy
-
-        g.gpumcd_set_profiling(ctx, False)
-        for k in range(args.warmup):
-            e2e_step(w.seed + 300 + k)
-        if dist:
-            dist.barrier()
-        torch.cuda.synchronize()
-        t0 = time.perf_counter()
-        for k in range(args.steps):
-            e2e_step(w.seed + 400 + k)
-        torch.cuda.synchronize()
-        e2e_t = (time.perf_counter() - t0) / args.steps
-        if dist:
-            tt = torch.tensor([e2e_t], dtype=torch.float64, device=dev)
-            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-            e2e_t = float(tt.item())
-        blob_bytes = 4 * (w.tables.photon.size + w.tables.electron.size + w.tables.ms_a.size + 2 * w.tables.n_energy)
-        e2e = {"value": world * n / e2e_t, "unit": "histories/s",
-               "h2d_bytes_per_step": int(rho.numel() * 5 + blob_bytes), "d2h_bytes_per_step": int(rho.numel() * 4),
-               "ms_per_step": e2e_t * 1e3,
-               "what": "gpumcd_set_phantom_host + gpumcd_set_source + gpumcd_run_host per step, wall clock, pinned host buffers"}
-
-    g.gpumcd_destroy(ctx)
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
@@ -467,16 +565,21 @@ def main():
                "sample": f"first {ns} histories of {w.name}, OpenMP over all host cores, {dt:.1f} s"}
 
     if rank == 0:
+        o = head["options"]
         line = {
-            "metric": "coupled photon-electron histories/s", "value": value, "unit": "histories/s",
-            "ch_steps_per_s": ch_steps / t_s, "photon_flights_per_s": flights / t_s,
-            "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": t_ms / args.steps,
+            "metric": "coupled photon-electron histories/s", "value": head["value"], "unit": "histories/s",
+            "ch_steps_per_s": head["ch_steps_per_s"], "photon_flights_per_s": head["photon_flights_per_s"],
+            "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": head["ms_per_step"],
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": {"workload": w.name, "histories_per_step_per_gpu": n, "scheduler": int(opt.scheduler), "hom_tol": float(opt.hom_tol),
-                       "wave_size": int(opt.wave_size), "l2": "flushed between timed steps (512 MiB write)",
-                       "tally": "fp64 atomics", "parallelism": f"histories x{world}"},
-            "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "roofline_tally": tally,
-            "roofline_hbm": hbm, "cpu_baseline": cpu, "wall_s_timed_region": wall,
+            "config": {"workload": w.name, "histories_per_step_per_gpu": n, "scheduler": o["scheduler"], "hom_tol": o["hom_tol"],
+                       "wave_size": o["wave_size"], "cta_threads": o["cta_threads"],
+                       "l2": "flushed between timed steps (512 MiB write)",
+                       "tally": {0: "fp64 atomics", 1: "warp-aggregated fp64 atomics", 2: "64-bit fixed-point atomics"}[o["tally_mode"]],
+                       "parallelism": f"histories x{world}"},
+            "clocks": clocks, "e2e": head["e2e"], "gpu_launches": head["gpu_launches"], "roofline": head["roofline"],
+            "roofline_tally": head.get("roofline_tally"), "roofline_hbm": head["roofline_hbm"], "cpu_baseline": cpu,
+            "wall_s_timed_region": head["wall_s_timed_region"], "bank_high_water": head["bank_high_water"],
+            "per_config": per_config or None,
         }
         print(json.dumps(line))
     if dist:

@@ -86,9 +86,12 @@ typedef struct {
                               0: the paper's scheme (L166): one launch per pass, one thread per
                               particle, the host reads the queue counts between passes            */
     uint32_t warp_stack;   /* scheduler 1: capacity of a warp's electron stack and of its photon
-                              stack, records; default 1024, at least 192 (a warp changes particle
-                              type before a stack fills up, so small stacks cost speed, not
-                              correctness)                                                         */
+                              stack, records; default 1024, at least 256.  A warp changes particle
+                              type before the other type's stack fills up, which keeps the stacks
+                              short (a few hundred records on the five configurations), but a
+                              history that breeds more secondaries than a stack holds overflows it:
+                              that is reported (GPUMCD_ERR_BANK_OVERFLOW from gpumcd_run_host and
+                              gpumcd_get_counters, overflow_count), never silently dropped        */
     uint32_t cta_threads;  /* scheduler 1: threads of the persistent kernel's one CTA per SM: 0 or 512
                               (default; 128 registers per thread, short drain phase) or 1024 (64
                               registers, twice the warps; slower on every workload measured, kept
@@ -103,6 +106,28 @@ typedef struct {
                               the path of its two hinge legs (every voxel's path-length share in
                               expectation).  e_s-max then bounds the step in uniform regions:
                               2-2.5 x fewer steps at 0.25 cm voxels                                 */
+    int32_t tally_mode;    /* how deposits are added to the energy grid (the paper only says the dose arrays
+                              "are summed", L188):
+                              0 (default): one fp64 atomic add per deposit, resolved in L2;
+                              1: warp-aggregated: lanes of a warp that deposit in the same voxel at the same
+                                 time add up first (fp64, lane order) and issue one atomic;
+                              2: 64-bit fixed point: every deposit is rounded to a multiple of 2^-k MeV (k chosen
+                                 per run so that the grid cannot overflow, 31 for 1e8 histories of 20 MeV, at
+                                 most 40; exact for deposits >= 2^(24-k) MeV) and added as an integer: the result
+                                 does not depend on the order of the additions, so the same (seed, n_histories)
+                                 gives the same dose bit for bit, on either scheduler.
+                              Modes 1 and 2 need cta_threads 0 or 512.                                 */
+    int32_t table_memory;  /* scheduler 1: 0 (default) = the table blob is staged into shared memory by TMA
+                              bulk copies when it fits (up to ~220 KB: 7 materials at 1024 nodes), else read
+                              from global memory; 1 = always read from global memory (test hook)      */
+    uint32_t bank_high_g;  /* scheduler 1, tuning (0 = the library's choice: 80 at 512 threads, 512 at 1024): a
+                              warp stepping electrons changes to photons once this many photons are banked
+                              and fewer than bank_high_e electrons are left                             */
+    uint32_t bank_high_e;  /* scheduler 1, tuning (0 = 160 at 512 threads, 512 at 1024): the same for a warp
+                              flying photons.  Together they are the paper's compaction interval N (L180):
+                              how much work of one type is done before the other type is picked up      */
+    uint32_t bank_low;     /* scheduler 1, tuning (0 = 24, at most 64): once the source is exhausted a warp with
+                              fewer ready particles of its type than this changes to the other type      */
 } gpumcd_options;
 
 typedef struct {
@@ -159,7 +184,8 @@ int gpumcd_set_source(gpumcd_ctx *ctx, const gpumcd_source *src);
  * the dose grid.  dose_out_dev: caller-owned float[nx*ny*nz] on the device, OVERWRITTEN.
  * cuda_stream: a cudaStream_t (NULL = default stream); all work is enqueued on it.  With
  * scheduler 1 the call returns without waiting for the device; with scheduler 0 it waits between
- * passes.  Errors detected on the device (queue overflow) are reported by gpumcd_get_counters. */
+ * passes.  Errors detected on the device (queue overflow) are reported by gpumcd_get_counters (and by
+ * gpumcd_run_host, which waits for the run anyway). */
 int gpumcd_run(gpumcd_ctx *ctx, uint64_t n_histories, uint64_t seed, float *dose_out_dev,
                void *cuda_stream);
 
@@ -220,6 +246,13 @@ int gpumcd_get_profile(gpumcd_ctx *ctx, gpumcd_profile *host_out); /* waits for 
  * (no vendor figure exists for the L2's fp64 atomic rate).  Synchronous on cuda_stream; the energy tally
  * of the last run is overwritten (zeroed afterwards); needs a source. */
 int gpumcd_probe_tally(gpumcd_ctx *ctx, uint64_t n_updates, double *updates_per_second, void *cuda_stream);
+
+/* Device-side self-test of the random-number layer: for i < n, out_dev[4i..4i+3] =
+ * Philox4x32-10(counter = ctr_key_dev[6i..6i+3], key = ctr_key_dev[6i+4], ctr_key_dev[6i+5]) as the transport
+ * kernels compute it, and (uniform_dev != NULL) uniform_dev[4i..] = U(word) = ((word >> 9) + 1/2) 2^-23 as they
+ * turn words into uniforms.  All pointers are DEVICE pointers; asynchronous on cuda_stream. */
+int gpumcd_selftest_philox(const uint32_t *ctr_key_dev, uint32_t *out_dev, float *uniform_dev, uint64_t n,
+                           void *cuda_stream);
 
 /* Library-owned, NUL-terminated description of the last error on this context (or of the last
  * failed create when ctx == NULL); valid until the next call on the same context. */

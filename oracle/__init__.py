@@ -118,6 +118,14 @@ def philox(ctr, key):
     return [int(x) for x in o]
 
 
+def philox_batch(ctr_key: np.ndarray) -> np.ndarray:
+    """ctr_key: uint32 [n, 6] = counter (4 words) and key (2 words) per row; returns the blocks, uint32 [n, 4]."""
+    a = np.ascontiguousarray(ctr_key, np.uint32)
+    out = np.zeros((a.shape[0], 4), np.uint32)
+    lib().orc_philox_batch(_p(a), _p(out), C.c_int64(a.shape[0]))
+    return out
+
+
 def uniform(w: int) -> float:
     return lib().orc_uniform(int(w) & 0xFFFFFFFF)
 

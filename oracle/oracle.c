@@ -42,6 +42,12 @@ void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t ou
     out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
 }
 
+/* n blocks at once (test helper): in[6i..6i+3] = counter, in[6i+4], in[6i+5] = key; out[4i..4i+3] */
+void orc_philox_batch(const uint32_t *in, uint32_t *out, int64_t n)
+{
+    for (int64_t i = 0; i < n; ++i) orc_philox4x32_10(in + 6 * i, in + 6 * i + 4, out + 4 * i);
+}
+
 /* U(w) = ((w >> 9) + 1/2) 2^-23, in (0,1): Eq. 1 needs zeta in (0,1].
  * 23 bits plus the half: exactly representable in fp32's 24-bit significand, so a
  * single-precision implementation sees the same value.  The low 9 bits of w are unused. */

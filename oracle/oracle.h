@@ -90,6 +90,7 @@ typedef struct {
 
 /* ---- random numbers ---- */
 void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]);
+void orc_philox_batch(const uint32_t *in, uint32_t *out, int64_t n);
 double orc_uniform(uint32_t w);
 
 /* ---- tables ---- */

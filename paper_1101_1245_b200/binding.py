@@ -27,6 +27,7 @@ EXPORTS = ("gpumcd_default_options", "gpumcd_create", "gpumcd_create_host", "gpu
            "gpumcd_set_phantom_host", "gpumcd_set_source", "gpumcd_run",
            "gpumcd_run_host", "gpumcd_run_uncertainty", "gpumcd_run_trace", "gpumcd_get_counters", "gpumcd_get_energy_tally",
            "gpumcd_set_history_offset", "gpumcd_set_profiling", "gpumcd_get_profile", "gpumcd_probe_tally",
+           "gpumcd_selftest_philox",
            "gpumcd_last_error", "gpumcd_destroy")
 
 
@@ -40,7 +41,9 @@ class gpumcd_options(C.Structure):
     _fields_ = [("es_max_cm", C.c_float), ("f_eloss_max", C.c_float), ("boundary_nudge", C.c_float),
                 ("pair_mode", C.c_int32), ("photon_only", C.c_int32), ("majorant_scale", C.c_float),
                 ("wave_size", C.c_uint32), ("bank_factor", C.c_uint32), ("scheduler", C.c_int32),
-                ("warp_stack", C.c_uint32), ("cta_threads", C.c_uint32), ("hom_tol", C.c_float)]
+                ("warp_stack", C.c_uint32), ("cta_threads", C.c_uint32), ("hom_tol", C.c_float),
+                ("tally_mode", C.c_int32), ("table_memory", C.c_int32), ("bank_high_g", C.c_uint32),
+                ("bank_high_e", C.c_uint32), ("bank_low", C.c_uint32)]
 
 
 class gpumcd_source(C.Structure):
@@ -104,6 +107,7 @@ def load_library():
         lib.gpumcd_set_profiling.argtypes = [vp, C.c_int]
         lib.gpumcd_get_profile.argtypes = [vp, C.POINTER(gpumcd_profile)]
         lib.gpumcd_probe_tally.argtypes = [vp, C.c_uint64, C.POINTER(C.c_double), vp]
+        lib.gpumcd_selftest_philox.argtypes = [vp, vp, vp, C.c_uint64, vp]
         lib.gpumcd_last_error.argtypes = [vp]
         lib.gpumcd_last_error.restype = C.c_char_p
         lib.gpumcd_destroy.argtypes = [vp]
@@ -299,6 +303,19 @@ def gpumcd_probe_tally(ctx: Context, n_updates: int, stream=None) -> float:
     r = C.c_double(0.0)
     ctx._check(load_library().gpumcd_probe_tally(ctx._h, int(n_updates), C.byref(r), _stream_ptr(stream)))
     return r.value
+
+
+def gpumcd_selftest_philox(ctr_key_dev, out_dev, uniform_dev=None, stream=None) -> None:
+    """ctr_key_dev: torch int32 CUDA tensor [n, 6] (bit patterns of the uint32 counter and key words); out_dev: int32
+    [n, 4]; uniform_dev: float32 [n, 4] or None (include/gpumcd.h)."""
+    n = ctr_key_dev.shape[0]
+    for t, cols in ((ctr_key_dev, 6), (out_dev, 4)) + (((uniform_dev, 4),) if uniform_dev is not None else ()):
+        assert t.is_cuda and t.is_contiguous() and t.element_size() == 4 and tuple(t.shape) == (n, cols)
+    rc = load_library().gpumcd_selftest_philox(C.c_void_p(ctr_key_dev.data_ptr()), C.c_void_p(out_dev.data_ptr()),
+                                               C.c_void_p(uniform_dev.data_ptr()) if uniform_dev is not None else None,
+                                               int(n), _stream_ptr(stream))
+    if rc != GPUMCD_OK:
+        raise GpumcdError(rc, "gpumcd_selftest_philox failed")
 
 
 def gpumcd_last_error(ctx: Optional[Context]) -> str:

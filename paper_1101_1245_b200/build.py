@@ -41,9 +41,6 @@ def build(force: bool = False, verbose: bool = False) -> str:
             cmd.insert(1, "--use_fast_math")
         if verbose:
             cmd.insert(1, "-Xptxas=-v")
-        extra = os.environ.get("GPUMCD_NVCC_FLAGS", "")      # experiments only, e.g. -DGPUMCD_PTHREADS=768
-        if extra:
-            cmd[1:1] = extra.split()
         subprocess.run(cmd, check=True)
     return LIB
 

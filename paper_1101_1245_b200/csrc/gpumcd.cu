@@ -6,6 +6,8 @@
 
 #include <algorithm>
 #include <cmath>
+#include <map>
+#include <mutex>
 #include <cstdio>
 #include <cstring>
 #include <string>
@@ -74,6 +76,7 @@ __global__ void k_uniform_radius(float2 *__restrict__ phantom, int nx, int ny, i
 }
 
 // H0: one primary per history from block (hist, track 0, ctr 0); transport starts at ctr 1.
+template <class V>
 __global__ void k_source(Params P, SourceDev S, Queue q, unsigned long long hist0, unsigned n)
 {
     const unsigned i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -84,7 +87,7 @@ __global__ void k_source(Params P, SourceDev S, Queue q, unsigned long long hist
         e_inc = static_cast<double>(p.E);
         if (S.particle == 1 && !electron_tracked(P, p.E)) {
             // an electron below the cutoff (or photon_only): deposited where it is born
-            deposit(P, voxel_index(P.geo, p), p.E);
+            deposit<V>(P, voxel_index(P.geo, p), p.E);
             acc.cut(p.E);
             p.E = -1.0f; // marks an empty record
         }
@@ -99,7 +102,7 @@ __global__ void k_source(Params P, SourceDev S, Queue q, unsigned long long hist
 // Scheduler 0: one launch per pass, one thread per particle, run to completion
 // (the paper's base scheme, L166: alternate the two particle types until both lists are empty)
 // ---------------------------------------------------------------------------------------------
-template <bool TRACE>
+template <class V>
 __global__ void __launch_bounds__(kBlock) k_photon_pass(Params P, Queue in, unsigned n_in, Queue qE, Queue qG)
 {
     const unsigned i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -107,12 +110,12 @@ __global__ void __launch_bounds__(kBlock) k_photon_pass(Params P, Queue in, unsi
     if (i < n_in) {
         uint32_t extra;
         const Particle p = load_rec(in.A, in.B, in.C, i, extra);
-        if (p.E >= 0.0f) photon_run<TRACE>(P, p, L, qE, qG);
+        if (p.E >= 0.0f) photon_run<V>(P, p, L, qE, qG);
     }
     flush(P, L);
 }
 
-template <bool MULTI>
+template <class V>
 __global__ void __launch_bounds__(kBlock) k_electron_pass(Params P, Queue in, unsigned n_in, Queue qE, Queue qG)
 {
     const unsigned i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -120,20 +123,23 @@ __global__ void __launch_bounds__(kBlock) k_electron_pass(Params P, Queue in, un
     if (i < n_in) {
         uint32_t extra;
         const Particle p = load_rec(in.A, in.B, in.C, i, extra);
-        if (p.E >= 0.0f) electron_run<MULTI>(P, p, L, qE, qG);
+        if (p.E >= 0.0f) electron_run<V>(P, p, L, qE, qG);
     }
     flush(P, L);
 }
 
 // H8: dose = energy / mass / histories; also the total deposited energy
-__global__ void k_finalize(const double *__restrict__ edep, const float2 *__restrict__ phantom, size_t nvox,
-                           double inv_h3_n, float *__restrict__ dose, DevCounters *cnt)
+template <int TALLY>
+__global__ void k_finalize(Params P, size_t nvox, double inv_h3_n, float *__restrict__ dose)
 {
+    const float2 *__restrict__ phantom = P.geo.phantom;
+    DevCounters *cnt = P.cnt;
     double s = 0.0;
     for (size_t i = blockIdx.x * static_cast<size_t>(blockDim.x) + threadIdx.x; i < nvox;
          i += static_cast<size_t>(gridDim.x) * blockDim.x) {
-        const double e = edep[i];
+        const double e = tally_value<TALLY>(P, i);
         s += e;
+        if (TALLY == TALLY_FIXED) P.edep[i] = e; // from here on the tally holds MeV as fp64
         if (dose) dose[i] = static_cast<float>(e / static_cast<double>(phantom[i].x) * inv_h3_n);
     }
     s = wsum(s);
@@ -186,6 +192,7 @@ __global__ void k_finalize_uncertainty(const double *__restrict__ s1, const doub
 // the fp64 atomic rate of the L2): every thread adds `per_thread` values into the context's own energy grid
 // at pseudo-random voxels of the beam-shaped region x in [x0, x0+wx), y in [y0, y0+wy), all depths, the
 // address pattern of the condensed-history deposits, and nothing else.
+template <bool FIXED>
 __global__ void k_tally_probe(double *__restrict__ edep, int nx, int ny, int nz, int x0, int y0, int wx, int wy,
                               unsigned per_thread, unsigned seed)
 {
@@ -199,7 +206,22 @@ __global__ void k_tally_probe(double *__restrict__ edep, int nx, int ny, int nz,
         const unsigned ix = x0 + __umulhi(r.x, static_cast<unsigned>(wx));
         const unsigned iy = y0 + __umulhi(r.y, static_cast<unsigned>(wy));
         const unsigned iz = __umulhi(r.z, static_cast<unsigned>(nz));
-        atomicAdd(&edep[ix + static_cast<size_t>(nx) * (iy + static_cast<size_t>(ny) * iz)], 1.0);
+        const size_t lin = ix + static_cast<size_t>(nx) * (iy + static_cast<size_t>(ny) * iz);
+        if (FIXED) atomicAdd(reinterpret_cast<unsigned long long *>(edep) + lin, 1ull);
+        else atomicAdd(&edep[lin], 1.0);
+    }
+}
+
+// Device-side check of the random-number layer (gpumcd_selftest_philox): block i = Philox4x32-10 of counter
+// in[6i .. 6i+3] under key in[6i+4], in[6i+5], and the uniforms the transport code makes of its four words.
+__global__ void k_philox_selftest(const uint32_t *__restrict__ in, uint32_t *__restrict__ out, float *__restrict__ u,
+                                  unsigned long long n)
+{
+    for (unsigned long long i = blockIdx.x * static_cast<unsigned long long>(blockDim.x) + threadIdx.x; i < n;
+         i += static_cast<unsigned long long>(gridDim.x) * blockDim.x) {
+        const uint4 r = philox4x32_10(in[6 * i], in[6 * i + 1], in[6 * i + 2], in[6 * i + 3], in[6 * i + 4], in[6 * i + 5]);
+        out[4 * i] = r.x; out[4 * i + 1] = r.y; out[4 * i + 2] = r.z; out[4 * i + 3] = r.w;
+        if (u) { u[4 * i] = u01(r.x); u[4 * i + 1] = u01(r.y); u[4 * i + 2] = u01(r.z); u[4 * i + 3] = u01(r.w); }
     }
 }
 
@@ -257,6 +279,7 @@ struct gpumcd_ctx {
     unsigned long long high_water = 0;
     bool ran = false;
     unsigned long long hist_offset = 0;
+    float fx_scale = 1.0f;          // tally_mode 2: MeV -> integer units of the current run
     // launch accounting / optional event timing
     bool profiling = false;
     gpumcd_profile prof{};
@@ -320,6 +343,11 @@ extern "C" int gpumcd_default_options(gpumcd_options *opt)
     opt->warp_stack = 1024;
     opt->cta_threads = 0;
     opt->hom_tol = 0.0f;
+    opt->tally_mode = 0;
+    opt->table_memory = 0;
+    opt->bank_high_g = 0;
+    opt->bank_high_e = 0;
+    opt->bank_low = 0;
     return GPUMCD_OK;
 }
 
@@ -343,6 +371,44 @@ static void destroy_impl(gpumcd_ctx *c)
     cudaFree(c->stkA); cudaFree(c->stkB); cudaFree(c->stkC);
     for (auto &e : c->events) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
     delete c;
+}
+
+// The persistent kernel's variants: (trace | multi-voxel steps x tally mode) x tables in shared / global memory
+// x CTA size.  1024 threads per CTA exist for the fp64 tally only (the ablation of DESIGN.md 7).
+template <class V>
+static const void *persistent_variant(bool smem, int threads)
+{
+    if (threads == 512) return smem ? (const void *)k_persistent<V, true, 512> : (const void *)k_persistent<V, false, 512>;
+    if (V::TALLY == TALLY_F64) return smem ? (const void *)k_persistent<Variant<V::TRACE, V::MULTI, TALLY_F64>, true, 1024>
+                                           : (const void *)k_persistent<Variant<V::TRACE, V::MULTI, TALLY_F64>, false, 1024>;
+    return nullptr;
+}
+static const void *persistent_kernel(bool trace, bool multi, int tally, bool smem, int threads)
+{
+    if (trace) return persistent_variant<Variant<true, false, TALLY_F64>>(smem, threads); // a trace run tallies nothing of interest
+    if (multi) {
+        if (tally == TALLY_WARP) return persistent_variant<Variant<false, true, TALLY_WARP>>(smem, threads);
+        if (tally == TALLY_FIXED) return persistent_variant<Variant<false, true, TALLY_FIXED>>(smem, threads);
+        return persistent_variant<Variant<false, true, TALLY_F64>>(smem, threads);
+    }
+    if (tally == TALLY_WARP) return persistent_variant<Variant<false, false, TALLY_WARP>>(smem, threads);
+    if (tally == TALLY_FIXED) return persistent_variant<Variant<false, false, TALLY_FIXED>>(smem, threads);
+    return persistent_variant<Variant<false, false, TALLY_F64>>(smem, threads);
+}
+
+// cudaFuncAttributeMaxDynamicSharedMemorySize belongs to the kernel function, not to a context: it is only
+// ever raised, so that contexts with table blobs of different sizes can be alive at the same time.
+static int allow_dynamic_smem(gpumcd_ctx *ctx, const void *fn, size_t bytes)
+{
+    static std::mutex mu;
+    static std::map<const void *, size_t> allowed;
+    std::lock_guard<std::mutex> lock(mu);
+    size_t &cur = allowed[fn];
+    if (bytes > cur) {
+        CK(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(bytes)));
+        cur = bytes;
+    }
+    return GPUMCD_OK;
 }
 
 // Phantom -> device: pack {density, material}, validate, reduce rho_max per material, rebuild the
@@ -424,6 +490,8 @@ static int create_impl(gpumcd_ctx **out, const float *density, const uint8_t *ma
     if (!(opt.es_max_cm > 0.f) || !(opt.f_eloss_max > 0.f) || opt.f_eloss_max > 1.f || opt.boundary_nudge < 0.f ||
         !(opt.majorant_scale >= 1.f) || opt.wave_size == 0 || opt.bank_factor == 0 || opt.warp_stack > (1u << 20) ||
         (opt.cta_threads != 0 && opt.cta_threads != 512 && opt.cta_threads != 1024) || !(opt.hom_tol >= 0.f) ||
+        opt.tally_mode < 0 || opt.tally_mode > 2 || (opt.tally_mode != 0 && opt.cta_threads == 1024) ||
+        opt.table_memory < 0 || opt.table_memory > 1 || opt.bank_low > 64 ||
         static_cast<unsigned long long>(opt.wave_size) * opt.bank_factor > 0x7fffffffull) {
         set_error(nullptr, "bad options");
         return GPUMCD_ERR_INVALID_ARG;
@@ -489,28 +557,21 @@ static int create_impl(gpumcd_ctx **out, const float *density, const uint8_t *ma
         CK(cudaDeviceGetAttribute(&max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
         if (!coop) { set_error(ctx, "device does not support cooperative launches (scheduler 1)"); return GPUMCD_ERR_CUDA; }
         const size_t table_bytes = static_cast<size_t>(ctx->table_floats) * sizeof(float);
+        const int threads = opt.cta_threads == 1024 ? 1024 : 512;
+        const void *fn = persistent_kernel(false, opt.hom_tol > 0.f, opt.tally_mode, true, threads);
         cudaFuncAttributes fa{};
-        CK(cudaFuncGetAttributes(&fa, k_persistent<false, true, 1024, false>));
-        ctx->smem_tables = table_bytes + fa.sharedSizeBytes + 1024 <= static_cast<size_t>(max_smem);
+        CK(cudaFuncGetAttributes(&fa, fn));
+        ctx->smem_tables = opt.table_memory == 0 && table_bytes + fa.sharedSizeBytes + 1024 <= static_cast<size_t>(max_smem);
         const size_t dyn = ctx->smem_tables ? table_bytes : 0;
-        if (ctx->smem_tables) {
-            CK(cudaFuncSetAttribute(k_persistent<false, true, 512, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(dyn)));
-            CK(cudaFuncSetAttribute(k_persistent<true, true, 512, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(dyn)));
-            CK(cudaFuncSetAttribute(k_persistent<false, true, 1024, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(dyn)));
-            CK(cudaFuncSetAttribute(k_persistent<true, true, 1024, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(dyn)));
-            CK(cudaFuncSetAttribute(k_persistent<false, true, 512, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(dyn)));
-            CK(cudaFuncSetAttribute(k_persistent<false, true, 1024, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(dyn)));
-        }
+        fn = persistent_kernel(false, opt.hom_tol > 0.f, opt.tally_mode, ctx->smem_tables, threads);
+        { const int rc = allow_dynamic_smem(ctx, fn, dyn); if (rc != GPUMCD_OK) return rc; }
         int per_sm = 0;
-        if (ctx->smem_tables)
-            CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_persistent<false, true, 1024, false>, 1024, dyn));
-        else
-            CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_persistent<false, false, 1024, false>, 1024, 0));
+        CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, threads, dyn));
         if (per_sm < 1) { set_error(ctx, "persistent kernel does not fit on an SM"); return GPUMCD_ERR_CUDA; }
         ctx->p_grid = n_sm; // one CTA per SM
-        ctx->cap_r = std::max(opt.warp_stack, kMustMargin + 32u);
+        ctx->cap_r = std::max(opt.warp_stack, kMinStack);
         ctx->stride = 2 * ctx->cap_r + 3 * kPend;
-        const size_t n_warps = static_cast<size_t>(ctx->p_grid) * (kPThreadsMax / 32);
+        const size_t n_warps = static_cast<size_t>(ctx->p_grid) * (threads / 32); // of the CTA size actually used
         const size_t recs = n_warps * ctx->stride;
         CK(cudaMalloc(&ctx->stkA, recs * sizeof(float4)));
         CK(cudaMalloc(&ctx->stkB, recs * sizeof(float4)));
@@ -604,6 +665,7 @@ extern "C" int gpumcd_set_source(gpumcd_ctx *ctx, const gpumcd_source *s)
 static Params make_params(gpumcd_ctx *ctx, uint64_t seed, uint32_t hist_hi, bool photon_only, unsigned long long *trace)
 {
     Params P;
+    P.fx_scale = ctx->fx_scale;
     P.tab = ctx->tab;
     P.geo.phantom = ctx->phantom;
     P.geo.nx = ctx->nx; P.geo.ny = ctx->ny; P.geo.nz = ctx->nz;
@@ -624,6 +686,14 @@ static Params make_params(gpumcd_ctx *ctx, uint64_t seed, uint32_t hist_hi, bool
     return P;
 }
 
+// run `call` with TL bound to the context's tally mode as a compile-time constant
+#define WITH_TALLY(mode, call)                                                  \
+    do {                                                                        \
+        if ((mode) == TALLY_WARP) { constexpr int TL = TALLY_WARP; call; }      \
+        else if ((mode) == TALLY_FIXED) { constexpr int TL = TALLY_FIXED; call; } \
+        else { constexpr int TL = TALLY_F64; call; }                            \
+    } while (0)
+
 // Scheduler 0: per wave, fill the source list, then alternate photon and electron
 // passes until both lists are empty; the host reads the list lengths between passes.
 static int run_waves_host_loop(gpumcd_ctx *ctx, uint64_t h_begin, uint64_t n_hist, uint64_t seed, bool trace_mode,
@@ -640,8 +710,8 @@ static int run_waves_host_loop(gpumcd_ctx *ctx, uint64_t h_begin, uint64_t n_his
         CK(cudaMemsetAsync(ctx->qcount, 0, 4 * sizeof(unsigned), st));
         const int src_q = ctx->src.particle == 0 ? pcur : ecur;
         { LaunchScope ls(ctx, st, CLS_SOURCE);
-        k_source<<<static_cast<unsigned>((n + kBlock - 1) / kBlock), kBlock, 0, st>>>(P, ctx->src, make_queue(ctx, src_q), h0,
-                                                                                      static_cast<unsigned>(n)); }
+        WITH_TALLY(ctx->opt.tally_mode, (k_source<Variant<false, false, TL>><<<static_cast<unsigned>((n + kBlock - 1) / kBlock), kBlock, 0, st>>>(
+                                            P, ctx->src, make_queue(ctx, src_q), h0, static_cast<unsigned>(n)))); }
         CK(cudaGetLastError());
         unsigned cnt[4];
         for (;;) {
@@ -658,9 +728,10 @@ static int run_waves_host_loop(gpumcd_ctx *ctx, uint64_t h_begin, uint64_t n_his
                 // appended to the current electron list (not being consumed now)
                 { LaunchScope ls(ctx, st, CLS_PHOTON);
                 if (trace_mode)
-                    k_photon_pass<true><<<(m + kBlock - 1) / kBlock, kBlock, 0, st>>>(P, make_queue(ctx, pcur), m, make_queue(ctx, ecur), make_queue(ctx, pnext));
+                    k_photon_pass<Variant<true, false, TALLY_F64>><<<(m + kBlock - 1) / kBlock, kBlock, 0, st>>>(P, make_queue(ctx, pcur), m, make_queue(ctx, ecur), make_queue(ctx, pnext));
                 else
-                    k_photon_pass<false><<<(m + kBlock - 1) / kBlock, kBlock, 0, st>>>(P, make_queue(ctx, pcur), m, make_queue(ctx, ecur), make_queue(ctx, pnext)); }
+                    WITH_TALLY(ctx->opt.tally_mode, (k_photon_pass<Variant<false, false, TL>><<<(m + kBlock - 1) / kBlock, kBlock, 0, st>>>(
+                                                        P, make_queue(ctx, pcur), m, make_queue(ctx, ecur), make_queue(ctx, pnext)))); }
                 CK(cudaGetLastError());
                 CK(cudaMemsetAsync(ctx->qcount + pcur, 0, sizeof(unsigned), st));
                 std::swap(pcur, pnext);
@@ -668,9 +739,11 @@ static int run_waves_host_loop(gpumcd_ctx *ctx, uint64_t h_begin, uint64_t n_his
                 const unsigned m = cnt[ecur];
                 { LaunchScope ls(ctx, st, CLS_ELECTRON);
                 if (ctx->opt.hom_tol > 0.f)
-                    k_electron_pass<true><<<(m + kBlock - 1) / kBlock, kBlock, 0, st>>>(P, make_queue(ctx, ecur), m, make_queue(ctx, enext), make_queue(ctx, pcur));
+                    WITH_TALLY(ctx->opt.tally_mode, (k_electron_pass<Variant<false, true, TL>><<<(m + kBlock - 1) / kBlock, kBlock, 0, st>>>(
+                                                        P, make_queue(ctx, ecur), m, make_queue(ctx, enext), make_queue(ctx, pcur))));
                 else
-                    k_electron_pass<false><<<(m + kBlock - 1) / kBlock, kBlock, 0, st>>>(P, make_queue(ctx, ecur), m, make_queue(ctx, enext), make_queue(ctx, pcur)); }
+                    WITH_TALLY(ctx->opt.tally_mode, (k_electron_pass<Variant<false, false, TL>><<<(m + kBlock - 1) / kBlock, kBlock, 0, st>>>(
+                                                        P, make_queue(ctx, ecur), m, make_queue(ctx, enext), make_queue(ctx, pcur)))); }
                 CK(cudaGetLastError());
                 CK(cudaMemsetAsync(ctx->qcount + ecur, 0, sizeof(unsigned), st));
                 std::swap(ecur, enext);
@@ -711,36 +784,17 @@ static int run_persistent(gpumcd_ctx *ctx, uint64_t h_begin, uint64_t n_hist, ui
         // CTA size (see persistent.cuh): 512 threads unless the caller asks for 1024
         const int threads = ctx->opt.cta_threads == 1024 ? 1024 : 512;
         // banked particles of the other type that make a warp change to it: photons are cheap to work off
-        // (few per batch keeps the drain short), electrons are worth a fuller batch
-#ifndef GPUMCD_HG512
-#define GPUMCD_HG512 80u
-#endif
-#ifndef GPUMCD_HE512
-#define GPUMCD_HE512 160u
-#endif
-#ifndef GPUMCD_HG1024
-#define GPUMCD_HG1024 512u
-#endif
-#ifndef GPUMCD_HE1024
-#define GPUMCD_HE1024 512u
-#endif
-        a.high_g = threads == 512 ? GPUMCD_HG512 : GPUMCD_HG1024;
-        a.high_e = threads == 512 ? GPUMCD_HE512 : GPUMCD_HE1024;
+        // (few per batch keeps the drain short), electrons are worth a fuller batch; swept on configs 2-5
+        // (bench.py --ablation): 80 / 160 with 512 threads per SM, 512 / 512 with 1024
+        a.high_g = ctx->opt.bank_high_g ? ctx->opt.bank_high_g : (threads == 512 ? 80u : 512u);
+        a.high_e = ctx->opt.bank_high_e ? ctx->opt.bank_high_e : (threads == 512 ? 160u : 512u);
+        a.low = ctx->opt.bank_low ? ctx->opt.bank_low : kLowDefault;
         void *args[] = {&a};
-        // the kernel variant: trace (photon-only replay) x tables in shared memory x CTA size x multi-voxel steps
+        // the kernel variant: trace (photon-only replay) | multi-voxel steps x tally mode; tables in shared memory; CTA size
         const bool multi = ctx->opt.hom_tol > 0.f && !trace; // a trace run tracks no electrons
-        const void *fn;
-        if (multi) {
-            if (threads == 512) fn = ctx->smem_tables ? (const void *)k_persistent<false, true, 512, true> : (const void *)k_persistent<false, false, 512, true>;
-            else fn = ctx->smem_tables ? (const void *)k_persistent<false, true, 1024, true> : (const void *)k_persistent<false, false, 1024, true>;
-        } else if (threads == 512) {
-            if (ctx->smem_tables) fn = trace ? (const void *)k_persistent<true, true, 512, false> : (const void *)k_persistent<false, true, 512, false>;
-            else fn = trace ? (const void *)k_persistent<true, false, 512, false> : (const void *)k_persistent<false, false, 512, false>;
-        } else {
-            if (ctx->smem_tables) fn = trace ? (const void *)k_persistent<true, true, 1024, false> : (const void *)k_persistent<false, true, 1024, false>;
-            else fn = trace ? (const void *)k_persistent<true, false, 1024, false> : (const void *)k_persistent<false, false, 1024, false>;
-        }
+        const void *fn = persistent_kernel(trace != nullptr, multi, ctx->opt.tally_mode, ctx->smem_tables, threads);
         const size_t dyn = ctx->smem_tables ? static_cast<size_t>(ctx->table_floats) * sizeof(float) : 0;
+        { const int rc = allow_dynamic_smem(ctx, fn, dyn); if (rc != GPUMCD_OK) return rc; }
         { LaunchScope ls(ctx, st, CLS_ELECTRON);
         CK(cudaLaunchCooperativeKernel(fn, dim3(ctx->p_grid), dim3(threads), args, dyn, st)); }
         h0 += n;
@@ -761,6 +815,9 @@ static int begin_run(gpumcd_ctx *ctx, uint64_t n_hist, unsigned long long *trace
     ctx->prof = gpumcd_profile{};
     for (auto &e : ctx->events) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
     ctx->events.clear();
+    // tally_mode 2: the largest power of two (at most 2^40) for which even all the run's energy in one voxel
+    // stays below 2^62 units
+    ctx->fx_scale = std::ldexp(1.0f, std::min(40, std::max(0, 61 - std::ilogb(static_cast<double>(n_hist) * ctx->e_max + 1.0))));
     CK(cudaMemsetAsync(ctx->edep, 0, ctx->nvox * sizeof(double), st));
     CK(cudaMemsetAsync(ctx->cnt, 0, sizeof(DevCounters), st));
     if (trace_dev) CK(cudaMemsetAsync(trace_dev, 0, n_hist * sizeof(unsigned long long), st));
@@ -778,8 +835,10 @@ static int transport(gpumcd_ctx *ctx, uint64_t h_begin, uint64_t n_hist, uint64_
     const double h3 = static_cast<double>(ctx->h) * ctx->h * ctx->h;
     const int grid = static_cast<int>(std::min<size_t>((ctx->nvox + kBlock - 1) / kBlock, 148 * 8));
     { LaunchScope ls(ctx, st, CLS_FINALIZE);
-    k_finalize<<<grid, kBlock, 0, st>>>(ctx->edep, ctx->phantom, ctx->nvox, 1.0 / (h3 * static_cast<double>(n_hist)),
-                                        dose_dev, ctx->cnt); }
+    const Params P = make_params(ctx, seed, 0u, trace_dev != nullptr, trace_dev);
+    const double inv = 1.0 / (h3 * static_cast<double>(n_hist));
+    if (ctx->opt.tally_mode == TALLY_FIXED && !trace_dev) k_finalize<TALLY_FIXED><<<grid, kBlock, 0, st>>>(P, ctx->nvox, inv, dose_dev);
+    else k_finalize<TALLY_F64><<<grid, kBlock, 0, st>>>(P, ctx->nvox, inv, dose_dev); }
     CK(cudaGetLastError());
     return GPUMCD_OK;
 }
@@ -808,8 +867,11 @@ extern "C" int gpumcd_run_host(gpumcd_ctx *ctx, uint64_t n_histories, uint64_t s
     int rc = run_impl(ctx, n_histories, seed, tmp, nullptr, st);
     if (rc == GPUMCD_OK) {
         cudaError_t e = cudaMemcpyAsync(dose_out_host, tmp, ctx->nvox * sizeof(float), cudaMemcpyDeviceToHost, st);
+        unsigned long long dropped = 0;
+        if (e == cudaSuccess) e = cudaMemcpyAsync(&dropped, &ctx->cnt->overflow, sizeof dropped, cudaMemcpyDeviceToHost, st);
         if (e == cudaSuccess) e = cudaStreamSynchronize(st);
         if (e != cudaSuccess) { set_error(ctx, cudaGetErrorString(e)); rc = GPUMCD_ERR_CUDA; }
+        else if (dropped) { set_error(ctx, "particle queue overflow: the result is invalid"); rc = GPUMCD_ERR_BANK_OVERFLOW; }
     }
     return rc;
 }
@@ -940,11 +1002,13 @@ extern "C" int gpumcd_probe_tally(gpumcd_ctx *ctx, uint64_t n_updates, double *u
     CK(cudaEventCreate(&a)); CK(cudaEventCreate(&b));
     CK(cudaMemsetAsync(ctx->edep, 0, ctx->nvox * sizeof(double), st));
     // once untimed (first touch of the grid), once timed
-    k_tally_probe<<<blocks, threads, 0, st>>>(ctx->edep, ctx->nx, ctx->ny, ctx->nz, x0, y0, x1 - x0 + 1, y1 - y0 + 1,
-                                              static_cast<unsigned>(per_thread), 1u);
+    const bool fixed = ctx->opt.tally_mode == TALLY_FIXED; // the probe adds what the run adds: fp64 or 64-bit integers
+    auto probe = fixed ? k_tally_probe<true> : k_tally_probe<false>;
+    probe<<<blocks, threads, 0, st>>>(ctx->edep, ctx->nx, ctx->ny, ctx->nz, x0, y0, x1 - x0 + 1, y1 - y0 + 1,
+                                      static_cast<unsigned>(per_thread), 1u);
     CK(cudaEventRecord(a, st));
-    k_tally_probe<<<blocks, threads, 0, st>>>(ctx->edep, ctx->nx, ctx->ny, ctx->nz, x0, y0, x1 - x0 + 1, y1 - y0 + 1,
-                                              static_cast<unsigned>(per_thread), 2u);
+    probe<<<blocks, threads, 0, st>>>(ctx->edep, ctx->nx, ctx->ny, ctx->nz, x0, y0, x1 - x0 + 1, y1 - y0 + 1,
+                                      static_cast<unsigned>(per_thread), 2u);
     CK(cudaEventRecord(b, st));
     CK(cudaGetLastError());
     CK(cudaEventSynchronize(b));
@@ -954,6 +1018,16 @@ extern "C" int gpumcd_probe_tally(gpumcd_ctx *ctx, uint64_t n_updates, double *u
     CK(cudaMemsetAsync(ctx->edep, 0, ctx->nvox * sizeof(double), st)); // the tally of the last run is gone
     *updates_per_second = static_cast<double>(per_thread) * threads * blocks / (static_cast<double>(ms) * 1e-3);
     return GPUMCD_OK;
+}
+
+extern "C" int gpumcd_selftest_philox(const uint32_t *ctr_key_dev, uint32_t *out_dev, float *uniform_dev, uint64_t n,
+                                      void *cuda_stream)
+{
+    if (!ctr_key_dev || !out_dev) return GPUMCD_ERR_INVALID_ARG;
+    if (n == 0) return GPUMCD_OK;
+    const unsigned blocks = static_cast<unsigned>(std::min<uint64_t>((n + kBlock - 1) / kBlock, 148 * 8));
+    k_philox_selftest<<<blocks, kBlock, 0, static_cast<cudaStream_t>(cuda_stream)>>>(ctr_key_dev, out_dev, uniform_dev, n);
+    return cudaGetLastError() == cudaSuccess ? GPUMCD_OK : GPUMCD_ERR_CUDA;
 }
 
 extern "C" const char *gpumcd_last_error(gpumcd_ctx *ctx)

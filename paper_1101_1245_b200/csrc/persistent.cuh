@@ -29,9 +29,6 @@ namespace gpumcd {
 
 namespace cg = cooperative_groups;
 
-#ifndef GPUMCD_LOW
-#define GPUMCD_LOW 24
-#endif
 // Threads per persistent CTA (one CTA per SM): 512 by default (128 registers per thread, no spills; the
 // per-lane backlog when the source runs dry is half that of 1024 threads).  The 1024-thread build (64
 // registers, spills, twice the warps to hide latency) is kept as an option for the ablation: it was the
@@ -40,8 +37,19 @@ constexpr int kPThreadsMax = 1024;
 constexpr unsigned kFull = 0xffffffffu;
 constexpr unsigned kChunk = 32;            // primaries a warp claims per atomic on the source head
 constexpr unsigned kPend = 64;             // capacity of a waiting stack (EH, GI, GR): < 32 before a move, + 32 after
-constexpr unsigned kLow = GPUMCD_LOW;      // own-type particles below which a warp with no source changes type
-constexpr unsigned kMustMargin = 160;      // a ready stack within this many records of its capacity forces the change
+constexpr unsigned kLowDefault = 24;       // own-type particles below which a warp with no source changes type
+// Forced type changes.  Between two looks at the rules below photon mode banks at most 96 electrons (one Compton
+// batch: 32, one batch of pair events: 64) and electron mode at most 32 photons (one hard-event batch).
+//   photon mode leaves once ES holds cap - kRoomE or more (its interactions could overflow it otherwise);
+//   electron mode leaves once GS holds cap/2 - 32 or more (in photon mode a photon can at most turn into two,
+//     by a pair event, and annihilation photons do not multiply: 2 x cap/2 fits), provided ES + lanes are below
+//     cap - kRoomE, i.e. photon mode will not send the warp straight back (no ping-pong: a forced change is only
+//     made into a mode that can work);
+// if both stacks are that full the warp stays with the electrons, and knock-on electrons pile up on ES without a
+// bound other than the history itself: a push that finds a stack full is counted and reported
+// (GPUMCD_ERR_BANK_OVERFLOW), never dropped silently.
+constexpr unsigned kRoomE = 160;
+constexpr unsigned kMinStack = 256;        // smallest ready stack: cap - kRoomE must exceed low + 32
 
 struct SourceDev {
     int particle, shape;
@@ -133,6 +141,7 @@ struct PersistArgs {
     uint4 *stkC;
     unsigned cap_r;                // capacity of a ready stack (ES, GS)
     unsigned high_g, high_e;       // banked photons / electrons that make a warp change to that type
+    unsigned low;                  // own-type ready particles below which a warp with no source changes type
     unsigned stride;               // 2 cap_r + 3 kPend
     unsigned long long hist0;      // first history of the launch (low word never wraps inside a launch)
     unsigned n_hist;               // histories of the launch (< 2^32)
@@ -177,7 +186,7 @@ struct Warp {
     float4 *B;
     uint4 *C;
     unsigned cap_r;
-    unsigned high_g, high_e;
+    unsigned high_g, high_e, low;
     unsigned n[5];
     unsigned lt;   // lanes below this one
     unsigned hw;   // fullest ready stack seen
@@ -223,6 +232,7 @@ struct Warp {
     // ready stack s (SK_ES for an electron source, SK_GS for photons), from where free lanes pop them like
     // any other ready particle: the source code (H0) then always runs with full lanes.  Returns false if the
     // source is dry or the stack has no room for them right now.
+    template <class V>
     __device__ __forceinline__ bool bank_primaries(const PersistArgs &a, Claim &cl, int s)
     {
         cl.refill(a.head, a.n_hist);
@@ -235,7 +245,7 @@ struct Warp {
             q = make_primary(a.P, a.S, a.hist0 + (cl.next + lane));
             *e_inc += static_cast<double>(q.E);
             if (s == SK_ES && !electron_tracked(a.P, q.E)) { // below the cutoff (or photon_only): deposited where it is born
-                deposit(a.P, voxel_index(a.P.geo, q), q.E);
+                deposit<V>(a.P, voxel_index(a.P.geo, q), q.E);
                 Acc(a.P).cut(q.E);
                 on = false;
             }
@@ -250,7 +260,7 @@ struct Warp {
 // Electron mode: the lanes hold electrons due a condensed-history step.  Returns the type to go on
 // with (0 photons, 1 electrons never, -1 nothing left); on return no lane holds a particle.
 // ---------------------------------------------------------------------------------------------
-template <bool MULTI>
+template <class V>
 __device__ __forceinline__ int electron_mode(const PersistArgs &a, const float *__restrict__ TB, Warp &w, Claim &cl)
 {
     const Params &P = a.P;
@@ -273,7 +283,7 @@ __device__ __forceinline__ int electron_mode(const PersistArgs &a, const float *
                 uint32_t mbits;
                 p = load_rec(w.A, w.B, w.C, w.off(SK_EH) + w.n[SK_EH] - 1u - lane, mbits);
                 lnT = flog(p.E);
-                alive = electron_hard(P, TB, p, lnT, __uint_as_float(mbits), c, kind) == ST_ALIVE;
+                alive = electron_hard<V>(P, TB, p, lnT, __uint_as_float(mbits), c, kind) == ST_ALIVE;
             }
             w.n[SK_EH] -= nb;
             __syncwarp();
@@ -292,15 +302,15 @@ __device__ __forceinline__ int electron_mode(const PersistArgs &a, const float *
         // undone before some work has been done)
         const unsigned ready = static_cast<unsigned>(__popc(live)) + w.n[SK_ES];
         const unsigned E = ready + w.n[SK_EH], G = w.n[SK_GS] + w.n[SK_GI] + w.n[SK_GR];
-        const unsigned must = w.cap_r - kMustMargin;
         const bool src_g = !src_is_e && !cl.empty();
         // (only READY photons count towards the high-water mark: photon mode stays while it has kLow of them,
         // so a change made here is never undone before some work has been done)
         const unsigned Gr = w.n[SK_GS];
-        bool leave = Gr >= w.high_g && (E < w.high_e || (Gr >= must && E < must));
+        // (a change is only made if photon mode will not send the warp straight back: ES + lanes below its forced mark)
+        bool leave = ready + kRoomE < w.cap_r && ((Gr >= w.high_g && E < w.high_e) || Gr + 32u >= w.cap_r / 2u);
         if (!src_e) {
             if (ready == 0u) return (G != 0u || src_g) ? 0 : -1; // (EH is empty here)
-            leave = leave || (ready < kLow && (src_g || w.n[SK_GS] >= 32u));
+            leave = leave || (ready < w.low && (src_g || w.n[SK_GS] >= 32u));
         }
         if (leave) {
             w.push(P, SK_ES, alive, p, 0u);
@@ -311,7 +321,7 @@ __device__ __forceinline__ int electron_mode(const PersistArgs &a, const float *
         if (~live) {
             uint32_t extra;
             bool got = w.pop(SK_ES, !alive, p, extra);
-            if (src_e && __any_sync(kFull, !alive && !got) && w.bank_primaries(a, cl, SK_ES))
+            if (src_e && __any_sync(kFull, !alive && !got) && w.template bank_primaries<V>(a, cl, SK_ES))
                 got = w.pop(SK_ES, !alive && !got, p, extra) || got;
             if (got) {
                 lnT = flog(p.E);
@@ -322,7 +332,7 @@ __device__ __forceinline__ int electron_mode(const PersistArgs &a, const float *
         if (sm == 0u) continue;
         // ---- one condensed-history step for every lane that holds an electron
         int st = ST_ALIVE;
-        if (alive) st = electron_step<MULTI>(P, TB, p, lnT, M);
+        if (alive) st = electron_step<V>(P, TB, p, lnT, M);
         w.count(WC_STEP, sm);
         w.push(P, SK_EH, alive && st == ST_HARD, p, __float_as_uint(M));
         if (st != ST_ALIVE) alive = false;
@@ -331,7 +341,7 @@ __device__ __forceinline__ int electron_mode(const PersistArgs &a, const float *
 
 // Photon mode, interactions of up to 32 photons waiting in stack sk (H2).  KIND != 0: all of them are of
 // that kind (the compiler drops the other branches of photon_interact); else the kind is in the record.
-template <bool TRACE, int KIND>
+template <class V, int KIND>
 __device__ __forceinline__ void interact_batch(const Params &P, Warp &w, int sk, Particle &p, bool &alive)
 {
     const unsigned lane = threadIdx.x & 31;
@@ -354,7 +364,7 @@ __device__ __forceinline__ void interact_batch(const Params &P, Warp &w, int sk,
                            &w.ctl->wc[WC_PUSH_E], w.cap_r};
         const WarpStack qG{w.A + w.off(SK_GS), w.B + w.off(SK_GS), w.C + w.off(SK_GS), &w.ctl->n_gs,
                            &w.ctl->wc[WC_PUSH_G], w.cap_r};
-        alive = photon_interact<TRACE>(P, p, kind, qE, qG) == PM_FLIGHT;
+        alive = photon_interact<V>(P, p, kind, qE, qG) == PM_FLIGHT;
     }
     __syncwarp();
     w.n[SK_ES] = w.ctl->n_es;
@@ -374,7 +384,7 @@ __device__ __forceinline__ void interact_batch(const Params &P, Warp &w, int sk,
 // Photon mode: the lanes hold photons due a flight.  Returns the type to go on with (1 electrons,
 // -1 nothing left); on return no lane holds a particle.
 // ---------------------------------------------------------------------------------------------
-template <bool TRACE>
+template <class V>
 __device__ __forceinline__ int photon_mode(const PersistArgs &a, const float *__restrict__ TB, Warp &w, Claim &cl)
 {
     const Params &P = a.P;
@@ -390,23 +400,22 @@ __device__ __forceinline__ int photon_mode(const PersistArgs &a, const float *__
         // does not drag the long pair code along for one or two lanes
         const bool stuck = live == 0u && w.n[SK_GS] == 0u && !src_g;
         if (w.n[SK_GI] >= 32u || (w.n[SK_GI] != 0u && stuck)) {
-            interact_batch<TRACE, PM_COMPTON>(P, w, SK_GI, p, alive);
+            interact_batch<V, PM_COMPTON>(P, w, SK_GI, p, alive);
             continue;
         }
         if (w.n[SK_GR] >= 32u || (w.n[SK_GR] != 0u && stuck)) {
-            interact_batch<TRACE, 0>(P, w, SK_GR, p, alive);
+            interact_batch<V, 0>(P, w, SK_GR, p, alive);
             continue;
         }
         // ---- change of particle type?  (see electron_mode)
         const unsigned ready = static_cast<unsigned>(__popc(live)) + w.n[SK_GS];
         const unsigned G = ready + w.n[SK_GI] + w.n[SK_GR], E = w.n[SK_ES] + w.n[SK_EH];
-        const unsigned must = w.cap_r - kMustMargin;
         const bool src_e = !src_is_g && !cl.empty();
         const unsigned Er = w.n[SK_ES];
-        bool leave = Er >= w.high_e && (G < w.high_g || Er >= must);
+        bool leave = (Er >= w.high_e && G < w.high_g) || Er + kRoomE >= w.cap_r;
         if (!src_g) {
             if (ready == 0u) return (E != 0u || src_e) ? 1 : -1; // (GI is empty here)
-            leave = leave || (ready < kLow && (src_e || w.n[SK_ES] >= 32u));
+            leave = leave || (ready < w.low && (src_e || w.n[SK_ES] >= 32u));
         }
         if (leave) {
             w.push(P, SK_GS, alive, p, 0u);
@@ -417,7 +426,7 @@ __device__ __forceinline__ int photon_mode(const PersistArgs &a, const float *__
         if (~live) {
             uint32_t extra;
             bool got = w.pop(SK_GS, !alive, p, extra);
-            if (src_g && __any_sync(kFull, !alive && !got) && w.bank_primaries(a, cl, SK_GS))
+            if (src_g && __any_sync(kFull, !alive && !got) && w.template bank_primaries<V>(a, cl, SK_GS))
                 got = w.pop(SK_GS, !alive && !got, p, extra) || got;
             if (got) alive = true;
         }
@@ -425,7 +434,7 @@ __device__ __forceinline__ int photon_mode(const PersistArgs &a, const float *__
         if (fl == 0u) continue;
         // ---- one flight for every lane that holds a photon
         int mode = PM_DEAD;
-        if (alive) mode = photon_flight<TRACE>(P, TB, p);
+        if (alive) mode = photon_flight<V>(P, TB, p);
         w.count(WC_FLIGHT, fl);
         w.count(WC_FICT, __ballot_sync(kFull, mode == PM_FLIGHT));
         w.push(P, SK_GI, mode == PM_COMPTON, p, static_cast<uint32_t>(mode));
@@ -437,7 +446,7 @@ __device__ __forceinline__ int photon_mode(const PersistArgs &a, const float *__
 // ---------------------------------------------------------------------------------------------
 // The persistent kernel
 // ---------------------------------------------------------------------------------------------
-template <bool TRACE, bool SMEM_TABLES, int kPThreads, bool MULTI>
+template <class V, bool SMEM_TABLES, int kPThreads>
 __global__ void __launch_bounds__(kPThreads, 1) k_persistent(const __grid_constant__ PersistArgs a)
 {
     extern __shared__ __align__(128) float smem[];
@@ -462,6 +471,7 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(const __grid_consta
     w.cap_r = a.cap_r;
     w.high_g = a.high_g;
     w.high_e = a.high_e;
+    w.low = a.low;
     w.n[0] = w.n[1] = w.n[2] = w.n[3] = w.n[4] = 0u;
     w.lt = (1u << lane) - 1u;
     w.hw = 0u;
@@ -475,7 +485,7 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(const __grid_consta
     Claim cl;
     cl.exhausted = (a.n_hist == 0u);
     int type = a.S.particle;
-    while (type >= 0) type = (type == 1) ? electron_mode<MULTI>(a, TB, w, cl) : photon_mode<TRACE>(a, TB, w, cl);
+    while (type >= 0) type = (type == 1) ? electron_mode<V>(a, TB, w, cl) : photon_mode<V>(a, TB, w, cl);
 
     // ---- flush this warp's event counts and accounts
     __syncwarp();
@@ -494,8 +504,9 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(const __grid_consta
     double s = 0.0;
     for (size_t i = blockIdx.x * static_cast<size_t>(blockDim.x) + threadIdx.x; i < a.nvox;
          i += static_cast<size_t>(gridDim.x) * blockDim.x) {
-        const double e = P.edep[i];
+        const double e = tally_value<V::TALLY>(P, i);
         s += e;
+        if (V::TALLY == TALLY_FIXED) P.edep[i] = e; // from here on the tally holds MeV as fp64, whatever the mode
         if (a.dose) a.dose[i] = static_cast<float>(e / static_cast<double>(P.geo.phantom[i].x) * a.inv_h3_n);
     }
     s = wsum(s);

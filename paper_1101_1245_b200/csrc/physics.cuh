@@ -243,44 +243,4 @@ __device__ __forceinline__ void pair_angle(float T, float ur, float &c, float &s
     s = sqrtf(fmaxf(omc * (1.0f + c), 0.0f));
 }
 
-// Moller: eps = W/T in [K_cut/T, 1/2]
-__device__ __forceinline__ void sample_moller(const Rng &g, Particle &p, float T, float k_cut, float &eps,
-                                              float &uphi)
-{
-    const float tau = T * (1.0f / kMe);
-    const float q = tau / (tau + 1.0f);
-    const float g2 = q * q;
-    const float g3 = (2.0f * tau + 1.0f) / ((tau + 1.0f) * (tau + 1.0f));
-    const float gmax = 1.0f + 0.25f * g2 + (1.0f - g3);
-    const float emin = k_cut / T;
-    for (;;) {
-        const uint4 v = draw(g, p);
-        const float e = emin / (1.0f - u01(v.x) * (1.0f - 2.0f * emin));
-        const float r = e / (1.0f - e);
-        const float gg = 1.0f + g2 * e * e + r * (r - g3);
-        if (u01(v.y) * gmax <= gg) {
-            eps = e;
-            uphi = u01(v.z);
-            return;
-        }
-    }
-}
-
-// Bremsstrahlung photon energy in [k_c, T]
-__device__ __forceinline__ void sample_brems(const Rng &g, Particle &p, float T, float k_c, float &k, float &uphi)
-{
-    const float lr = logf(T / k_c);
-    const float iE = 1.0f / (T + kMe);
-    for (;;) {
-        const uint4 v = draw(g, p);
-        const float kk = k_c * expf(u01(v.x) * lr);
-        const float y = kk * iE;
-        if (u01(v.y) * (4.0f / 3.0f) <= fmaf(y, y, (4.0f / 3.0f) * (1.0f - y))) {
-            k = kk;
-            uphi = u01(v.z);
-            return;
-        }
-    }
-}
-
 } // namespace gpumcd

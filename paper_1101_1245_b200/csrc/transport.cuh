@@ -38,6 +38,16 @@ struct Opts {
     int pair_mode, photon_only;
 };
 
+// Compile-time variant of the transport code: TRACE records the primary track's event codes
+// (gpumcd_run_trace), MULTI selects multi-voxel electron steps (R32), TALLY the tally arithmetic
+// (gpumcd_options.tally_mode).
+enum : int { TALLY_F64 = 0, TALLY_WARP = 1, TALLY_FIXED = 2 };
+template <bool TRACE_, bool MULTI_, int TALLY_>
+struct Variant {
+    static constexpr bool TRACE = TRACE_, MULTI = MULTI_;
+    static constexpr int TALLY = TALLY_;
+};
+
 // Particle queue: three 16-byte SoA streams -> every push / pop is three 128-bit accesses.
 struct Queue {
     float4 *A;        // fx, fy, fz, E
@@ -66,7 +76,8 @@ struct Params {
     Geom geo;
     Opts opt;
     Rng rng;
-    double *edep;
+    double *edep;                 // energy tally; TALLY_FIXED: 64-bit integers in units of 1/fx_scale MeV until finalize
+    float fx_scale;               // TALLY_FIXED: a power of two chosen per run so that the grid cannot overflow
     DevCounters *cnt;
     unsigned long long *trace;    // or nullptr
     unsigned long long trace_off; // id of the run's first history
@@ -106,10 +117,38 @@ __device__ __forceinline__ unsigned voxel_index(const Geom &g, const Particle &p
            static_cast<unsigned>(g.ny) * static_cast<unsigned>(p.iz)); // <= 2^30 voxels
 }
 
-// H4/H8 tally: fp64 atomic add into the L2-resident energy grid
+// H4/H8 tally into the L2-resident energy grid (the paper only says the dose arrays "are summed", L188):
+//   TALLY_F64   one fp64 atomic add per lane (RED.E.ADD.F64, resolved in L2);
+//   TALLY_WARP  warp-aggregated: the lanes that are together here and hit the same voxel (match.any on the
+//               voxel index) add up in fp64 in lane order and their first lane issues one atomic;
+//   TALLY_FIXED 64-bit fixed point: e * 2^k rounded to an integer (exact for e >= 2^(24-k) MeV), integer
+//               atomic add: additions commute exactly, so the tally is bitwise reproducible.
+template <class V>
 __device__ __forceinline__ void deposit(const Params &P, unsigned lin, float e)
 {
-    atomicAdd(&P.edep[lin], static_cast<double>(e));
+    if (V::TALLY == TALLY_FIXED) {
+        atomicAdd(reinterpret_cast<unsigned long long *>(P.edep) + lin,
+                  static_cast<unsigned long long>(__float2ll_rn(e * P.fx_scale)));
+    } else if (V::TALLY == TALLY_WARP) {
+        const unsigned act = __activemask();
+        const unsigned grp = __match_any_sync(act, lin);
+        double s = static_cast<double>(e);
+        if (grp & (grp - 1u)) { // several lanes on this voxel: every one of them walks the group in lane order
+            s = 0.0;
+            for (unsigned m = grp; m; m &= m - 1u) s += static_cast<double>(__shfl_sync(grp, e, __ffs(m) - 1));
+        }
+        if ((threadIdx.x & 31) == __ffs(grp) - 1) atomicAdd(&P.edep[lin], s);
+    } else {
+        atomicAdd(&P.edep[lin], static_cast<double>(e));
+    }
+}
+// the tally entry as energy in MeV (finalize)
+template <int TALLY>
+__device__ __forceinline__ double tally_value(const Params &P, size_t i)
+{
+    if (TALLY == TALLY_FIXED)
+        return static_cast<double>(reinterpret_cast<const long long *>(P.edep)[i]) / static_cast<double>(P.fx_scale);
+    return P.edep[i];
 }
 
 // ---- records ---------------------------------------------------------------------------------
@@ -210,10 +249,10 @@ __device__ __forceinline__ bool photon_alive(int ev) { return ev == PH_COMPTON |
 // history's word in global memory.  The codes are non-zero, so the number of events recorded so far
 // is the index of the highest non-zero group + 1 and no per-particle trace state exists: a photon
 // can be parked in a stack and picked up by another lane of its warp (persistent.cuh) in between.
-template <bool TRACE>
+template <class V>
 __device__ __forceinline__ void record(const Params &P, const Particle &p, int code)
 {
-    if (TRACE && p.track == 0u) {
+    if (V::TRACE && p.track == 0u) {
         volatile unsigned long long *t =
             P.trace + (((static_cast<unsigned long long>(P.rng.hist_hi) << 32) | p.hist) - P.trace_off);
         const unsigned long long bits = *t;
@@ -225,7 +264,7 @@ __device__ __forceinline__ void record(const Params &P, const Particle &p, int c
 // One flight (Eq. 1 with the Woodcock majorant of Eq. 3) and the choice of the interaction at its
 // end (Eq. 2 per type; the remainder up to mu_max is fictitious, L59).  Returns the next mode:
 // PM_DEAD (escaped), PM_FLIGHT (fictitious interaction: nothing changes), or the interaction.
-template <bool TRACE>
+template <class V>
 __device__ __forceinline__ int photon_flight(const Params &P, const float *__restrict__ TB, Particle &p)
 {
     const Tables &tb = P.tab;
@@ -236,7 +275,7 @@ __device__ __forceinline__ int photon_flight(const Params &P, const float *__res
     advance(p, s * P.geo.inv_h);
     if (!inside(P.geo, p)) {
         Acc(P).esc(p.E);
-        record<TRACE>(P, p, 4);
+        record<V>(P, p, 4);
         return PM_DEAD;
     }
     const float2 pv = __ldg(&P.geo.phantom[voxel_index(P.geo, p)]);
@@ -245,14 +284,15 @@ __device__ __forceinline__ int photon_flight(const Params &P, const float *__res
     const float r = u01(w.y) * mu_max;
     const float c1 = rho * interp(col, iE);
     const float c2 = fmaf(rho, interp(col + tb.gE.n, iE), c1);
-    const float c3 = fmaf(rho, interp(col + 2 * tb.gE.n, iE), c2);
+    // pair production needs E > 2 m (L74; R33: the interpolated column is not zero just below the threshold)
+    const float c3 = p.E > 2.0f * kMe ? fmaf(rho, interp(col + 2 * tb.gE.n, iE), c2) : c2;
     if (r >= c3) return PM_FLIGHT;
     return r < c1 ? PM_COMPTON : (r < c2 ? PM_PHOTO : PM_PAIR);
 }
 
 // The interaction `kind` (PM_COMPTON / PM_PHOTO / PM_PAIR) at the photon's position.  Returns
 // PM_FLIGHT if the photon goes on (Compton above P_cut), else PM_DEAD.
-template <bool TRACE, class QE, class QG>
+template <class V, class QE, class QG>
 __device__ __forceinline__ int photon_interact(const Params &P, Particle &p, int kind, const QE &qE, const QG &qG)
 {
     const Tables &tb = P.tab;
@@ -260,7 +300,7 @@ __device__ __forceinline__ int photon_interact(const Params &P, Particle &p, int
     const unsigned lin = voxel_index(P.geo, p);
     if (kind == PM_COMPTON) {
         // ---- Compton (L65) ----
-        record<TRACE>(P, p, 1);
+        record<V>(P, p, 1);
         float eps, t, uphi, nu, nv, nw, sp, cp;
         sample_compton(P.rng, p, eps, t, uphi);
         sincos2pi(uphi, sp, cp);
@@ -277,22 +317,22 @@ __device__ __forceinline__ int photon_interact(const Params &P, Particle &p, int
             c.ctr = 0u;
             push_e(P, qE, c);
         } else {
-            deposit(P, lin, Te);
+            deposit<V>(P, lin, Te);
             acc.cut(Te);
         }
         p.E = E1;
         p.u = nu; p.v = nv; p.w = nw;
         if (p.E < tb.p_cut) {
-            deposit(P, lin, p.E);
+            deposit<V>(P, lin, p.E);
             acc.cut(p.E);
-            record<TRACE>(P, p, 5);
+            record<V>(P, p, 5);
             return PM_DEAD;
         }
         return PM_FLIGHT;
     }
     if (kind == PM_PHOTO) {
         // ---- photoelectric (L67-72): one electron with T = E_phot ----
-        record<TRACE>(P, p, 2);
+        record<V>(P, p, 2);
         if (electron_tracked(P, p.E)) {
             float nu_, uphi, sp, cp;
             sample_sauter(P.rng, p, p.E, nu_, uphi);
@@ -303,13 +343,13 @@ __device__ __forceinline__ int photon_interact(const Params &P, Particle &p, int
             c.ctr = 0u;
             push_e(P, qE, c);
         } else {
-            deposit(P, lin, p.E);
+            deposit<V>(P, lin, p.E);
             acc.cut(p.E);
         }
         return PM_DEAD;
     }
     // ---- pair production (L74): two electrons, no positron ----
-    record<TRACE>(P, p, 3);
+    record<V>(P, p, 3);
     const uint4 v = draw(P.rng, p);
     const float Tsum = p.E - 2.0f * kMe;
     const float T1 = u01(v.x) * Tsum;
@@ -338,7 +378,7 @@ __device__ __forceinline__ int photon_interact(const Params &P, Particle &p, int
         c.E = T1; c.track = id.x;
         push_e(P, qE, c);
     } else {
-        deposit(P, lin, T1);
+        deposit<V>(P, lin, T1);
         acc.cut(T1);
     }
     if (t2) {
@@ -346,7 +386,7 @@ __device__ __forceinline__ int photon_interact(const Params &P, Particle &p, int
         c.E = T2; c.track = id.y;
         push_e(P, qE, c);
     } else {
-        deposit(P, lin, T2);
+        deposit<V>(P, lin, T2);
         acc.cut(T2);
     }
     acc.pair();
@@ -357,21 +397,21 @@ __device__ __forceinline__ int photon_interact(const Params &P, Particle &p, int
         c.u = -ax; c.v = -ay; c.w = -az; c.track = id.w;
         push_g(P, qG, c);
     } else {
-        deposit(P, lin, 2.0f * kMe);
+        deposit<V>(P, lin, 2.0f * kMe);
         acc.cut(2.0f * kMe);
     }
     return PM_DEAD;
 }
 
 // flight + interaction; returns the event (the photon is alive afterwards iff photon_alive(event))
-template <bool TRACE>
+template <class V>
 __device__ int photon_step(const Params &P, const float *__restrict__ TB, Particle &p, const Queue &qE,
                            const Queue &qG)
 {
-    const int kind = photon_flight<TRACE>(P, TB, p);
+    const int kind = photon_flight<V>(P, TB, p);
     if (kind == PM_DEAD) return PH_ESCAPE;
     if (kind == PM_FLIGHT) return PH_FICT;
-    const int next = photon_interact<TRACE>(P, p, kind, qE, qG);
+    const int next = photon_interact<V>(P, p, kind, qE, qG);
     if (kind == PM_COMPTON) return next == PM_FLIGHT ? PH_COMPTON : PH_ABSORBED;
     return kind == PM_PHOTO ? PH_PHOTO : PH_PAIR;
 }
@@ -441,7 +481,7 @@ __device__ __forceinline__ unsigned voxel_ahead(const Geom &g, const Particle &p
               : fallback;
 }
 
-template <bool MULTI>
+template <class V>
 __device__ __forceinline__ int electron_step(const Params &P, const float *__restrict__ TB, Particle &p, float &lnT,
                                              float &M)
 {
@@ -468,7 +508,7 @@ __device__ __forceinline__ int electron_step(const Params &P, const float *__res
     const float L0 = rho * interp(el, iT);
     const float e_cap = fminf(P.opt.es_max, fdiv(P.opt.f_eloss * T, L0));
     float d_vox;
-    if (MULTI) // R32: the boundary that limits the step is the next change of medium along d
+    if (V::MULTI) // R32: the boundary that limits the step is the next change of medium along d
         d_vox = (hom_distance(P, p, pv, fminf(e_hard, e_cap) * P.geo.inv_h) + P.opt.nudge) * P.geo.h;
     else
         d_vox = (fminf(dx, fminf(dy, dz)) + P.opt.nudge) * P.geo.h;
@@ -479,7 +519,7 @@ __device__ __forceinline__ int electron_step(const Params &P, const float *__res
     const float Tmid = fmaxf(fmaf(-0.5f * L0, es, T), tb.e_min);
     const float dE = es * rho * interp(el, locate(tb.gE, flog(Tmid)));
     if (T - dE < tb.e_cut) {
-        deposit(P, lin, T);
+        deposit<V>(P, lin, T);
         acc.cut(T);
         return ST_DEAD;
     }
@@ -493,12 +533,12 @@ __device__ __forceinline__ int electron_step(const Params &P, const float *__res
     // path (first leg, then second leg); its uniform comes from the low bits of a.y, a.z, a.w that u01
     // does not use
     float s_dep = 0.0f;
-    if (MULTI) {
+    if (V::MULTI) {
         const uint32_t bits = (a.y & 0x1ffu) | ((a.z & 0x1ffu) << 9) | ((a.w & 0x1fu) << 18);
         s_dep = fmaf(__uint2float_rz(bits), 1.0f / 8388608.0f, 1.0f / 16777216.0f) * esv;
-        if (s_dep <= leg1) deposit(P, voxel_ahead(P.geo, p, s_dep, lin), dE);
+        if (s_dep <= leg1) deposit<V>(P, voxel_ahead(P.geo, p, s_dep, lin), dE);
     } else {
-        deposit(P, lin, dE);
+        deposit<V>(P, lin, dE);
     }
     p.fx = fmaf(leg1, p.u, p.fx);
     p.fy = fmaf(leg1, p.v, p.fy);
@@ -515,7 +555,7 @@ __device__ __forceinline__ int electron_step(const Params &P, const float *__res
         sincos2pi(u01(a.w), sp, cp);
         rotate(p.u, p.v, p.w, fmaf(-2.0f, mu, 1.0f), 2.0f * sqrtf(mu * (1.0f - mu)), cp, sp, p.u, p.v, p.w);
     }
-    if (MULTI && s_dep > leg1) deposit(P, voxel_ahead(P.geo, p, s_dep - leg1, lin), dE);
+    if (V::MULTI && s_dep > leg1) deposit<V>(P, voxel_ahead(P.geo, p, s_dep - leg1, lin), dE);
     advance(p, (1.0f - zeta) * esv);
     p.E = T1;
     lnT = lnT1;
@@ -533,6 +573,7 @@ __device__ __forceinline__ int electron_step(const Params &P, const float *__res
 // ---------------------------------------------------------------------------------------------
 enum : int { HK_FICT = 0, HK_MOLLER = 1, HK_BREMS = 2 };
 
+template <class V>
 __device__ __forceinline__ int electron_hard(const Params &P, const float *__restrict__ TB, Particle &p, float &lnT,
                                              float M, Particle &child, int &kind)
 {
@@ -544,10 +585,11 @@ __device__ __forceinline__ int electron_hard(const Params &P, const float *__res
     const float2 pv1 = __ldg(&P.geo.phantom[lin1]);
     const float *el1 = TB + tb.off_el + mat_of(pv1) * 4 * nE;
     const Interp i1 = locate(tb.gE, lnT);
-    const float sM = pv1.x * interp(el1 + nE, i1);
+    const float T1 = p.E;
+    // a Moller event transfers W in [K_cut, T/2] (L90): none for T <= 2 K_cut (R33)
+    const float sM = T1 > 2.0f * tb.e_cut ? pv1.x * interp(el1 + nE, i1) : 0.0f;
     const float sB = pv1.x * interp(el1 + 2 * nE, i1);
     const float r = u01(b.x) * M;
-    const float T1 = p.E;
     kind = HK_FICT;
     if (r >= sM + sB) return ST_ALIVE;
     // One rejection loop serves both samplers (one Philox block per trial, as everywhere): the lanes
@@ -610,7 +652,7 @@ __device__ __forceinline__ int electron_hard(const Params &P, const float *__res
     child.E = x;
     p.E = T1 - x;
     if (p.E < tb.e_cut) {
-        deposit(P, lin1, p.E);
+        deposit<V>(P, lin1, p.E);
         acc.cut(p.E);
         return ST_DEAD;
     }
@@ -627,12 +669,12 @@ struct Local {
     unsigned steps = 0, moller = 0, brems = 0, hfict = 0;
 };
 
-template <bool TRACE>
+template <class V>
 __device__ void photon_run(const Params &P, Particle p, Local &L, const Queue &qE, const Queue &qG)
 {
     const float *TB = P.tab.blob;
     for (;;) {
-        const int ev = photon_step<TRACE>(P, TB, p, qE, qG);
+        const int ev = photon_step<V>(P, TB, p, qE, qG);
         L.flights++;
         L.compton += (ev == PH_COMPTON || ev == PH_ABSORBED);
         L.photo += (ev == PH_PHOTO);
@@ -642,18 +684,18 @@ __device__ void photon_run(const Params &P, Particle p, Local &L, const Queue &q
     }
 }
 
-template <bool MULTI>
+template <class V>
 __device__ void electron_run(const Params &P, Particle p, Local &L, const Queue &qE, const Queue &qG)
 {
     float lnT = flog(p.E), M;
     const float *TB = P.tab.blob;
     for (;;) {
-        int st = electron_step<MULTI>(P, TB, p, lnT, M);
+        int st = electron_step<V>(P, TB, p, lnT, M);
         L.steps++;
         if (st == ST_HARD) {
             Particle c;
             int kind;
-            st = electron_hard(P, TB, p, lnT, M, c, kind);
+            st = electron_hard<V>(P, TB, p, lnT, M, c, kind);
             if (kind == HK_MOLLER) { L.moller++; push_e(P, qE, c); }
             else if (kind == HK_BREMS) { L.brems++; push_g(P, qG, c); }
             else L.hfict++;

@@ -9,14 +9,14 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 def test_reference_arm_prints_one_json_line_with_the_contract_keys():
     out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--steps", "1",
-                          "--warmup", "0", "--ref-histories", "2000"], capture_output=True, text=True, timeout=300, cwd=ROOT)
+                          "--warmup", "0", "--ref-histories", "2000"], capture_output=True, text=True, timeout=600, cwd=ROOT)
     assert out.returncode == 0, out.stderr
     lines = [l for l in out.stdout.splitlines() if l.strip()]
     assert len(lines) == 1
     d = json.loads(lines[0])
     assert d["impl"] == "reference" and d["unit"] == "histories/s" and d["higher_is_better"] is True
     assert d["metric"] == "coupled photon-electron histories/s" and d["value"] > 0 and d["ch_steps_per_s"] > 0
-    assert d["config"]["workload"] == "cfg2_15MeV_electron_10x10_water128"
+    assert d["config"]["workload"] == "cfg5_18MV_photon_10x10_ctlike256"      # the headline workload of the GPU arm
     assert d["cpu_baseline"]["kind"] == "oracle" and d["cpu_baseline"]["cores"] >= 1
     assert d["e2e"] == {"value": d["value"], "unit": "histories/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}
     assert d["dtype"] == "f64" and d["vs_baseline"] is None and d["steps"] == 1

@@ -326,11 +326,12 @@ def test_error_paths(workloads):
             g.gpumcd_run(ctx, 20000, 1, dose2)
             g.gpumcd_get_counters(ctx)
         assert e.value.status == -4
-    # scheduler 1: a warp changes type before a stack fills up (persistent.cuh kMustMargin), so even the
-    # smallest stacks the library accepts (192 records) hold what a warp banks: same events, no overflow
+    # scheduler 1: a warp changes type before a stack fills up (persistent.cuh "Forced type changes"), so even the
+    # smallest stacks the library accepts (256 records; smaller requests are raised to that) hold what a warp
+    # banks: same events, no overflow
     ref = run_gpu(w2, 200_000, scheduler=1)
     small = run_gpu(w2, 200_000, scheduler=1, warp_stack=192)
-    assert small["counters"]["overflow_count"] == 0 and small["counters"]["bank_high_water"] <= 192
+    assert small["counters"]["overflow_count"] == 0 and small["counters"]["bank_high_water"] <= 256
     for k in INT_KEYS:
         assert small["counters"][k] == ref["counters"][k], k
 
