@@ -37,7 +37,8 @@ typedef struct gpumcd_ctx gpumcd_ctx; /* opaque, owned by the library */
 
 typedef enum {
     GPUMCD_OK = 0,
-    GPUMCD_ERR_INVALID_ARG = -1,   /* null pointer, bad size, material id out of range, density <= 0 */
+    GPUMCD_ERR_INVALID_ARG = -1,   /* null pointer, bad size, material id out of range, density outside
+                                      [2^-20, 2^12) g/cm^3 (9.5e-7 .. 4096) or not a number */
     GPUMCD_ERR_CUDA = -2,          /* a CUDA runtime call failed; see gpumcd_last_error */
     GPUMCD_ERR_OOM = -3,           /* device allocation failed */
     GPUMCD_ERR_BANK_OVERFLOW = -4, /* a particle queue filled up; the run's result is invalid
@@ -128,6 +129,11 @@ typedef struct {
                               how much work of one type is done before the other type is picked up      */
     uint32_t bank_low;     /* scheduler 1, tuning (0 = 24, at most 64): once the source is exhausted a warp with
                               fewer ready particles of its type than this changes to the other type      */
+    int32_t l2_persist;    /* scheduler 1: 1 = the packed phantom (4 bytes per voxel) is read through a persisting
+                              L2 access window, so that the tally and the particle stacks cannot evict it
+                              (raises the device-wide cudaLimitPersistingL2CacheSize to the phantom's size, up
+                              to the device maximum; the lines stay set aside until gpumcd_release_l2);
+                              0 (default) = plain caching                                                */
 } gpumcd_options;
 
 typedef struct {
@@ -227,6 +233,10 @@ int gpumcd_get_energy_tally(gpumcd_ctx *ctx, double *edep_out_dev);
  * first_history + n_histories - 1 (disjoint ranges on different GPUs give independent samples of
  * the same stream family).  Default 0.  Trace output is indexed from first_history. */
 int gpumcd_set_history_offset(gpumcd_ctx *ctx, uint64_t first_history);
+
+/* l2_persist = 1: wait for the context's last run and give the persisting L2 lines back to normal use
+ * (cudaCtxResetPersistingL2Cache).  A no-op otherwise. */
+int gpumcd_release_l2(gpumcd_ctx *ctx);
 
 /* Per-kernel device times of the last run, measured with CUDA events on the run's stream, and the
  * number of kernels the run launched.  Recording is off by default (it adds events around every

@@ -6,6 +6,6 @@ paper (gamma index, Eq. 14-15; uncertainty, Eq. 12-13).
 """
 from .binding import (Context, GpumcdError, gpumcd_create, gpumcd_create_host, gpumcd_default_options,  # noqa: F401
                       gpumcd_destroy, gpumcd_get_counters, gpumcd_get_energy_tally, gpumcd_last_error,
-                      gpumcd_get_profile, gpumcd_probe_tally, gpumcd_selftest_philox, gpumcd_run, gpumcd_run_host, gpumcd_run_trace, gpumcd_run_uncertainty,
+                      gpumcd_get_profile, gpumcd_probe_tally, gpumcd_selftest_philox, gpumcd_release_l2, gpumcd_run, gpumcd_run_host, gpumcd_run_trace, gpumcd_run_uncertainty,
                       gpumcd_set_history_offset, gpumcd_set_phantom, gpumcd_set_phantom_host, gpumcd_set_profiling,
                       gpumcd_set_source, load_library)

@@ -27,7 +27,7 @@ EXPORTS = ("gpumcd_default_options", "gpumcd_create", "gpumcd_create_host", "gpu
            "gpumcd_set_phantom_host", "gpumcd_set_source", "gpumcd_run",
            "gpumcd_run_host", "gpumcd_run_uncertainty", "gpumcd_run_trace", "gpumcd_get_counters", "gpumcd_get_energy_tally",
            "gpumcd_set_history_offset", "gpumcd_set_profiling", "gpumcd_get_profile", "gpumcd_probe_tally",
-           "gpumcd_selftest_philox",
+           "gpumcd_selftest_philox", "gpumcd_release_l2",
            "gpumcd_last_error", "gpumcd_destroy")
 
 
@@ -43,7 +43,7 @@ class gpumcd_options(C.Structure):
                 ("wave_size", C.c_uint32), ("bank_factor", C.c_uint32), ("scheduler", C.c_int32),
                 ("warp_stack", C.c_uint32), ("cta_threads", C.c_uint32), ("hom_tol", C.c_float),
                 ("tally_mode", C.c_int32), ("table_memory", C.c_int32), ("bank_high_g", C.c_uint32),
-                ("bank_high_e", C.c_uint32), ("bank_low", C.c_uint32)]
+                ("bank_high_e", C.c_uint32), ("bank_low", C.c_uint32), ("l2_persist", C.c_int32)]
 
 
 class gpumcd_source(C.Structure):
@@ -108,6 +108,7 @@ def load_library():
         lib.gpumcd_get_profile.argtypes = [vp, C.POINTER(gpumcd_profile)]
         lib.gpumcd_probe_tally.argtypes = [vp, C.c_uint64, C.POINTER(C.c_double), vp]
         lib.gpumcd_selftest_philox.argtypes = [vp, vp, vp, C.c_uint64, vp]
+        lib.gpumcd_release_l2.argtypes = [vp]
         lib.gpumcd_last_error.argtypes = [vp]
         lib.gpumcd_last_error.restype = C.c_char_p
         lib.gpumcd_destroy.argtypes = [vp]
@@ -286,6 +287,10 @@ def gpumcd_get_energy_tally(ctx: Context, edep_out_dev) -> None:
 
 def gpumcd_set_history_offset(ctx: Context, first_history: int) -> None:
     ctx._check(load_library().gpumcd_set_history_offset(ctx._h, int(first_history)))
+
+
+def gpumcd_release_l2(ctx: Context) -> None:
+    ctx._check(load_library().gpumcd_release_l2(ctx._h))
 
 
 def gpumcd_set_profiling(ctx: Context, enable: bool) -> None:

@@ -20,25 +20,27 @@ constexpr int kBlock = 256;
 // ---------------------------------------------------------------------------------------------
 // Setup kernels
 // ---------------------------------------------------------------------------------------------
-// Pack {density, material} per voxel, validate, and reduce the largest density of each material
-// (H10; positive floats order like their bit patterns, so atomicMax on the bits is a float max).
-__global__ void k_pack_phantom(const float *__restrict__ density, const uint8_t *__restrict__ material,
-                               size_t nvox, int n_mat, float2 *__restrict__ out, unsigned *rho_max_bits,
+// Pack {density, material} per voxel into 4 bytes (transport.cuh pack_voxel_record), validate, and reduce the
+// largest density of each material (H10; positive floats order like their bit patterns, so atomicMax on the bits
+// is a float max).
+__global__ void k_pack_phantom(const float *__restrict__ density, const uint8_t *__restrict__ material, Geom g,
+                               size_t nvox, int n_mat, uint32_t *__restrict__ out, unsigned *rho_max_bits,
                                unsigned *n_bad)
 {
     __shared__ unsigned s_max[8];
     if (threadIdx.x < 8) s_max[threadIdx.x] = 0u;
     __syncthreads();
     for (size_t i = blockIdx.x * static_cast<size_t>(blockDim.x) + threadIdx.x; i < nvox;
-         i += static_cast<size_t>(gridDim.x) * blockDim.x) {
-        const float d = density[i];
-        const int m = material[i];
-        if (m >= n_mat || !(d > 0.0f) || !isfinite(d)) {
+         i += static_cast<size_t>(gridDim.x) * blockDim.x) { // i: internal index
+        const size_t src = caller_index(g, i);
+        const uint32_t d = __float_as_uint(density[src]);
+        const int m = material[src];
+        if (m >= n_mat || !density_packable(d)) { // (NaN, inf, zero, negative and denormal densities fail the range test)
             atomicAdd(n_bad, 1u);
-            out[i] = make_float2(1.0f, __int_as_float(0));
+            out[i] = pack_voxel_record(__float_as_uint(1.0f), 0);
         } else {
-            atomicMax(&s_max[m], __float_as_uint(d));
-            out[i] = make_float2(d, __int_as_float(m));
+            atomicMax(&s_max[m], d);
+            out[i] = pack_voxel_record(d, m);
         }
     }
     __syncthreads();
@@ -47,15 +49,16 @@ __global__ void k_pack_phantom(const float *__restrict__ density, const uint8_t 
 
 // Multi-voxel steps (hom_tol > 0): the uniform radius of every voxel, R = the largest r <= r_max such that
 // all voxels within Chebyshev distance r lie inside the phantom and continue the voxel's medium (same
-// material, |density - own| <= hom_tol * own); stored in bits 8-10 of the record's material word.
-__global__ void k_uniform_radius(float2 *__restrict__ phantom, int nx, int ny, int nz, float hom_tol, int r_max)
+// material, |density - own| <= hom_tol * own).
+__global__ void k_uniform_radius(const uint32_t *__restrict__ phantom, uint8_t *__restrict__ radius, Geom g,
+                                 float hom_tol, int r_max)
 {
+    const int nx = g.nx, ny = g.ny, nz = g.nz;
     const size_t nvox = static_cast<size_t>(nx) * ny * nz;
     for (size_t i = blockIdx.x * static_cast<size_t>(blockDim.x) + threadIdx.x; i < nvox;
-         i += static_cast<size_t>(gridDim.x) * blockDim.x) {
+         i += static_cast<size_t>(gridDim.x) * blockDim.x) { // i: internal index
         const int ix = static_cast<int>(i % nx), iy = static_cast<int>((i / nx) % ny), iz = static_cast<int>(i / (static_cast<size_t>(nx) * ny));
-        const float2 pv0 = phantom[i];
-        const int m0 = __float_as_int(pv0.y) & 0xff;
+        const Voxel pv0 = unpack_voxel(phantom[i]);
         const float band = hom_tol * pv0.x;
         int R = 0;
         for (int r = 1; r <= r_max; ++r) {
@@ -64,14 +67,14 @@ __global__ void k_uniform_radius(float2 *__restrict__ phantom, int nx, int ny, i
                 for (int dy = -r; ok && dy <= r; ++dy) {
                     const bool shell_row = (dz == -r || dz == r || dy == -r || dy == r);
                     for (int dx = -r; ok && dx <= r; dx += (shell_row ? 1 : 2 * r)) { // the shell at distance r only
-                        const float2 pv = phantom[static_cast<size_t>(ix + dx) + static_cast<size_t>(nx) * ((iy + dy) + static_cast<size_t>(ny) * (iz + dz))];
-                        ok = ((__float_as_int(pv.y) & 0xff) == m0) && fabsf(pv.x - pv0.x) <= band;
+                        const Voxel pv = unpack_voxel(phantom[lin_of(g, ix + dx, iy + dy, iz + dz)]);
+                        ok = pv.m == pv0.m && fabsf(pv.x - pv0.x) <= band;
                     }
                 }
             if (!ok) break;
             R = r;
         }
-        reinterpret_cast<int *>(phantom)[2 * i + 1] = m0 | (R << 8);
+        radius[i] = static_cast<uint8_t>(R);
     }
 }
 
@@ -132,7 +135,7 @@ __global__ void __launch_bounds__(kBlock) k_electron_pass(Params P, Queue in, un
 template <int TALLY>
 __global__ void k_finalize(Params P, size_t nvox, double inv_h3_n, float *__restrict__ dose)
 {
-    const float2 *__restrict__ phantom = P.geo.phantom;
+    const uint32_t *__restrict__ phantom = P.geo.phantom;
     DevCounters *cnt = P.cnt;
     double s = 0.0;
     for (size_t i = blockIdx.x * static_cast<size_t>(blockDim.x) + threadIdx.x; i < nvox;
@@ -140,7 +143,7 @@ __global__ void k_finalize(Params P, size_t nvox, double inv_h3_n, float *__rest
         const double e = tally_value<TALLY>(P, i);
         s += e;
         if (TALLY == TALLY_FIXED) P.edep[i] = e; // from here on the tally holds MeV as fp64
-        if (dose) dose[i] = static_cast<float>(e / static_cast<double>(phantom[i].x) * inv_h3_n);
+        if (dose) dose[caller_index(P.geo, i)] = static_cast<float>(e / static_cast<double>(unpack_voxel(phantom[i]).x) * inv_h3_n);
     }
     s = wsum(s);
     __shared__ double part[32];
@@ -173,19 +176,29 @@ __global__ void k_accumulate_batch(double *__restrict__ edep, double *__restrict
 // dose = total energy / mass / histories (H8); Delta D = sqrt((<x^2> - <x>^2) / (B - 1)) / mass (Eq. 13);
 // the energy tally is left holding the total of all batches.
 __global__ void k_finalize_uncertainty(const double *__restrict__ s1, const double *__restrict__ sx,
-                                       const double *__restrict__ sxx, const float2 *__restrict__ phantom,
+                                       const double *__restrict__ sxx, Geom g,
                                        size_t nvox, double inv_h3, double inv_n, double n_batches,
                                        float *__restrict__ dose, float *__restrict__ sigma, double *__restrict__ edep)
 {
+    const uint32_t *__restrict__ phantom = g.phantom;
     for (size_t i = blockIdx.x * static_cast<size_t>(blockDim.x) + threadIdx.x; i < nvox;
          i += static_cast<size_t>(gridDim.x) * blockDim.x) {
-        const double inv_mass = inv_h3 / static_cast<double>(phantom[i].x);
+        const double inv_mass = inv_h3 / static_cast<double>(unpack_voxel(phantom[i]).x);
         const double mean = sx[i] / n_batches;
         const double var = (sxx[i] / n_batches - mean * mean) / (n_batches - 1.0);
-        dose[i] = static_cast<float>(s1[i] * inv_mass * inv_n);
-        sigma[i] = static_cast<float>(sqrt(fmax(var, 0.0)) * inv_mass);
+        const size_t o = caller_index(g, i);
+        dose[o] = static_cast<float>(s1[i] * inv_mass * inv_n);
+        sigma[o] = static_cast<float>(sqrt(fmax(var, 0.0)) * inv_mass);
         edep[i] = s1[i];
     }
+}
+
+// gpumcd_get_energy_tally: the tally in the caller's [nz][ny][nx] order
+__global__ void k_export_tally(const double *__restrict__ edep, Geom g, size_t nvox, double *__restrict__ out)
+{
+    for (size_t i = blockIdx.x * static_cast<size_t>(blockDim.x) + threadIdx.x; i < nvox;
+         i += static_cast<size_t>(gridDim.x) * blockDim.x)
+        out[caller_index(g, i)] = edep[i];
 }
 
 // Tally probe (the denominator of the tally's roofline, since no vendor figure exists for
@@ -193,7 +206,7 @@ __global__ void k_finalize_uncertainty(const double *__restrict__ s1, const doub
 // at pseudo-random voxels of the beam-shaped region x in [x0, x0+wx), y in [y0, y0+wy), all depths, the
 // address pattern of the condensed-history deposits, and nothing else.
 template <bool FIXED>
-__global__ void k_tally_probe(double *__restrict__ edep, int nx, int ny, int nz, int x0, int y0, int wx, int wy,
+__global__ void k_tally_probe(double *__restrict__ edep, Geom g, int x0, int y0, int wx, int wy,
                               unsigned per_thread, unsigned seed)
 {
     const unsigned tid = blockIdx.x * blockDim.x + threadIdx.x;
@@ -205,8 +218,8 @@ __global__ void k_tally_probe(double *__restrict__ edep, int nx, int ny, int nz,
         r.z = r.z * 1103515245u + 12345u;
         const unsigned ix = x0 + __umulhi(r.x, static_cast<unsigned>(wx));
         const unsigned iy = y0 + __umulhi(r.y, static_cast<unsigned>(wy));
-        const unsigned iz = __umulhi(r.z, static_cast<unsigned>(nz));
-        const size_t lin = ix + static_cast<size_t>(nx) * (iy + static_cast<size_t>(ny) * iz);
+        const unsigned iz = __umulhi(r.z, static_cast<unsigned>(g.nz));
+        const size_t lin = lin_of(g, static_cast<int>(ix), static_cast<int>(iy), static_cast<int>(iz));
         if (FIXED) atomicAdd(reinterpret_cast<unsigned long long *>(edep) + lin, 1ull);
         else atomicAdd(&edep[lin], 1.0);
     }
@@ -233,6 +246,8 @@ __global__ void k_philox_selftest(const uint32_t *__restrict__ in, uint32_t *__r
 using namespace gpumcd;
 
 constexpr int kMaxQueues = 4;
+constexpr int kSpecSmemBins = 1024;
+constexpr size_t kSpecSmemBytes = (kSpecSmemBins + 1) * (sizeof(double) + sizeof(float)) + 4; // padded to 16 bytes
 
 struct gpumcd_ctx {
     int nx = 0, ny = 0, nz = 0;
@@ -241,7 +256,8 @@ struct gpumcd_ctx {
     float e_max = 0.f;
     gpumcd_options opt{};
     // device memory
-    float2 *phantom = nullptr;
+    uint32_t *phantom = nullptr;      // packed records, 4 B per voxel
+    uint8_t *radius = nullptr;        // hom_tol > 0: uniform radius per voxel
     float *stage_density = nullptr;   // device staging of host volumes (gpumcd_create_host / set_phantom_host)
     uint8_t *stage_material = nullptr;
     unsigned *scratch = nullptr;      // 8 rho_max bit patterns + 1 bad-voxel count
@@ -270,6 +286,9 @@ struct gpumcd_ctx {
     int p_grid = 0;                 // CTAs of the persistent kernel (one per SM)
     bool smem_tables = false;
     unsigned table_floats = 0;
+    size_t spec_smem_bytes = 0;     // dynamic shared memory reserved behind the tables for the spectrum arrays
+    size_t l2_window = 0;           // l2_persist: bytes of the phantom covered by the persisting access window
+    float l2_hit_ratio = 0.f;
     // host state
     Tables tab{};
     bool have_source = false;
@@ -319,6 +338,16 @@ static void set_error(gpumcd_ctx *ctx, const char *msg)
     if (ctx) ctx->err = msg; else g_create_error = msg;
 }
 
+static Geom make_geom(const gpumcd_ctx *c)
+{
+    Geom g;
+    g.phantom = c->phantom;
+    g.radius = c->radius;
+    g.nx = c->nx; g.ny = c->ny; g.nz = c->nz;
+    g.h = c->h; g.inv_h = 1.0f / c->h;
+    return g;
+}
+
 static Queue make_queue(gpumcd_ctx *c, int k)
 {
     Queue q;
@@ -348,6 +377,7 @@ extern "C" int gpumcd_default_options(gpumcd_options *opt)
     opt->bank_high_g = 0;
     opt->bank_high_e = 0;
     opt->bank_low = 0;
+    opt->l2_persist = 0;
     return GPUMCD_OK;
 }
 
@@ -355,6 +385,7 @@ static void destroy_impl(gpumcd_ctx *c)
 {
     if (!c) return;
     cudaFree(c->phantom);
+    cudaFree(c->radius);
     cudaFree(c->stage_density);
     cudaFree(c->stage_material);
     cudaFree(c->scratch);
@@ -432,17 +463,17 @@ static int load_phantom(gpumcd_ctx *ctx, const float *density, const uint8_t *ma
     }
     CK(cudaMemsetAsync(ctx->scratch, 0, 12 * sizeof(unsigned), nullptr));
     const int grid = static_cast<int>(std::min<size_t>((nvox + kBlock - 1) / kBlock, 148 * 8));
-    k_pack_phantom<<<grid, kBlock>>>(d_density, d_material, nvox, ctx->n_mat, ctx->phantom, ctx->scratch, ctx->scratch + 8);
+    k_pack_phantom<<<grid, kBlock>>>(d_density, d_material, make_geom(ctx), nvox, ctx->n_mat, ctx->phantom, ctx->scratch, ctx->scratch + 8);
     CK(cudaGetLastError());
     if (ctx->opt.hom_tol > 0.f) {
         const int r_max = std::min(7, static_cast<int>(std::ceil(ctx->opt.es_max_cm / ctx->h)) + 1);
-        k_uniform_radius<<<grid, kBlock>>>(ctx->phantom, ctx->nx, ctx->ny, ctx->nz, ctx->opt.hom_tol, r_max);
+        k_uniform_radius<<<grid, kBlock>>>(ctx->phantom, ctx->radius, make_geom(ctx), ctx->opt.hom_tol, r_max);
         CK(cudaGetLastError());
     }
     unsigned h_scratch[12];
     CK(cudaMemcpy(h_scratch, ctx->scratch, sizeof h_scratch, cudaMemcpyDeviceToHost));
     if (h_scratch[8] != 0) {
-        set_error(ctx, "phantom has a material id >= n_materials or a density that is not a positive finite number");
+        set_error(ctx, "phantom has a material id >= n_materials or a density outside [2^-20, 2^12) g/cm^3 (or not a number)");
         return GPUMCD_ERR_INVALID_ARG;
     }
     double rho_max[8];
@@ -491,7 +522,7 @@ static int create_impl(gpumcd_ctx **out, const float *density, const uint8_t *ma
         !(opt.majorant_scale >= 1.f) || opt.wave_size == 0 || opt.bank_factor == 0 || opt.warp_stack > (1u << 20) ||
         (opt.cta_threads != 0 && opt.cta_threads != 512 && opt.cta_threads != 1024) || !(opt.hom_tol >= 0.f) ||
         opt.tally_mode < 0 || opt.tally_mode > 2 || (opt.tally_mode != 0 && opt.cta_threads == 1024) ||
-        opt.table_memory < 0 || opt.table_memory > 1 || opt.bank_low > 64 ||
+        opt.table_memory < 0 || opt.table_memory > 1 || opt.bank_low > 64 || opt.l2_persist < 0 || opt.l2_persist > 1 ||
         static_cast<unsigned long long>(opt.wave_size) * opt.bank_factor > 0x7fffffffull) {
         set_error(nullptr, "bad options");
         return GPUMCD_ERR_INVALID_ARG;
@@ -531,7 +562,8 @@ static int create_impl(gpumcd_ctx **out, const float *density, const uint8_t *ma
     ctx->table_floats = static_cast<unsigned>(ctx->blob_host.size());
 
     // ---- phantom (and the majorants that depend on it) ----
-    CK(cudaMalloc(&ctx->phantom, nvox * sizeof(float2)));
+    CK(cudaMalloc(&ctx->phantom, nvox * sizeof(uint32_t)));
+    if (opt.hom_tol > 0.f) CK(cudaMalloc(&ctx->radius, nvox));
     CK(cudaMalloc(&ctx->scratch, 12 * sizeof(unsigned)));
     {
         const int rc = load_phantom(ctx, density, material, on_host);
@@ -557,12 +589,16 @@ static int create_impl(gpumcd_ctx **out, const float *density, const uint8_t *ma
         CK(cudaDeviceGetAttribute(&max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
         if (!coop) { set_error(ctx, "device does not support cooperative launches (scheduler 1)"); return GPUMCD_ERR_CUDA; }
         const size_t table_bytes = static_cast<size_t>(ctx->table_floats) * sizeof(float);
-        const int threads = opt.cta_threads == 1024 ? 1024 : 512;
+        const int threads = opt.cta_threads ? static_cast<int>(opt.cta_threads) : 512;
         const void *fn = persistent_kernel(false, opt.hom_tol > 0.f, opt.tally_mode, true, threads);
         cudaFuncAttributes fa{};
         CK(cudaFuncGetAttributes(&fa, fn));
         ctx->smem_tables = opt.table_memory == 0 && table_bytes + fa.sharedSizeBytes + 1024 <= static_cast<size_t>(max_smem);
-        const size_t dyn = ctx->smem_tables ? table_bytes : 0;
+        // behind the tables: room for a spectrum of up to kSpecSmemBins bins (cdf as double, edges as float), if it fits
+        ctx->spec_smem_bytes = 0;
+        if (ctx->smem_tables && table_bytes + kSpecSmemBytes + fa.sharedSizeBytes + 1024 <= static_cast<size_t>(max_smem))
+            ctx->spec_smem_bytes = kSpecSmemBytes;
+        const size_t dyn = ctx->smem_tables ? table_bytes + ctx->spec_smem_bytes : 0;
         fn = persistent_kernel(false, opt.hom_tol > 0.f, opt.tally_mode, ctx->smem_tables, threads);
         { const int rc = allow_dynamic_smem(ctx, fn, dyn); if (rc != GPUMCD_OK) return rc; }
         int per_sm = 0;
@@ -577,6 +613,20 @@ static int create_impl(gpumcd_ctx **out, const float *density, const uint8_t *ma
         CK(cudaMalloc(&ctx->stkB, recs * sizeof(float4)));
         CK(cudaMalloc(&ctx->stkC, recs * sizeof(uint4)));
         CK(cudaMalloc(&ctx->head, sizeof(unsigned)));
+        // l2_persist: set aside L2 for the packed phantom (the one array every move reads)
+        ctx->l2_window = 0;
+        if (opt.l2_persist == 1) {
+            int max_persist = 0, max_window = 0;
+            CK(cudaDeviceGetAttribute(&max_persist, cudaDevAttrMaxPersistingL2CacheSize, dev));
+            CK(cudaDeviceGetAttribute(&max_window, cudaDevAttrMaxAccessPolicyWindowSize, dev));
+            const size_t want = nvox * sizeof(uint32_t);
+            size_t cur = 0;
+            CK(cudaDeviceGetLimit(&cur, cudaLimitPersistingL2CacheSize));
+            const size_t carve = std::min<size_t>(want, static_cast<size_t>(max_persist));
+            if (carve > cur) CK(cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, carve)); // device-wide: only ever raised
+            ctx->l2_window = std::min<size_t>(want, static_cast<size_t>(max_window));
+            ctx->l2_hit_ratio = ctx->l2_window ? std::min(1.0f, static_cast<float>(static_cast<double>(std::max(carve, cur)) / static_cast<double>(ctx->l2_window))) : 0.f;
+        }
     }
     CK(cudaDeviceSynchronize());
     guard.ok = true;
@@ -667,9 +717,7 @@ static Params make_params(gpumcd_ctx *ctx, uint64_t seed, uint32_t hist_hi, bool
     Params P;
     P.fx_scale = ctx->fx_scale;
     P.tab = ctx->tab;
-    P.geo.phantom = ctx->phantom;
-    P.geo.nx = ctx->nx; P.geo.ny = ctx->ny; P.geo.nz = ctx->nz;
-    P.geo.h = ctx->h; P.geo.inv_h = 1.0f / ctx->h;
+    P.geo = make_geom(ctx);
     P.opt.es_max = ctx->opt.es_max_cm;
     P.opt.f_eloss = ctx->opt.f_eloss_max;
     P.opt.nudge = ctx->opt.boundary_nudge;
@@ -777,12 +825,13 @@ static int run_persistent(gpumcd_ctx *ctx, uint64_t h_begin, uint64_t n_hist, ui
         a.hist0 = h0;
         a.n_hist = static_cast<unsigned>(n);
         a.table_floats = ctx->table_floats;
+        a.spec_in_smem = (ctx->spec_smem_bytes != 0 && ctx->src.n_spec > 0 && ctx->src.n_spec <= kSpecSmemBins) ? 1 : 0;
         a.inv_h3_n = 1.0 / (h3 * static_cast<double>(n_hist));
         a.dose = dose_dev;
         a.nvox = ctx->nvox;
         a.finalize = (h0 + n == h_end) ? 1 : 0;
         // CTA size (see persistent.cuh): 512 threads unless the caller asks for 1024
-        const int threads = ctx->opt.cta_threads == 1024 ? 1024 : 512;
+        const int threads = ctx->opt.cta_threads ? static_cast<int>(ctx->opt.cta_threads) : 512;
         // banked particles of the other type that make a warp change to it: photons are cheap to work off
         // (few per batch keeps the drain short), electrons are worth a fuller batch; swept on configs 2-5
         // (bench.py --ablation): 80 / 160 with 512 threads per SM, 512 / 512 with 1024
@@ -793,10 +842,25 @@ static int run_persistent(gpumcd_ctx *ctx, uint64_t h_begin, uint64_t n_hist, ui
         // the kernel variant: trace (photon-only replay) | multi-voxel steps x tally mode; tables in shared memory; CTA size
         const bool multi = ctx->opt.hom_tol > 0.f && !trace; // a trace run tracks no electrons
         const void *fn = persistent_kernel(trace != nullptr, multi, ctx->opt.tally_mode, ctx->smem_tables, threads);
-        const size_t dyn = ctx->smem_tables ? static_cast<size_t>(ctx->table_floats) * sizeof(float) : 0;
+        const size_t dyn = ctx->smem_tables ? static_cast<size_t>(ctx->table_floats) * sizeof(float) + ctx->spec_smem_bytes : 0;
         { const int rc = allow_dynamic_smem(ctx, fn, dyn); if (rc != GPUMCD_OK) return rc; }
         { LaunchScope ls(ctx, st, CLS_ELECTRON);
-        CK(cudaLaunchCooperativeKernel(fn, dim3(ctx->p_grid), dim3(threads), args, dyn, st)); }
+        cudaLaunchConfig_t cfg{};
+        cfg.gridDim = dim3(ctx->p_grid); cfg.blockDim = dim3(threads); cfg.dynamicSmemBytes = dyn; cfg.stream = st;
+        cudaLaunchAttribute attr[2];
+        attr[0].id = cudaLaunchAttributeCooperative;
+        attr[0].val.cooperative = 1;
+        cfg.attrs = attr; cfg.numAttrs = 1;
+        if (ctx->l2_window) { // phantom reads of this launch hit a persisting carve-out of the L2
+            attr[1].id = cudaLaunchAttributeAccessPolicyWindow;
+            attr[1].val.accessPolicyWindow.base_ptr = ctx->phantom;
+            attr[1].val.accessPolicyWindow.num_bytes = ctx->l2_window;
+            attr[1].val.accessPolicyWindow.hitRatio = ctx->l2_hit_ratio;
+            attr[1].val.accessPolicyWindow.hitProp = cudaAccessPropertyPersisting;
+            attr[1].val.accessPolicyWindow.missProp = cudaAccessPropertyStreaming;
+            cfg.numAttrs = 2;
+        }
+        CK(cudaLaunchKernelExC(&cfg, fn, args)); }
         h0 += n;
     }
     return GPUMCD_OK;
@@ -906,7 +970,7 @@ extern "C" int gpumcd_run_uncertainty(gpumcd_ctx *ctx, uint64_t n_histories, uin
     }
     const double h3 = static_cast<double>(ctx->h) * ctx->h * ctx->h;
     { LaunchScope ls(ctx, st, CLS_FINALIZE);
-    k_finalize_uncertainty<<<grid, kBlock, 0, st>>>(s1, sx, sxx, ctx->phantom, nvox, 1.0 / h3,
+    k_finalize_uncertainty<<<grid, kBlock, 0, st>>>(s1, sx, sxx, make_geom(ctx), nvox, 1.0 / h3,
                                                     1.0 / static_cast<double>(n_histories), static_cast<double>(n_batches),
                                                     dose_out_dev, sigma_out_dev, ctx->edep); }
     CK(cudaGetLastError());
@@ -950,7 +1014,9 @@ extern "C" int gpumcd_get_counters(gpumcd_ctx *ctx, gpumcd_counters *out)
 extern "C" int gpumcd_get_energy_tally(gpumcd_ctx *ctx, double *edep_out_dev)
 {
     if (!ctx || !edep_out_dev) return GPUMCD_ERR_INVALID_ARG;
-    CK(cudaMemcpyAsync(edep_out_dev, ctx->edep, ctx->nvox * sizeof(double), cudaMemcpyDeviceToDevice, ctx->last_stream));
+    const int grid = static_cast<int>(std::min<size_t>((ctx->nvox + kBlock - 1) / kBlock, 148 * 8));
+    k_export_tally<<<grid, kBlock, 0, ctx->last_stream>>>(ctx->edep, make_geom(ctx), ctx->nvox, edep_out_dev);
+    CK(cudaGetLastError());
     return GPUMCD_OK;
 }
 
@@ -958,6 +1024,14 @@ extern "C" int gpumcd_set_history_offset(gpumcd_ctx *ctx, uint64_t first_history
 {
     if (!ctx) return GPUMCD_ERR_INVALID_ARG;
     ctx->hist_offset = first_history;
+    return GPUMCD_OK;
+}
+
+extern "C" int gpumcd_release_l2(gpumcd_ctx *ctx)
+{
+    if (!ctx) return GPUMCD_ERR_INVALID_ARG;
+    if (ctx->ran) CK(cudaStreamSynchronize(ctx->last_stream));
+    if (ctx->l2_window) CK(cudaCtxResetPersistingL2Cache());
     return GPUMCD_OK;
 }
 
@@ -1004,10 +1078,11 @@ extern "C" int gpumcd_probe_tally(gpumcd_ctx *ctx, uint64_t n_updates, double *u
     // once untimed (first touch of the grid), once timed
     const bool fixed = ctx->opt.tally_mode == TALLY_FIXED; // the probe adds what the run adds: fp64 or 64-bit integers
     auto probe = fixed ? k_tally_probe<true> : k_tally_probe<false>;
-    probe<<<blocks, threads, 0, st>>>(ctx->edep, ctx->nx, ctx->ny, ctx->nz, x0, y0, x1 - x0 + 1, y1 - y0 + 1,
+    const Geom geo = make_geom(ctx);
+    probe<<<blocks, threads, 0, st>>>(ctx->edep, geo, x0, y0, x1 - x0 + 1, y1 - y0 + 1,
                                       static_cast<unsigned>(per_thread), 1u);
     CK(cudaEventRecord(a, st));
-    probe<<<blocks, threads, 0, st>>>(ctx->edep, ctx->nx, ctx->ny, ctx->nz, x0, y0, x1 - x0 + 1, y1 - y0 + 1,
+    probe<<<blocks, threads, 0, st>>>(ctx->edep, geo, x0, y0, x1 - x0 + 1, y1 - y0 + 1,
                                       static_cast<unsigned>(per_thread), 2u);
     CK(cudaEventRecord(b, st));
     CK(cudaGetLastError());

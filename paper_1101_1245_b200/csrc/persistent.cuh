@@ -60,7 +60,9 @@ struct SourceDev {
 };
 
 // H0: primary of one history from block (hist, track 0, ctr 0); transport starts at ctr 1.
-__device__ __forceinline__ Particle make_primary(const Params &P, const SourceDev &S, unsigned long long hist)
+// (cdf, edges: the spectrum arrays, S.cdf / S.edges or their copies in shared memory)
+__device__ __forceinline__ Particle make_primary(const Params &P, const SourceDev &S, unsigned long long hist,
+                                                 const double *__restrict__ cdf, const float *__restrict__ edges)
 {
     Particle p;
     p.hist = static_cast<uint32_t>(hist);
@@ -83,17 +85,29 @@ __device__ __forceinline__ Particle make_primary(const Params &P, const SourceDe
     p.u = 0.0f; p.v = 0.0f; p.w = 1.0f;
     double E = S.energy;
     if (S.n_spec > 0) {
-        const double target = static_cast<double>(u01(w.z)) * S.cdf[S.n_spec];
+        const double target = static_cast<double>(u01(w.z)) * cdf[S.n_spec];
         int lo = 0, hi = S.n_spec - 1; // largest j with cdf[j] <= target, clamped to n_spec-1
         while (lo < hi) {
             const int mid = (lo + hi + 1) >> 1;
-            if (S.cdf[mid] <= target) lo = mid; else hi = mid - 1;
+            if (cdf[mid] <= target) lo = mid; else hi = mid - 1;
         }
-        const double e0 = S.edges[lo], e1 = S.edges[lo + 1];
+        const double e0 = edges[lo], e1 = edges[lo + 1];
         E = e0 + static_cast<double>(u01(w.w)) * (e1 - e0);
     }
     p.E = static_cast<float>(E);
     return p;
+}
+
+__device__ __forceinline__ Particle make_primary(const Params &P, const SourceDev &S, unsigned long long hist)
+{
+    return make_primary(P, S, hist, S.cdf, S.edges);
+}
+
+// the kernel's dynamic shared memory: [table blob | spectrum cdf (double) | spectrum edges (float)]
+__device__ __forceinline__ float *dyn_smem()
+{
+    extern __shared__ __align__(128) float dyn_smem_base[];
+    return dyn_smem_base;
 }
 
 // ---- TMA bulk copy of the table blob into shared memory (G7) --------------------------------
@@ -146,6 +160,7 @@ struct PersistArgs {
     unsigned long long hist0;      // first history of the launch (low word never wraps inside a launch)
     unsigned n_hist;               // histories of the launch (< 2^32)
     unsigned table_floats;         // length of the table blob, padded to a multiple of 4 floats
+    int spec_in_smem;              // the spectrum's cdf and bin edges are copied into shared memory behind the tables
     double inv_h3_n;
     float *dose;                   // or nullptr
     size_t nvox;
@@ -242,7 +257,15 @@ struct Warp {
         bool on = lane < k;
         Particle q;
         if (on) {
-            q = make_primary(a.P, a.S, a.hist0 + (cl.next + lane));
+            // the spectrum arrays: their shared-memory copies if the kernel staged them (512 bins: nine dependent
+            // look-ups per primary, which were 3 % of config 5's stall samples from global memory)
+            const double *cdf = a.S.cdf;
+            const float *edges = a.S.edges;
+            if (a.spec_in_smem) {
+                cdf = reinterpret_cast<const double *>(dyn_smem() + a.table_floats);
+                edges = reinterpret_cast<const float *>(cdf + (a.S.n_spec + 1));
+            }
+            q = make_primary(a.P, a.S, a.hist0 + (cl.next + lane), cdf, edges);
             *e_inc += static_cast<double>(q.E);
             if (s == SK_ES && !electron_tracked(a.P, q.E)) { // below the cutoff (or photon_only): deposited where it is born
                 deposit<V>(a.P, voxel_index(a.P.geo, q), q.E);
@@ -449,7 +472,7 @@ __device__ __forceinline__ int photon_mode(const PersistArgs &a, const float *__
 template <class V, bool SMEM_TABLES, int kPThreads>
 __global__ void __launch_bounds__(kPThreads, 1) k_persistent(const __grid_constant__ PersistArgs a)
 {
-    extern __shared__ __align__(128) float smem[];
+    float *smem = dyn_smem();
     constexpr int kPWarps = kPThreads / 32;
     __shared__ uint64_t bar;
     __shared__ WarpCtl s_ctl[kPWarps];
@@ -461,6 +484,15 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(const __grid_consta
     if (SMEM_TABLES) {
         stage_tables(smem, P.tab.blob, a.table_floats, &bar);
         TB = smem;
+        if (a.spec_in_smem) {
+            double *sc = reinterpret_cast<double *>(smem + a.table_floats);
+            float *se = reinterpret_cast<float *>(sc + (a.S.n_spec + 1));
+            for (int i = threadIdx.x; i <= a.S.n_spec; i += kPThreads) {
+                sc[i] = a.S.cdf[i];
+                se[i] = a.S.edges[i];
+            }
+            __syncthreads();
+        }
     }
     const unsigned lane = threadIdx.x & 31;
     const size_t gwarp = (blockIdx.x * static_cast<size_t>(blockDim.x) + threadIdx.x) >> 5;
@@ -507,7 +539,7 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(const __grid_consta
         const double e = tally_value<V::TALLY>(P, i);
         s += e;
         if (V::TALLY == TALLY_FIXED) P.edep[i] = e; // from here on the tally holds MeV as fp64, whatever the mode
-        if (a.dose) a.dose[i] = static_cast<float>(e / static_cast<double>(P.geo.phantom[i].x) * a.inv_h3_n);
+        if (a.dose) a.dose[caller_index(P.geo, i)] = static_cast<float>(e / static_cast<double>(unpack_voxel(P.geo.phantom[i]).x) * a.inv_h3_n);
     }
     s = wsum(s);
     __shared__ double part[kPWarps];

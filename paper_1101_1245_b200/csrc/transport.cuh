@@ -28,7 +28,8 @@ struct Tables {
 };
 
 struct Geom {
-    const float2 *phantom; // {density, material id as int bits} per voxel
+    const uint32_t *phantom; // packed {density, material id}, 4 bytes per voxel (pack_voxel_record)
+    const uint8_t *radius;   // multi-voxel steps only (else nullptr): the uniform radius of every voxel
     int nx, ny, nz;
     float h, inv_h;
 };
@@ -98,12 +99,34 @@ struct Acc {
     __device__ __forceinline__ void inc(double e) const { atomicAdd(&slot()->e_inc, e); }
 };
 
-// Phantom record: x = density, y = bits: material id in the low 8 bits; bits 8-10 (multi-voxel steps
-// only, else 0) = the uniform radius R of the voxel: every voxel within Chebyshev distance R continues
-// its medium (same material, density within hom_tol), so no ray from inside it meets a change of
-// medium before R voxel sizes.
-__device__ __forceinline__ int mat_of(float2 pv) { return __float_as_int(pv.y) & 0xff; }
-__device__ __forceinline__ int radius_of(float2 pv) { return (__float_as_int(pv.y) >> 8) & 7; }
+// Phantom record, 4 bytes per voxel (half of {float density, int material}: the phantom is fetched at every move,
+// PAPER.md L168, and a warp waits for the slowest of its 32 fetches, so what matters is that the whole phantom
+// stays in L2).  Lossless: a density is a positive finite float, so its sign bit is 0, and with its biased
+// exponent in [kExpLo, kExpLo + 32), i.e. 2^-20 <= rho < 2^12 g/cm^3 (checked when the phantom is loaded), three
+// exponent bits are free too:  bits 0-27 = (exponent - kExpLo) << 23 | mantissa,  bits 28-31 = material id.
+constexpr uint32_t kExpLo = 107u;
+struct Voxel {
+    float x; // density, g/cm^3 (bit for bit the caller's)
+    int m;   // material id
+};
+__host__ __device__ __forceinline__ bool density_packable(uint32_t float_bits)
+{
+    const uint32_t e = float_bits >> 23; // sign bit included: a negative number fails too
+    return e >= kExpLo && e < kExpLo + 32u;
+}
+__host__ __device__ __forceinline__ uint32_t pack_voxel_record(uint32_t float_bits, int m)
+{
+    return (float_bits - (kExpLo << 23)) | (static_cast<uint32_t>(m) << 28);
+}
+__device__ __forceinline__ Voxel unpack_voxel(uint32_t b)
+{
+    return Voxel{__uint_as_float((b & 0x0fffffffu) + (kExpLo << 23)), static_cast<int>(b >> 28)};
+}
+__device__ __forceinline__ Voxel fetch_voxel(const Geom &g, unsigned lin) { return unpack_voxel(__ldg(&g.phantom[lin])); }
+__device__ __forceinline__ int mat_of(Voxel pv) { return pv.m; }
+// Multi-voxel steps: the uniform radius R of a voxel (0-7): every voxel within Chebyshev distance R continues
+// its medium (same material, density within hom_tol), so no ray from inside it meets a change of medium before
+// R voxel sizes.
 
 __device__ __forceinline__ bool inside(const Geom &g, const Particle &p)
 {
@@ -111,11 +134,19 @@ __device__ __forceinline__ bool inside(const Geom &g, const Particle &p)
            (static_cast<unsigned>(p.iy) < static_cast<unsigned>(g.ny)) &
            (static_cast<unsigned>(p.iz) < static_cast<unsigned>(g.nz));
 }
-__device__ __forceinline__ unsigned voxel_index(const Geom &g, const Particle &p)
+// Internal layout of the library's volumes (phantom, tally, radius): the caller's, x fastest,
+// lin = ix + nx (iy + ny iz); <= 2^30 voxels.  These two functions are the only place that knows it.
+// (Measured alternative: z fastest, the beam axis, so that consecutive steps of a track share 32-byte sectors:
+// 1 % on config 5, nothing on configs 2-4, and a pencil beam (config 1) then piles its deposits onto a few
+// sectors of one column, whose atomics serialise: 0.155 -> 0.28 ms.  Dropped.)
+__device__ __forceinline__ unsigned lin_of(const Geom &g, int ix, int iy, int iz)
 {
-    return static_cast<unsigned>(p.ix) + static_cast<unsigned>(g.nx) * (static_cast<unsigned>(p.iy) +
-           static_cast<unsigned>(g.ny) * static_cast<unsigned>(p.iz)); // <= 2^30 voxels
+    return static_cast<unsigned>(ix) + static_cast<unsigned>(g.nx) * (static_cast<unsigned>(iy) +
+           static_cast<unsigned>(g.ny) * static_cast<unsigned>(iz));
 }
+__device__ __forceinline__ unsigned voxel_index(const Geom &g, const Particle &p) { return lin_of(g, p.ix, p.iy, p.iz); }
+// internal index t -> index in the caller's [nz][ny][nx] arrays
+__device__ __forceinline__ size_t caller_index(const Geom &, size_t t) { return t; }
 
 // H4/H8 tally into the L2-resident energy grid (the paper only says the dose arrays "are summed", L188):
 //   TALLY_F64   one fp64 atomic add per lane (RED.E.ADD.F64, resolved in L2);
@@ -278,7 +309,7 @@ __device__ __forceinline__ int photon_flight(const Params &P, const float *__res
         record<V>(P, p, 4);
         return PM_DEAD;
     }
-    const float2 pv = __ldg(&P.geo.phantom[voxel_index(P.geo, p)]);
+    const Voxel pv = fetch_voxel(P.geo, voxel_index(P.geo, p));
     const float rho = pv.x;
     const float *col = TB + mat_of(pv) * 3 * tb.gE.n;
     const float r = u01(w.y) * mu_max;
@@ -442,10 +473,10 @@ __device__ __forceinline__ float exit_distance(float fx, float fy, float fz, flo
 // d_hom: distance along the direction to the first voxel that does not continue the start voxel's
 // medium (other material, density off by more than hom_tol, outside the phantom); +inf if none
 // within s_max.
-__device__ __forceinline__ float hom_distance(const Params &P, const Particle &p, float2 pv0, float s_max)
+__device__ __forceinline__ float hom_distance(const Params &P, const Particle &p, unsigned lin0, Voxel pv0, float s_max)
 {
     // the voxel's uniform radius (precomputed per phantom) answers most look-aheads without a walk
-    if (s_max < static_cast<float>(radius_of(pv0))) return __int_as_float(0x7f800000);
+    if (s_max < static_cast<float>(__ldg(&P.geo.radius[lin0]))) return __int_as_float(0x7f800000);
     float fx = p.fx, fy = p.fy, fz = p.fz, t = 0.0f;
     int ix = p.ix, iy = p.iy, iz = p.iz;
     const float band = P.opt.hom_tol * pv0.x;
@@ -461,8 +492,7 @@ __device__ __forceinline__ float hom_distance(const Params &P, const Particle &p
         if (static_cast<unsigned>(ix) >= static_cast<unsigned>(P.geo.nx) ||
             static_cast<unsigned>(iy) >= static_cast<unsigned>(P.geo.ny) ||
             static_cast<unsigned>(iz) >= static_cast<unsigned>(P.geo.nz)) return t;
-        const float2 pv = __ldg(&P.geo.phantom[static_cast<unsigned>(ix) + static_cast<unsigned>(P.geo.nx) *
-                                               (static_cast<unsigned>(iy) + static_cast<unsigned>(P.geo.ny) * static_cast<unsigned>(iz))]);
+        const Voxel pv = fetch_voxel(P.geo, lin_of(P.geo, ix, iy, iz));
         if (mat_of(pv) != mat_of(pv0) || fabsf(pv.x - pv0.x) > band) return t;
     }
     return t;
@@ -477,8 +507,7 @@ __device__ __forceinline__ unsigned voxel_ahead(const Geom &g, const Particle &p
     const int iz = p.iz + static_cast<int>(floorf(fmaf(t, p.w, p.fz)));
     const bool in = (static_cast<unsigned>(ix) < static_cast<unsigned>(g.nx)) & (static_cast<unsigned>(iy) < static_cast<unsigned>(g.ny)) &
                     (static_cast<unsigned>(iz) < static_cast<unsigned>(g.nz));
-    return in ? static_cast<unsigned>(ix) + static_cast<unsigned>(g.nx) * (static_cast<unsigned>(iy) + static_cast<unsigned>(g.ny) * static_cast<unsigned>(iz))
-              : fallback;
+    return in ? lin_of(g, ix, iy, iz) : fallback;
 }
 
 template <class V>
@@ -489,7 +518,7 @@ __device__ __forceinline__ int electron_step(const Params &P, const float *__res
     const Tables &tb = P.tab;
     const int nE = tb.gE.n;
     const unsigned lin = voxel_index(P.geo, p);
-    const float2 pv = __ldg(&P.geo.phantom[lin]);
+    const Voxel pv = fetch_voxel(P.geo, lin);
     const float rho = pv.x;
     const float *el = TB + tb.off_el + mat_of(pv) * 4 * nE;
     const float T = p.E;
@@ -509,7 +538,7 @@ __device__ __forceinline__ int electron_step(const Params &P, const float *__res
     const float e_cap = fminf(P.opt.es_max, fdiv(P.opt.f_eloss * T, L0));
     float d_vox;
     if (V::MULTI) // R32: the boundary that limits the step is the next change of medium along d
-        d_vox = (hom_distance(P, p, pv, fminf(e_hard, e_cap) * P.geo.inv_h) + P.opt.nudge) * P.geo.h;
+        d_vox = (hom_distance(P, p, lin, pv, fminf(e_hard, e_cap) * P.geo.inv_h) + P.opt.nudge) * P.geo.h;
     else
         d_vox = (fminf(dx, fminf(dy, dz)) + P.opt.nudge) * P.geo.h;
     // Eq. 4
@@ -582,7 +611,7 @@ __device__ __forceinline__ int electron_hard(const Params &P, const float *__res
     const int nE = tb.gE.n;
     const uint4 b = draw(P.rng, p);
     const unsigned lin1 = voxel_index(P.geo, p);
-    const float2 pv1 = __ldg(&P.geo.phantom[lin1]);
+    const Voxel pv1 = fetch_voxel(P.geo, lin1);
     const float *el1 = TB + tb.off_el + mat_of(pv1) * 4 * nE;
     const Interp i1 = locate(tb.gE, lnT);
     const float T1 = p.E;
