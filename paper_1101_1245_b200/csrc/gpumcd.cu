@@ -84,6 +84,7 @@ __global__ void k_source(Params P, SourceDev S, Queue q, unsigned long long hist
 {
     const unsigned i = blockIdx.x * blockDim.x + threadIdx.x;
     const Acc acc(P);
+    acc_init();
     double e_inc = 0.0;
     if (i < n) {
         Particle p = make_primary(P, S, hist0 + i);
@@ -96,8 +97,7 @@ __global__ void k_source(Params P, SourceDev S, Queue q, unsigned long long hist
         }
         store_rec(q.A, q.B, q.C, i, p, 0u);
     }
-    e_inc = wsum(e_inc);
-    if ((threadIdx.x & 31) == 0 && e_inc != 0.0) acc.inc(e_inc);
+    acc_flush(P, e_inc);
     if (i == 0) *q.count = n;
 }
 
@@ -110,6 +110,7 @@ __global__ void __launch_bounds__(kBlock) k_photon_pass(Params P, Queue in, unsi
 {
     const unsigned i = blockIdx.x * blockDim.x + threadIdx.x;
     Local L;
+    acc_init();
     if (i < n_in) {
         uint32_t extra;
         const Particle p = load_rec(in.A, in.B, in.C, i, extra);
@@ -123,6 +124,7 @@ __global__ void __launch_bounds__(kBlock) k_electron_pass(Params P, Queue in, un
 {
     const unsigned i = blockIdx.x * blockDim.x + threadIdx.x;
     Local L;
+    acc_init();
     if (i < n_in) {
         uint32_t extra;
         const Particle p = load_rec(in.A, in.B, in.C, i, extra);
@@ -1004,8 +1006,8 @@ extern "C" int gpumcd_get_counters(gpumcd_ctx *ctx, gpumcd_counters *out)
         out->e_incident += d.slot[k].e_inc;
         out->e_dep_cutoff += d.slot[k].e_cut;
         out->e_escaped += d.slot[k].e_esc;
-        out->e_pair_rest += d.slot[k].e_pair;
     }
+    out->e_pair_rest = static_cast<double>(d.photon_pair) * (2.0 * static_cast<double>(kMe)); // 2 m c^2 per pair event (R6)
     out->e_dep_continuous = d.e_dep_total - out->e_dep_cutoff;
     if (d.overflow) { set_error(ctx, "particle queue overflow: the result is invalid"); return GPUMCD_ERR_BANK_OVERFLOW; }
     return GPUMCD_OK;

@@ -510,6 +510,7 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(const __grid_consta
     w.ctl = &s_ctl[threadIdx.x >> 5];
     w.e_inc = &s_einc[threadIdx.x];
     s_einc[threadIdx.x] = 0.0;
+    acc_init();
     if (lane < WC_N) w.ctl->wc[lane] = 0u;
     __syncwarp();
 
@@ -525,11 +526,8 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(const __grid_consta
         const unsigned v = w.ctl->wc[lane];
         if (v) atomicAdd(&P.cnt->photon_flights + lane, static_cast<unsigned long long>(v));
     }
-    const double e_new = wsum(s_einc[threadIdx.x]);
-    if (lane == 0) {
-        if (e_new != 0.0) Acc(P).inc(e_new);
-        if (w.hw) atomicMax(&P.cnt->high_water, static_cast<unsigned long long>(w.hw));
-    }
+    acc_flush(P, s_einc[threadIdx.x]);
+    if (lane == 0 && w.hw) atomicMax(&P.cnt->high_water, static_cast<unsigned long long>(w.hw));
     if (!a.finalize) return;
     grid.sync();
     // ---- H8 finalize: dose = energy / mass / histories, and the total deposited energy

@@ -59,8 +59,8 @@ struct Queue {
 };
 
 constexpr int kEnergySlots = 64;
-struct EnergySlot { // energy accounts, spread over slots so that the atomics do not pile on one address
-    double e_esc, e_cut, e_pair, e_inc;
+struct EnergySlot { // energy accounts in global memory, spread over slots so that the flushes do not pile on one address
+    double e_esc, e_cut, e_inc;
 };
 struct DevCounters {
     unsigned long long photon_flights, photon_compton, photon_photo, photon_pair, photon_fict;
@@ -84,20 +84,31 @@ struct Params {
     unsigned long long trace_off; // id of the run's first history
 };
 
-// energy accounts of the calling warp (rare events: the slot address is recomputed at every use
-// instead of being kept in registers)
+// Energy accounts (escaped, deposited below a cutoff): every thread adds into its own two fp64 slots in shared
+// memory, and a kernel flushes them once at its end (acc_flush).  They used to be fp64 atomics on 64 slots in
+// global memory, one per escape / cutoff deposit: a few 1e8 atomics per run on 2 KB, i.e. on one L2 slice, whose
+// queue then held up every other request of the SMs (config 5: the phantom loads waited ~3000 cycles).
+constexpr int kAccThreads = 1024; // largest CTA of any kernel that uses the accounts
 struct Acc {
-    DevCounters *cnt;
-    __device__ __forceinline__ explicit Acc(const Params &P) : cnt(P.cnt) {}
-    __device__ __forceinline__ EnergySlot *slot() const
+    __device__ __forceinline__ explicit Acc(const Params &) {}
+    static __device__ __forceinline__ double *slots()
     {
-        return &cnt->slot[((blockIdx.x * blockDim.x + threadIdx.x) >> 5) & (kEnergySlots - 1)];
+        __shared__ double s_acc[2 * kAccThreads];
+        return s_acc;
     }
-    __device__ __forceinline__ void esc(float e) const { atomicAdd(&slot()->e_esc, static_cast<double>(e)); }
-    __device__ __forceinline__ void cut(float e) const { atomicAdd(&slot()->e_cut, static_cast<double>(e)); }
-    __device__ __forceinline__ void pair() const { atomicAdd(&slot()->e_pair, 2.0 * static_cast<double>(kMe)); }
-    __device__ __forceinline__ void inc(double e) const { atomicAdd(&slot()->e_inc, e); }
+    __device__ __forceinline__ void esc(float e) const { slots()[threadIdx.x] += static_cast<double>(e); }
+    __device__ __forceinline__ void cut(float e) const { slots()[kAccThreads + threadIdx.x] += static_cast<double>(e); }
 };
+// all threads of the CTA, before any transport code runs
+__device__ __forceinline__ void acc_init()
+{
+    Acc::slots()[threadIdx.x] = 0.0;
+    Acc::slots()[kAccThreads + threadIdx.x] = 0.0;
+}
+__device__ __forceinline__ EnergySlot *energy_slot(const Params &P)
+{
+    return &P.cnt->slot[((blockIdx.x * blockDim.x + threadIdx.x) >> 5) & (kEnergySlots - 1)];
+}
 
 // Phantom record, 4 bytes per voxel (half of {float density, int material}: the phantom is fetched at every move,
 // PAPER.md L168, and a warp waits for the slowest of its 32 fetches, so what matters is that the whole phantom
@@ -420,7 +431,6 @@ __device__ __forceinline__ int photon_interact(const Params &P, Particle &p, int
         deposit<V>(P, lin, T2);
         acc.cut(T2);
     }
-    acc.pair();
     if (P.opt.pair_mode == 1) {
         c.E = kMe;
         c.u = ax; c.v = ay; c.w = az; c.track = id.z;
@@ -740,13 +750,28 @@ __device__ __forceinline__ double wsum(double v)
     for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
     return v;
 }
+// all 32 lanes of every warp, after the transport code: the warp's energy accounts (and e_inc, its share of the
+// primaries' energy) go to the global slots with one atomic each
+__device__ __forceinline__ void acc_flush(const Params &P, double e_inc)
+{
+    const double esc = wsum(Acc::slots()[threadIdx.x]);
+    const double cut = wsum(Acc::slots()[kAccThreads + threadIdx.x]);
+    e_inc = wsum(e_inc);
+    if ((threadIdx.x & 31) == 0) {
+        EnergySlot *s = energy_slot(P);
+        if (esc != 0.0) atomicAdd(&s->e_esc, esc);
+        if (cut != 0.0) atomicAdd(&s->e_cut, cut);
+        if (e_inc != 0.0) atomicAdd(&s->e_inc, e_inc);
+    }
+}
 __device__ __forceinline__ void bump(unsigned long long *c, unsigned v)
 {
     if (v) atomicAdd(c, static_cast<unsigned long long>(v));
 }
 // all 32 lanes of every warp must call this
-__device__ void flush(const Params &P, const Local &L)
+__device__ void flush(const Params &P, const Local &L, double e_inc = 0.0)
 {
+    acc_flush(P, e_inc);
     const unsigned f = wsum(L.flights), c = wsum(L.compton), ph = wsum(L.photo), pr = wsum(L.pair), fi = wsum(L.fict);
     const unsigned st = wsum(L.steps), mo = wsum(L.moller), br = wsum(L.brems), hf = wsum(L.hfict);
     if ((threadIdx.x & 31) == 0) {
