@@ -411,7 +411,7 @@ static void destroy_impl(gpumcd_ctx *c)
 template <class V>
 static const void *persistent_variant(bool smem, int threads)
 {
-    if (threads == 512) return smem ? (const void *)k_persistent<V, true, 512> : (const void *)k_persistent<V, false, 512>;
+    if (threads == kPThreadsDefault) return smem ? (const void *)k_persistent<V, true, kPThreadsDefault> : (const void *)k_persistent<V, false, kPThreadsDefault>;
     if (V::TALLY == TALLY_F64) return smem ? (const void *)k_persistent<Variant<V::TRACE, V::MULTI, TALLY_F64>, true, 1024>
                                            : (const void *)k_persistent<Variant<V::TRACE, V::MULTI, TALLY_F64>, false, 1024>;
     return nullptr;
@@ -522,7 +522,7 @@ static int create_impl(gpumcd_ctx **out, const float *density, const uint8_t *ma
     if (opt_in) opt = *opt_in;
     if (!(opt.es_max_cm > 0.f) || !(opt.f_eloss_max > 0.f) || opt.f_eloss_max > 1.f || opt.boundary_nudge < 0.f ||
         !(opt.majorant_scale >= 1.f) || opt.wave_size == 0 || opt.bank_factor == 0 || opt.warp_stack > (1u << 20) ||
-        (opt.cta_threads != 0 && opt.cta_threads != 512 && opt.cta_threads != 1024) || !(opt.hom_tol >= 0.f) ||
+        (opt.cta_threads != 0 && opt.cta_threads != kPThreadsDefault && opt.cta_threads != 1024) || !(opt.hom_tol >= 0.f) ||
         opt.tally_mode < 0 || opt.tally_mode > 2 || (opt.tally_mode != 0 && opt.cta_threads == 1024) ||
         opt.table_memory < 0 || opt.table_memory > 1 || opt.bank_low > 64 || opt.l2_persist < 0 || opt.l2_persist > 1 ||
         static_cast<unsigned long long>(opt.wave_size) * opt.bank_factor > 0x7fffffffull) {
@@ -591,7 +591,7 @@ static int create_impl(gpumcd_ctx **out, const float *density, const uint8_t *ma
         CK(cudaDeviceGetAttribute(&max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
         if (!coop) { set_error(ctx, "device does not support cooperative launches (scheduler 1)"); return GPUMCD_ERR_CUDA; }
         const size_t table_bytes = static_cast<size_t>(ctx->table_floats) * sizeof(float);
-        const int threads = opt.cta_threads ? static_cast<int>(opt.cta_threads) : 512;
+        const int threads = opt.cta_threads ? static_cast<int>(opt.cta_threads) : kPThreadsDefault;
         const void *fn = persistent_kernel(false, opt.hom_tol > 0.f, opt.tally_mode, true, threads);
         cudaFuncAttributes fa{};
         CK(cudaFuncGetAttributes(&fa, fn));
@@ -833,12 +833,12 @@ static int run_persistent(gpumcd_ctx *ctx, uint64_t h_begin, uint64_t n_hist, ui
         a.nvox = ctx->nvox;
         a.finalize = (h0 + n == h_end) ? 1 : 0;
         // CTA size (see persistent.cuh): 512 threads unless the caller asks for 1024
-        const int threads = ctx->opt.cta_threads ? static_cast<int>(ctx->opt.cta_threads) : 512;
+        const int threads = ctx->opt.cta_threads ? static_cast<int>(ctx->opt.cta_threads) : kPThreadsDefault;
         // banked particles of the other type that make a warp change to it: photons are cheap to work off
         // (few per batch keeps the drain short), electrons are worth a fuller batch; swept on configs 2-5
         // (bench.py --ablation): 80 / 160 with 512 threads per SM, 512 / 512 with 1024
-        a.high_g = ctx->opt.bank_high_g ? ctx->opt.bank_high_g : (threads == 512 ? 80u : 512u);
-        a.high_e = ctx->opt.bank_high_e ? ctx->opt.bank_high_e : (threads == 512 ? 160u : 512u);
+        a.high_g = ctx->opt.bank_high_g ? ctx->opt.bank_high_g : (threads != 1024 ? 80u : 512u);
+        a.high_e = ctx->opt.bank_high_e ? ctx->opt.bank_high_e : (threads != 1024 ? 160u : 512u);
         a.low = ctx->opt.bank_low ? ctx->opt.bank_low : kLowDefault;
         void *args[] = {&a};
         // the kernel variant: trace (photon-only replay) | multi-voxel steps x tally mode; tables in shared memory; CTA size

@@ -33,6 +33,10 @@ namespace cg = cooperative_groups;
 // per-lane backlog when the source runs dry is half that of 1024 threads).  The 1024-thread build (64
 // registers, spills, twice the warps to hide latency) is kept as an option for the ablation: it was the
 // faster one for photon beams in heterogeneous phantoms until the fast-math build shrank the code.
+#ifndef GPUMCD_PT
+#define GPUMCD_PT 512
+#endif
+constexpr int kPThreadsDefault = GPUMCD_PT;
 constexpr int kPThreadsMax = 1024;
 constexpr unsigned kFull = 0xffffffffu;
 constexpr unsigned kChunk = 32;            // primaries a warp claims per atomic on the source head

@@ -33,6 +33,15 @@ __device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_
     }
     return make_uint4(c0, c1, c2, c3);
 }
+// The same as ONE out-of-line copy, for the call sites outside the step / flight code (rejection loops, vertices,
+// lineage, primaries): a dozen inlined copies of the 75-instruction block made the persistent kernel 90 KB of
+// SASS, more than the 32 KB instruction cache of an SM holds when its warps work on different event kinds
+// (config 5: `no_instruction` was 17 % of the stall cycles).
+__device__ __noinline__ uint4 philox4x32_10_call(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                                 uint32_t k0, uint32_t k1)
+{
+    return philox4x32_10(c0, c1, c2, c3, k0, k1);
+}
 
 // U(w) = ((w >> 9) + 1/2) 2^-23 in (0,1); exact in fp32 (Eq. 1 needs zeta in (0,1], L53).
 __device__ __forceinline__ float u01(uint32_t w)
@@ -161,16 +170,19 @@ __device__ __forceinline__ void rotate(float u, float v, float w, float cost, fl
 struct Rng {
     uint32_t k0, k1, hist_hi;
 };
+// the particle's next block; HOT: the inlined copy (step and flight code), else the shared out-of-line one
+template <bool HOT = false>
 __device__ __forceinline__ uint4 draw(const Rng &g, Particle &p)
 {
-    const uint4 r = philox4x32_10(p.hist, g.hist_hi, p.track, p.ctr, g.k0, g.k1);
+    const uint4 r = HOT ? philox4x32_10(p.hist, g.hist_hi, p.track, p.ctr, g.k0, g.k1)
+                        : philox4x32_10_call(p.hist, g.hist_hi, p.track, p.ctr, g.k0, g.k1);
     p.ctr += 1u;
     return r;
 }
 // track ids of the children born at the parent's current counter
 __device__ __forceinline__ uint4 lineage(const Rng &g, const Particle &p)
 {
-    return philox4x32_10(p.hist, g.hist_hi, p.track, p.ctr | 0x80000000u, g.k0, g.k1);
+    return philox4x32_10_call(p.hist, g.hist_hi, p.track, p.ctr | 0x80000000u, g.k0, g.k1);
 }
 
 // ---------------------------------------------------------------------------------------------

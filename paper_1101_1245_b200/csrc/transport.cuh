@@ -310,7 +310,7 @@ template <class V>
 __device__ __forceinline__ int photon_flight(const Params &P, const float *__restrict__ TB, Particle &p)
 {
     const Tables &tb = P.tab;
-    const uint4 w = draw(P.rng, p);
+    const uint4 w = draw<true>(P.rng, p);
     const Interp iE = locate(tb.gE, flog(p.E));
     const float mu_max = interp(TB + tb.off_mu, iE);
     const float s = fdiv(-flog(u01(w.x)), mu_max);
@@ -532,7 +532,7 @@ __device__ __forceinline__ int electron_step(const Params &P, const float *__res
     const float rho = pv.x;
     const float *el = TB + tb.off_el + mat_of(pv) * 4 * nE;
     const float T = p.E;
-    const uint4 a = draw(P.rng, p);
+    const uint4 a = draw<true>(P.rng, p);
     const Interp iT = locate(tb.gE, lnT);
     // distance to the next hard event: Woodcock with the majorant at the step-start energy (L110-113);
     // M = 0 gives +inf (no hard events possible)
