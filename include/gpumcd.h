@@ -137,14 +137,25 @@ typedef struct {
 } gpumcd_options;
 
 typedef struct {
-    int32_t particle;    /* 0 photon, 1 electron */
-    int32_t shape;       /* 0 pencil beam, 1 parallel rectangular field */
+    int32_t particle;    /* 0 photon, 1 electron (shapes 0 and 1; a phase space carries the type per record) */
+    int32_t shape;       /* 0 pencil beam, 1 parallel rectangular field, 2 phase space */
     float cx, cy;        /* field centre on the z = 0 face, cm */
     float wx, wy;        /* full field widths, cm (ignored for a pencil beam) */
     float energy;        /* MeV, used when n_spec == 0 */
     int32_t n_spec;      /* number of spectrum bins, 0 = monoenergetic */
     const float *spec_E; /* HOST, n_spec+1 bin edges, MeV, increasing */
     const float *spec_w; /* HOST, n_spec non-negative bin weights; energy is uniform inside a bin */
+    /* shape 2, a phase space (the paper's future work beside spectrum sources): n_phsp records of
+     * 8 floats {x, y, z (cm, phantom frame), u, v, w (unit direction, used as given), E (MeV, kinetic for an
+     * electron), type (0.0 photon, 1.0 electron)}.  History h starts from record h mod n_phsp, exactly as given
+     * (no random number is drawn for the primary; its transport starts at draw counter 1 like every other
+     * primary).  A record outside the phantom counts as escaped at birth, one below its type's cutoff is
+     * deposited where it is (R5, R35).  gpumcd_set_source copies the records (library-owned) and checks
+     * them: type 0 or 1, finite numbers, E inside the energy range of the tables (GPUMCD_ERR_TABLE_RANGE).
+     * cx .. spec_w are ignored. */
+    uint64_t n_phsp;
+    const float *phsp;     /* n_phsp x 8 floats: DEVICE memory, or HOST memory if phsp_on_host != 0 */
+    int32_t phsp_on_host;
 } gpumcd_source;
 
 typedef struct {

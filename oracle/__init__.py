@@ -36,7 +36,8 @@ class _Source(C.Structure):
     _fields_ = [("particle", C.c_int32), ("shape", C.c_int32),
                 ("cx", C.c_double), ("cy", C.c_double), ("wx", C.c_double), ("wy", C.c_double),
                 ("energy", C.c_double), ("n_spec", C.c_int32),
-                ("spec_E", C.c_void_p), ("spec_w", C.c_void_p)]
+                ("spec_E", C.c_void_p), ("spec_w", C.c_void_p),
+                ("n_phsp", C.c_int64), ("phsp", C.c_void_p)]
 
 
 class Counters(C.Structure):
@@ -103,9 +104,14 @@ def _source_c(src):
         keep = (e, w)
         n_spec = int(w.size)
         pe, pw = _p(e), _p(w)
+    n_phsp, pp = 0, None
+    if getattr(src, "phsp", None) is not None:
+        ps = np.ascontiguousarray(src.phsp, np.float32).reshape(-1, 8)
+        keep = keep + (ps,)
+        n_phsp, pp = int(ps.shape[0]), _p(ps)
     f32 = lambda v: float(np.float32(v))   # the boundary (include/gpumcd.h) carries these as float32
     s = _Source(src.particle, src.shape, f32(src.cx), f32(src.cy), f32(src.wx), f32(src.wy), f32(src.energy),
-                n_spec, pe, pw)
+                n_spec, pe, pw, n_phsp, pp)
     return s, keep
 
 

@@ -826,6 +826,18 @@ static void electron_history(world_t *W, particle_t p)
 /* ---------------- source (PAPER.md L166 initParticle; R17) ---------------- */
 static int make_primary(world_t *W, const orc_source *src, const double *cdf, particle_t *p)
 {
+    if (src->shape == 2) {
+        /* phase space (R35): record h mod n, exactly as given; no draw is made
+         * for the primary and its transport starts at counter 1 like every other primary's */
+        const float *r = src->phsp + 8 * (size_t)(W->hist % (uint64_t)src->n_phsp);
+        p->type = r[7] != 0.0f;
+        for (int k = 0; k < 3; ++k) { p->x[k] = (double)r[k]; p->d[k] = (double)r[3 + k]; }
+        p->E = (double)r[6];
+        p->track = 0;
+        p->ctr = 1;
+        p->primary = 1;
+        return 0;
+    }
     stream_t s = make_stream(W->seed, W->hist, 0, 0);
     uint32_t w[4];
     draw(&s, w);
@@ -869,7 +881,14 @@ static int run_impl(const float *density, const uint8_t *material, int32_t nx, i
     if (!density || !material || !t || !opt || !src || !edep_out) return -1;
     if (nx <= 0 || ny <= 0 || nz <= 0 || voxel_cm <= 0.0) return -1;
     if (t->n_materials <= 0 || t->n_energy < 2 || t->e_cut < t->e_min) return -1;
-    if (src->n_spec == 0 && (src->energy > t->e_max || src->energy < t->e_min)) return -1;
+    if (src->shape == 2) {
+        if (src->n_phsp <= 0 || !src->phsp) return -1;
+        for (int64_t i = 0; i < src->n_phsp; ++i) {
+            const float *r = src->phsp + 8 * (size_t)i;
+            if (!(r[7] == 0.0f || r[7] == 1.0f)) return -1;
+            if (!((double)r[6] >= t->e_min && (double)r[6] <= t->e_max)) return -1;
+        }
+    } else if (src->n_spec == 0 && (src->energy > t->e_max || src->energy < t->e_min)) return -1;
     if (opt->majorant_scale < 1.0) return -1;
     const size_t nvox = (size_t)nx * ny * nz;
 
@@ -944,6 +963,14 @@ static int run_impl(const float *density, const uint8_t *material, int32_t nx, i
             W->c.e_incident += p.E;
             W->c.n_histories++;
             W->stack[W->sp++] = p;
+            if (src->shape == 2 && p.type == 0) {
+                /* a phase-space photon is treated like a photon pushed at a vertex: outside the phantom it
+                 * has escaped, below P_cut it is deposited where it is (R5, R35); electron_history applies
+                 * the same two rules to every electron it is handed */
+                int v[3];
+                if (!locate(W, p.x, v)) { W->c.e_escaped += p.E; W->sp = 0; }
+                else if (p.E < t->p_cut) { deposit(W, v, p.E, DEP_CUTOFF); W->sp = 0; }
+            }
             while (W->sp > 0 && !W->overflow) {
                 particle_t q = W->stack[--W->sp];
                 if (q.type == 0) photon_history(W, q); else electron_history(W, q);

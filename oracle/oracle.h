@@ -71,12 +71,16 @@ typedef struct {
 
 typedef struct {
     int32_t particle; /* 0 photon, 1 electron */
-    int32_t shape;    /* 0 pencil, 1 parallel rectangle */
+    int32_t shape;    /* 0 pencil, 1 parallel rectangle, 2 phase space */
     double cx, cy, wx, wy;
     double energy;    /* used when n_spec == 0 */
     int32_t n_spec;
     const float *spec_E; /* n_spec+1 bin edges */
     const float *spec_w; /* n_spec weights */
+    /* shape 2, phase space (R35): n_phsp records {x, y, z, u, v, w, E, type};
+     * history h starts from record h mod n_phsp exactly as given, no draw, transport from counter 1 */
+    int64_t n_phsp;
+    const float *phsp;
 } orc_source;
 
 typedef struct {

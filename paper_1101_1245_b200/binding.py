@@ -49,7 +49,8 @@ class gpumcd_options(C.Structure):
 class gpumcd_source(C.Structure):
     _fields_ = [("particle", C.c_int32), ("shape", C.c_int32), ("cx", C.c_float), ("cy", C.c_float),
                 ("wx", C.c_float), ("wy", C.c_float), ("energy", C.c_float), ("n_spec", C.c_int32),
-                ("spec_E", C.c_void_p), ("spec_w", C.c_void_p)]
+                ("spec_E", C.c_void_p), ("spec_w", C.c_void_p),
+                ("n_phsp", C.c_uint64), ("phsp", C.c_void_p), ("phsp_on_host", C.c_int32)]
 
 
 class gpumcd_counters(C.Structure):
@@ -221,15 +222,25 @@ def gpumcd_set_phantom_host(ctx: Context, density: np.ndarray, material: np.ndar
 
 
 def gpumcd_set_source(ctx: Context, source) -> None:
-    """``source``: an inputs.Source (particle, shape, cx, cy, wx, wy, energy, spec_edges, spec_weights)."""
+    """``source``: an inputs.Source (particle, shape, cx, cy, wx, wy, energy, spec_edges, spec_weights, phsp)."""
     n_spec, pe, pw, keep = 0, None, None, ()
     if getattr(source, "spec_edges", None) is not None:
         e = np.ascontiguousarray(source.spec_edges, np.float32)
         w = np.ascontiguousarray(source.spec_weights, np.float32)
         keep = (e, w)
         n_spec, pe, pw = int(w.size), _hptr(e), _hptr(w)
+    n_phsp, pp, on_host = 0, None, 0
+    ps = getattr(source, "phsp", None)
+    if ps is not None:  # a torch CUDA tensor (device records) or a numpy array (host records), float32 [n, 8]
+        if isinstance(ps, np.ndarray):
+            ps = np.ascontiguousarray(ps, np.float32).reshape(-1, 8)
+            n_phsp, pp, on_host = int(ps.shape[0]), _hptr(ps), 1
+        else:
+            assert ps.is_cuda and ps.is_contiguous() and str(ps.dtype) == "torch.float32" and ps.shape[-1] == 8
+            n_phsp, pp = int(ps.numel() // 8), ps.data_ptr()
+        keep = keep + (ps,)
     s = gpumcd_source(source.particle, source.shape, source.cx, source.cy, source.wx, source.wy, source.energy,
-                      n_spec, pe, pw)
+                      n_spec, pe, pw, n_phsp, pp, on_host)
     ctx._check(load_library().gpumcd_set_source(ctx._h, C.byref(s)))
     del keep
 

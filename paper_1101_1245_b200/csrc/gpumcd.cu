@@ -78,27 +78,32 @@ __global__ void k_uniform_radius(const uint32_t *__restrict__ phantom, uint8_t *
     }
 }
 
-// H0: one primary per history from block (hist, track 0, ctr 0); transport starts at ctr 1.
+// H0: one primary per history (from block (hist, track 0, ctr 0), or a phase-space record); transport starts at
+// ctr 1.  The primaries go to the list of their type (a phase space may hold both).
 template <class V>
-__global__ void k_source(Params P, SourceDev S, Queue q, unsigned long long hist0, unsigned n)
+__global__ void k_source(Params P, SourceDev S, Queue qG, Queue qE, unsigned long long hist0, unsigned n)
 {
     const unsigned i = blockIdx.x * blockDim.x + threadIdx.x;
     const Acc acc(P);
     acc_init();
     double e_inc = 0.0;
     if (i < n) {
-        Particle p = make_primary(P, S, hist0 + i);
+        int type;
+        const Particle p = make_primary(P, S, hist0 + i, type);
         e_inc = static_cast<double>(p.E);
-        if (S.particle == 1 && !electron_tracked(P, p.E)) {
-            // an electron below the cutoff (or photon_only): deposited where it is born
+        if (S.shape == 2 && !inside(P.geo, p)) {
+            acc.esc(p.E); // a phase-space record outside the phantom: escaped at birth
+        } else if (type == 1 ? !electron_tracked(P, p.E) : (S.shape == 2 && p.E < P.tab.p_cut)) {
+            // below its cutoff (or photon_only): deposited where it is born (R5)
             deposit<V>(P, voxel_index(P.geo, p), p.E);
             acc.cut(p.E);
-            p.E = -1.0f; // marks an empty record
+        } else if (type == 1) {
+            push(P, qE, p, nullptr);
+        } else {
+            push(P, qG, p, nullptr);
         }
-        store_rec(q.A, q.B, q.C, i, p, 0u);
     }
     acc_flush(P, e_inc);
-    if (i == 0) *q.count = n;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -227,6 +232,28 @@ __global__ void k_tally_probe(double *__restrict__ edep, Geom g, int x0, int y0,
     }
 }
 
+// gpumcd_set_source, shape 2: check the phase-space records and count them by type.
+// out[0] bad records (type not 0 / 1, a number that is not finite), out[1] energies outside the tables,
+// out[2] photons, out[3] electrons
+__global__ void k_check_phsp(const float4 *__restrict__ rec, unsigned long long n, float e_lo, float e_hi,
+                             unsigned long long *out)
+{
+    unsigned long long bad = 0, range = 0, ng = 0, ne = 0;
+    for (unsigned long long i = blockIdx.x * static_cast<unsigned long long>(blockDim.x) + threadIdx.x; i < n;
+         i += static_cast<unsigned long long>(gridDim.x) * blockDim.x) {
+        const float4 a = rec[2 * i], b = rec[2 * i + 1];
+        const bool fin = isfinite(a.x) && isfinite(a.y) && isfinite(a.z) && isfinite(a.w) && isfinite(b.x) &&
+                         isfinite(b.y) && isfinite(b.z);
+        if (!fin || !(b.w == 0.0f || b.w == 1.0f)) { ++bad; continue; }
+        if (!(b.z >= e_lo && b.z <= e_hi)) ++range;
+        if (b.w == 0.0f) ++ng; else ++ne;
+    }
+    if (bad) atomicAdd(&out[0], bad);
+    if (range) atomicAdd(&out[1], range);
+    if (ng) atomicAdd(&out[2], ng);
+    if (ne) atomicAdd(&out[3], ne);
+}
+
 // Device-side check of the random-number layer (gpumcd_selftest_philox): block i = Philox4x32-10 of counter
 // in[6i .. 6i+3] under key in[6i+4], in[6i+5], and the uniforms the transport code makes of its four words.
 __global__ void k_philox_selftest(const uint32_t *__restrict__ in, uint32_t *__restrict__ out, float *__restrict__ u,
@@ -279,6 +306,7 @@ struct gpumcd_ctx {
     unsigned qcap = 0;
     double *spec_cdf = nullptr;
     float *spec_edges = nullptr;
+    float4 *phsp = nullptr;         // phase-space records of the current source (shape 2), library-owned
     // scheduler 1 (persistent kernel)
     unsigned *head = nullptr;       // next primary to be claimed
     float4 *stkA = nullptr, *stkB = nullptr; // per-warp stacks (persistent.cuh)
@@ -400,6 +428,7 @@ static void destroy_impl(gpumcd_ctx *c)
     for (int k = 0; k < kMaxQueues; ++k) { cudaFree(c->qA[k]); cudaFree(c->qB[k]); cudaFree(c->qC[k]); }
     cudaFree(c->spec_cdf);
     cudaFree(c->spec_edges);
+    cudaFree(c->phsp);
     cudaFree(c->head);
     cudaFree(c->stkA); cudaFree(c->stkB); cudaFree(c->stkC);
     for (auto &e : c->events) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
@@ -666,9 +695,43 @@ extern "C" int gpumcd_set_phantom(gpumcd_ctx *ctx, const float *density_dev, con
 extern "C" int gpumcd_set_source(gpumcd_ctx *ctx, const gpumcd_source *s)
 {
     if (!ctx || !s) return GPUMCD_ERR_INVALID_ARG;
-    if ((s->particle != 0 && s->particle != 1) || (s->shape != 0 && s->shape != 1) || s->n_spec < 0) {
+    if ((s->particle != 0 && s->particle != 1) || s->shape < 0 || s->shape > 2 || s->n_spec < 0) {
         set_error(ctx, "bad source description");
         return GPUMCD_ERR_INVALID_ARG;
+    }
+    if (ctx->ran) CK(cudaStreamSynchronize(ctx->last_stream)); // the last run still reads the old source arrays
+    if (s->shape == 2) {
+        // ---- phase space (R35): copy the records, check them, count them by type
+        if (!s->phsp || s->n_phsp == 0) { set_error(ctx, "empty phase space"); return GPUMCD_ERR_INVALID_ARG; }
+        float4 *rec = nullptr;
+        const size_t bytes = static_cast<size_t>(s->n_phsp) * 8 * sizeof(float);
+        CK(cudaMalloc(&rec, bytes));
+        struct Free { float4 *&p; ~Free() { cudaFree(p); } } guard{rec};
+        CK(cudaMemcpy(rec, s->phsp, bytes, s->phsp_on_host ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice));
+        unsigned long long *d_out = nullptr, h_out[4];
+        CK(cudaMalloc(&d_out, sizeof h_out));
+        struct Free2 { unsigned long long *p; ~Free2() { cudaFree(p); } } guard2{d_out};
+        CK(cudaMemset(d_out, 0, sizeof h_out));
+        const unsigned blocks = static_cast<unsigned>(std::min<uint64_t>((s->n_phsp + kBlock - 1) / kBlock, 148 * 8));
+        k_check_phsp<<<blocks, kBlock>>>(rec, s->n_phsp, ctx->tab.e_min, ctx->e_max, d_out);
+        CK(cudaGetLastError());
+        CK(cudaMemcpy(h_out, d_out, sizeof h_out, cudaMemcpyDeviceToHost));
+        if (h_out[0]) { set_error(ctx, "phase space: a record has a type other than 0 / 1 or a number that is not finite"); return GPUMCD_ERR_INVALID_ARG; }
+        if (h_out[1]) { set_error(ctx, "phase space: an energy lies outside the energy range of the tables"); return GPUMCD_ERR_TABLE_RANGE; }
+        SourceDev d{};
+        d.shape = 2;
+        d.has_g = h_out[2] != 0; d.has_e = h_out[3] != 0;
+        d.particle = d.has_g ? 0 : 1;
+        d.n_phsp = s->n_phsp;
+        cudaFree(ctx->phsp);
+        ctx->phsp = rec;
+        rec = nullptr; // owned by the context from here on
+        d.phsp = ctx->phsp;
+        cudaFree(ctx->spec_cdf); ctx->spec_cdf = nullptr;
+        cudaFree(ctx->spec_edges); ctx->spec_edges = nullptr;
+        ctx->src = d;
+        ctx->have_source = true;
+        return GPUMCD_OK;
     }
     const double wx = s->shape == 1 ? s->wx : 0.0, wy = s->shape == 1 ? s->wy : 0.0;
     if (wx < 0 || wy < 0 || s->cx - 0.5 * wx < 0 || s->cx + 0.5 * wx >= static_cast<double>(ctx->nx) * ctx->h ||
@@ -681,6 +744,8 @@ extern "C" int gpumcd_set_source(gpumcd_ctx *ctx, const gpumcd_source *s)
     d.particle = s->particle; d.shape = s->shape;
     d.cx = s->cx; d.cy = s->cy; d.wx = wx; d.wy = wy; d.energy = s->energy;
     d.n_spec = s->n_spec;
+    d.has_g = s->particle == 0; d.has_e = s->particle == 1;
+    cudaFree(ctx->phsp); ctx->phsp = nullptr;
     cudaFree(ctx->spec_cdf); ctx->spec_cdf = nullptr;
     cudaFree(ctx->spec_edges); ctx->spec_edges = nullptr;
     if (s->n_spec > 0) {
@@ -758,10 +823,9 @@ static int run_waves_host_loop(gpumcd_ctx *ctx, uint64_t h_begin, uint64_t n_his
         n = std::min<uint64_t>(n, 0x100000000ull - (h0 & 0xffffffffull)); // a wave never straddles 2^32
         const Params P = make_params(ctx, seed, static_cast<uint32_t>(h0 >> 32), trace_mode, trace);
         CK(cudaMemsetAsync(ctx->qcount, 0, 4 * sizeof(unsigned), st));
-        const int src_q = ctx->src.particle == 0 ? pcur : ecur;
         { LaunchScope ls(ctx, st, CLS_SOURCE);
         WITH_TALLY(ctx->opt.tally_mode, (k_source<Variant<false, false, TL>><<<static_cast<unsigned>((n + kBlock - 1) / kBlock), kBlock, 0, st>>>(
-                                            P, ctx->src, make_queue(ctx, src_q), h0, static_cast<unsigned>(n)))); }
+                                            P, ctx->src, make_queue(ctx, pcur), make_queue(ctx, ecur), h0, static_cast<unsigned>(n)))); }
         CK(cudaGetLastError());
         unsigned cnt[4];
         for (;;) {
@@ -1065,6 +1129,10 @@ extern "C" int gpumcd_probe_tally(gpumcd_ctx *ctx, uint64_t n_updates, double *u
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     // the field's footprint on the grid (a pencil beam: a 3 x 3 voxel column)
     const double h = ctx->h;
+    if (ctx->src.shape == 2) { // a phase space: its footprint is not known, take the whole face
+        ctx->src.cx = 0.5 * ctx->nx * h; ctx->src.cy = 0.5 * ctx->ny * h;
+        ctx->src.wx = (ctx->nx - 1) * h; ctx->src.wy = (ctx->ny - 1) * h;
+    }
     int x0 = static_cast<int>(std::floor((ctx->src.cx - 0.5 * ctx->src.wx) / h)) - (ctx->src.shape == 0 ? 1 : 0);
     int y0 = static_cast<int>(std::floor((ctx->src.cy - 0.5 * ctx->src.wy) / h)) - (ctx->src.shape == 0 ? 1 : 0);
     int x1 = static_cast<int>(std::floor((ctx->src.cx + 0.5 * ctx->src.wx) / h)) + (ctx->src.shape == 0 ? 1 : 0);

@@ -61,17 +61,45 @@ struct SourceDev {
     int n_spec;
     const double *cdf;  // n_spec+1, unnormalised running sum of the weights
     const float *edges; // n_spec+1
+    const float4 *phsp; // shape 2: n_phsp records of two float4 {x, y, z, u}, {v, w, E, type}
+    unsigned long long n_phsp;
+    int has_g, has_e;   // the source makes photons / electrons (a phase space may make both)
 };
 
 // H0: primary of one history from block (hist, track 0, ctr 0); transport starts at ctr 1.
 // (cdf, edges: the spectrum arrays, S.cdf / S.edges or their copies in shared memory)
+// `type` returns the primary's particle type (0 photon, 1 electron).  A phase-space primary (shape 2, PAPER.md
+// L389, R35) is record hist mod n_phsp exactly as given: no block is drawn for it, and it may lie
+// outside the phantom (the caller checks).
 __device__ __forceinline__ Particle make_primary(const Params &P, const SourceDev &S, unsigned long long hist,
-                                                 const double *__restrict__ cdf, const float *__restrict__ edges)
+                                                 const double *__restrict__ cdf, const float *__restrict__ edges,
+                                                 int &type)
 {
     Particle p;
     p.hist = static_cast<uint32_t>(hist);
     p.track = 0u;
     p.ctr = 0u;
+    type = S.particle;
+    if (S.shape == 2) {
+        const unsigned long long r = hist % S.n_phsp;
+        const float4 a = __ldg(&S.phsp[2 * r]), b = __ldg(&S.phsp[2 * r + 1]);
+        const double inv_h = 1.0 / static_cast<double>(P.geo.h);
+        const double vx = static_cast<double>(a.x) * inv_h, vy = static_cast<double>(a.y) * inv_h,
+                     vz = static_cast<double>(a.z) * inv_h;
+        const double fx = floor(vx), fy = floor(vy), fz = floor(vz);
+        // (cells far outside the phantom are clamped to just outside, so that they fit the packed record)
+        p.ix = static_cast<int>(fmin(fmax(fx, -1.0), 1024.0));
+        p.iy = static_cast<int>(fmin(fmax(fy, -1.0), 1024.0));
+        p.iz = static_cast<int>(fmin(fmax(fz, -1.0), 1024.0));
+        p.fx = static_cast<float>(vx - fx);
+        p.fy = static_cast<float>(vy - fy);
+        p.fz = static_cast<float>(vz - fz);
+        p.u = a.w; p.v = b.x; p.w = b.y;
+        p.E = b.z;
+        p.ctr = 1u;
+        type = b.w != 0.0f;
+        return p;
+    }
     const uint4 w = draw(P.rng, p);
     double x = S.cx, y = S.cy;
     if (S.shape == 1) {
@@ -102,9 +130,9 @@ __device__ __forceinline__ Particle make_primary(const Params &P, const SourceDe
     return p;
 }
 
-__device__ __forceinline__ Particle make_primary(const Params &P, const SourceDev &S, unsigned long long hist)
+__device__ __forceinline__ Particle make_primary(const Params &P, const SourceDev &S, unsigned long long hist, int &type)
 {
-    return make_primary(P, S, hist, S.cdf, S.edges);
+    return make_primary(P, S, hist, S.cdf, S.edges, type);
 }
 
 // the kernel's dynamic shared memory: [table blob | spectrum cdf (double) | spectrum edges (float)]
@@ -247,18 +275,19 @@ struct Warp {
         n[s] -= take;
         return got;
     }
-    // Converged code: the whole warp makes this warp's next (up to 32) primaries at once and banks them on
-    // ready stack s (SK_ES for an electron source, SK_GS for photons), from where free lanes pop them like
-    // any other ready particle: the source code (H0) then always runs with full lanes.  Returns false if the
-    // source is dry or the stack has no room for them right now.
+    // Converged code: the whole warp makes this warp's next (up to 32) primaries at once and banks them on the
+    // ready stack of their type (ES electrons, GS photons; a phase space may hold both), from where free lanes pop
+    // them like any other ready particle: the source code (H0) then always runs with full lanes.  Returns false if
+    // the source is dry or a stack has no room for them right now.
     template <class V>
-    __device__ __forceinline__ bool bank_primaries(const PersistArgs &a, Claim &cl, int s)
+    __device__ __forceinline__ bool bank_primaries(const PersistArgs &a, Claim &cl)
     {
         cl.refill(a.head, a.n_hist);
         const unsigned k = cl.end - cl.next;
-        if (k == 0u || n[s] + k > cap_r) return false;
+        if (k == 0u || (a.S.has_e && n[SK_ES] + k > cap_r) || (a.S.has_g && n[SK_GS] + k > cap_r)) return false;
         const unsigned lane = threadIdx.x & 31;
         bool on = lane < k;
+        int type = a.S.particle;
         Particle q;
         if (on) {
             // the spectrum arrays: their shared-memory copies if the kernel staged them (512 bins: nine dependent
@@ -269,15 +298,20 @@ struct Warp {
                 cdf = reinterpret_cast<const double *>(dyn_smem() + a.table_floats);
                 edges = reinterpret_cast<const float *>(cdf + (a.S.n_spec + 1));
             }
-            q = make_primary(a.P, a.S, a.hist0 + (cl.next + lane), cdf, edges);
+            q = make_primary(a.P, a.S, a.hist0 + (cl.next + lane), cdf, edges, type);
             *e_inc += static_cast<double>(q.E);
-            if (s == SK_ES && !electron_tracked(a.P, q.E)) { // below the cutoff (or photon_only): deposited where it is born
+            if (a.S.shape == 2 && !inside(a.P.geo, q)) { // a phase-space record outside the phantom: escaped at birth
+                Acc(a.P).esc(q.E);
+                on = false;
+            } else if (type == 1 ? !electron_tracked(a.P, q.E) : (a.S.shape == 2 && q.E < a.P.tab.p_cut)) {
+                // below its cutoff (or photon_only): deposited where it is born (R5)
                 deposit<V>(a.P, voxel_index(a.P.geo, q), q.E);
                 Acc(a.P).cut(q.E);
                 on = false;
             }
         }
-        push(a.P, s, on, q, 0u);
+        if (a.S.has_e) push(a.P, SK_ES, on && type == 1, q, 0u);
+        if (a.S.has_g) push(a.P, SK_GS, on && type == 0, q, 0u);
         cl.next += k;
         return true;
     }
@@ -292,7 +326,7 @@ __device__ __forceinline__ int electron_mode(const PersistArgs &a, const float *
 {
     const Params &P = a.P;
     const unsigned lane = threadIdx.x & 31;
-    const bool src_is_e = a.S.particle == 1;
+    const bool src_is_e = a.S.has_e != 0, src_is_g = a.S.has_g != 0;
     Particle p;
     float lnT = 0.f, M = 0.f;
     bool alive = false;
@@ -329,7 +363,7 @@ __device__ __forceinline__ int electron_mode(const PersistArgs &a, const float *
         // undone before some work has been done)
         const unsigned ready = static_cast<unsigned>(__popc(live)) + w.n[SK_ES];
         const unsigned E = ready + w.n[SK_EH], G = w.n[SK_GS] + w.n[SK_GI] + w.n[SK_GR];
-        const bool src_g = !src_is_e && !cl.empty();
+        const bool src_g = src_is_g && !cl.empty();
         // (only READY photons count towards the high-water mark: photon mode stays while it has kLow of them,
         // so a change made here is never undone before some work has been done)
         const unsigned Gr = w.n[SK_GS];
@@ -348,7 +382,7 @@ __device__ __forceinline__ int electron_mode(const PersistArgs &a, const float *
         if (~live) {
             uint32_t extra;
             bool got = w.pop(SK_ES, !alive, p, extra);
-            if (src_e && __any_sync(kFull, !alive && !got) && w.template bank_primaries<V>(a, cl, SK_ES))
+            if (src_e && __any_sync(kFull, !alive && !got) && w.template bank_primaries<V>(a, cl))
                 got = w.pop(SK_ES, !alive && !got, p, extra) || got;
             if (got) {
                 lnT = flog(p.E);
@@ -415,8 +449,7 @@ template <class V>
 __device__ __forceinline__ int photon_mode(const PersistArgs &a, const float *__restrict__ TB, Warp &w, Claim &cl)
 {
     const Params &P = a.P;
-    const unsigned lane = threadIdx.x & 31;
-    const bool src_is_g = a.S.particle == 0;
+    const bool src_is_g = a.S.has_g != 0, src_is_e = a.S.has_e != 0;
     Particle p;
     bool alive = false;
     for (;;) {
@@ -437,7 +470,7 @@ __device__ __forceinline__ int photon_mode(const PersistArgs &a, const float *__
         // ---- change of particle type?  (see electron_mode)
         const unsigned ready = static_cast<unsigned>(__popc(live)) + w.n[SK_GS];
         const unsigned G = ready + w.n[SK_GI] + w.n[SK_GR], E = w.n[SK_ES] + w.n[SK_EH];
-        const bool src_e = !src_is_g && !cl.empty();
+        const bool src_e = src_is_e && !cl.empty();
         const unsigned Er = w.n[SK_ES];
         bool leave = (Er >= w.high_e && G < w.high_g) || Er + kRoomE >= w.cap_r;
         if (!src_g) {
@@ -453,7 +486,7 @@ __device__ __forceinline__ int photon_mode(const PersistArgs &a, const float *__
         if (~live) {
             uint32_t extra;
             bool got = w.pop(SK_GS, !alive, p, extra);
-            if (src_g && __any_sync(kFull, !alive && !got) && w.template bank_primaries<V>(a, cl, SK_GS))
+            if (src_g && __any_sync(kFull, !alive && !got) && w.template bank_primaries<V>(a, cl))
                 got = w.pop(SK_GS, !alive && !got, p, extra) || got;
             if (got) alive = true;
         }
@@ -521,7 +554,7 @@ __global__ void __launch_bounds__(kPThreads, 1) k_persistent(const __grid_consta
     // Each warp works on its own until the source is exhausted and its stacks are empty.
     Claim cl;
     cl.exhausted = (a.n_hist == 0u);
-    int type = a.S.particle;
+    int type = a.S.has_g ? 0 : 1;
     while (type >= 0) type = (type == 1) ? electron_mode<V>(a, TB, w, cl) : photon_mode<V>(a, TB, w, cl);
 
     // ---- flush this warp's event counts and accounts

@@ -238,7 +238,7 @@ __device__ __forceinline__ void push(const Params &P, const Queue &q, const Part
     unsigned base = 0;
     if (lane == leader) {
         base = atomicAdd(q.count, static_cast<unsigned>(__popc(mask)));
-        atomicAdd(tally, static_cast<unsigned long long>(__popc(mask)));
+        if (tally) atomicAdd(tally, static_cast<unsigned long long>(__popc(mask)));
     }
     base = __shfl_sync(mask, base, leader);
     const unsigned slot = base + __popc(mask & ((1u << lane) - 1u));

@@ -18,7 +18,7 @@ from . import phantoms, spectra
 from .tables import TableBundle, build_tables
 
 PHOTON, ELECTRON = 0, 1
-PENCIL, RECTANGLE = 0, 1
+PENCIL, RECTANGLE, PHASE_SPACE = 0, 1, 2
 
 
 @dataclass
@@ -32,6 +32,7 @@ class Source:
     energy: float = 0.0
     spec_edges: Optional[np.ndarray] = None    # float32[n+1]
     spec_weights: Optional[np.ndarray] = None  # float32[n]
+    phsp: Optional[np.ndarray] = None          # shape PHASE_SPACE: float32[n, 8] {x, y, z, u, v, w, E, type}
 
 
 @dataclass

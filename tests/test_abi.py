@@ -41,7 +41,7 @@ def test_struct_layouts_match_the_header(lib):
     assert ctypes.sizeof(b.gpumcd_options) == 72
     assert ctypes.sizeof(b.gpumcd_counters) == 14 * 8 + 5 * 8
     assert ctypes.sizeof(b.gpumcd_tables) == 64
-    assert ctypes.sizeof(b.gpumcd_source) == 48
+    assert ctypes.sizeof(b.gpumcd_source) == 72
     opt = b.gpumcd_default_options()
     assert (opt.es_max_cm, opt.f_eloss_max, opt.pair_mode, opt.photon_only) == (0.5, 0.25, 1, 0)
     assert opt.wave_size == 1 << 20 and opt.bank_factor == 8 and opt.majorant_scale == 1.0
