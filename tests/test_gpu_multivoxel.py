@@ -38,7 +38,7 @@ def test_dose_parity_with_multi_voxel_steps(cfg, n, scheduler):
     # energy conservation on the device and agreement of the total with the oracle
     out = total(cg) + cg["e_escaped"]
     assert abs(out / cg["e_incident"] - 1.0) <= 1e-6
-    assert total(cg) == pytest.approx(total(co), rel=5e-5)
+    assert total(cg) == pytest.approx(total(co), rel=1e-5)   # BASELINE.json's bar (measured: <= 5e-6 at these sizes)
     gm, gsig = ev.batch_mean_sigma(np.stack(gs))
     om, osig = ev.batch_mean_sigma(np.stack(os_))
     assert ev.voxel_agreement(om, osig, gm, gsig, frac=0.1, k=3.0) >= 0.99
@@ -70,7 +70,7 @@ def test_paper_slab_geometry_with_multi_voxel_steps():
     o = oracle.run_workload(w, n, MV)
     for k in INT_KEYS:
         assert abs(g["counters"][k] - o.counters[k]) <= 10 + 2e-3 * o.counters[k], k
-    assert total(g["counters"]) == pytest.approx(total(o.counters), rel=3e-5)
+    assert total(g["counters"]) == pytest.approx(total(o.counters), rel=1e-5)
     assert ev.gamma_pass_rate(o.dose.astype(np.float64), g["dose"].astype(np.float64), w.voxel_cm, frac=0.1) >= 0.99
     # planar depth-dose: identical within 0.2 % of the maximum
     dg, do = g["edep"].sum(axis=(1, 2)), o.edep.sum(axis=(1, 2))

@@ -190,12 +190,16 @@ def test_wave_partition_does_not_change_the_result(scheduler, workloads):
 
 def test_pair_rest_energy_deposited_locally(workloads):
     w = workloads[3]
-    n = 50_000
+    n = 400_000
     o = oracle.run_workload(w, n, oracle.Options(pair_mode=0))
     g = run_gpu(w, n, pair_mode=0)
     assert g["counters"]["photon_pair"] == pytest.approx(o.counters["photon_pair"], rel=1e-3)
     assert g["counters"]["e_pair_rest"] == pytest.approx(o.counters["e_pair_rest"], rel=1e-3)
-    assert abs(g["edep"].sum() - o.edep.sum()) / o.edep.sum() <= 1e-4
+    # 3e-5, not 1e-5: a 15 MeV photon beam deposits a quarter of its energy, with a per-history spread larger
+    # than the mean, so the ~1e-3 of the histories that leave the oracle's path by an fp32 flip
+    # move the total by ~1e-5 sqrt(4e6 / n); measured over three seeds: 6e-5 at n = 5e4, <= 1.5e-5 at 4e5,
+    # <= 1.7e-5 at 4e6 (config 3 itself is held to 1e-5 at its full 4e6 histories in test_dose_parity)
+    assert abs(g["edep"].sum() - o.edep.sum()) / o.edep.sum() <= 3e-5
     bal = (total_deposit(g["counters"]) + g["counters"]["e_escaped"]) / g["counters"]["e_incident"] - 1
     assert abs(bal) <= 1e-6
 
@@ -217,7 +221,7 @@ def test_spectrum_source(workloads):
     o = oracle.run_workload(w, n, oracle.Options(photon_only=1))
     g = run_gpu(w, n, photon_only=1)
     assert g["counters"]["e_incident"] == pytest.approx(o.counters["e_incident"], rel=1e-6)
-    assert abs(g["edep"].sum() - o.edep.sum()) / o.edep.sum() <= 1e-4
+    assert abs(g["edep"].sum() - o.edep.sum()) / o.edep.sum() <= 1e-5
 
 
 def test_majorant_inflation_changes_only_fictitious_counts(workloads):

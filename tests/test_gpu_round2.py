@@ -79,8 +79,11 @@ def test_tally_modes_give_the_same_tally(cfg, n):
             np.testing.assert_allclose(g["dose"], (g["edep"] / mass / n).astype(np.float32), rtol=2e-6, atol=0)
             bal = (total(g["counters"]) + g["counters"]["e_escaped"]) / g["counters"]["e_incident"] - 1.0
             assert abs(bal) <= 1e-6
-            # and against the oracle: BASELINE.json's bar on the total
-            assert abs(total(g["counters"]) - total(o.counters)) / total(o.counters) <= 1e-5 + 3e-3 / np.sqrt(n / 1e5)
+            # and against the oracle: BASELINE.json's bar on the total, 1e-5 at the size test_dose_parity runs
+            # the configuration at (n_full); the difference is the statistical one of the few histories that an
+            # fp32 flip takes off the oracle's path, so it grows as 1 / sqrt(n) below that size
+            n_full = {1: 100_000, 2: 1_000_000, 3: 4_000_000, 4: 4_000_000, 5: 8_000_000}[cfg]
+            assert abs(total(g["counters"]) - total(o.counters)) / total(o.counters) <= 1e-5 * np.sqrt(n_full / n)
 
 
 @pytest.mark.parametrize("cfg,n", [(2, 150_000), (4, 600_000)])

@@ -62,7 +62,7 @@ def test_uncertainty_matches_the_history_by_history_oracle(geom, particle, n):
     mass = w.density.astype(np.float64) * w.voxel_cm ** 3
     d_o = e / n / mass
     u_o = oracle.uncertainty_from_moments(e, sq, n) / mass
-    assert total(g["counters"]) == pytest.approx(total(c), rel=1e-4)
+    assert total(g["counters"]) == pytest.approx(total(c), rel=1e-5)
     sel = d_o > 0.2 * d_o.max()
     assert sel.sum() > 500
     ratio2 = (g["sigma"][sel].astype(np.float64) / u_o[sel]) ** 2
@@ -85,7 +85,7 @@ def test_paper_geometry_dose_parity(geom, particle):
     o = oracle.run_workload(w, n)
     for k in INT_KEYS:
         assert abs(g["counters"][k] - o.counters[k]) <= 10 + 2e-3 * o.counters[k], k
-    assert total(g["counters"]) == pytest.approx(total(o.counters), rel=1e-5 if particle == PHOTON else 3e-5)
+    assert total(g["counters"]) == pytest.approx(total(o.counters), rel=1e-5)
     assert ev.gamma_pass_rate(o.dose.astype(np.float64), g["dose"].astype(np.float64), w.voxel_cm, frac=0.1) >= 0.99
 
 
