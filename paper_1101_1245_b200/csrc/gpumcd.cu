@@ -89,7 +89,7 @@ __global__ void k_source(Params P, SourceDev S, Queue qG, Queue qE, unsigned lon
     double e_inc = 0.0;
     if (i < n) {
         int type;
-        const Particle p = make_primary(P, S, hist0 + i, type);
+        const Particle p = S.shape == 2 ? make_primary<true>(P, S, hist0 + i, type) : make_primary<false>(P, S, hist0 + i, type);
         e_inc = static_cast<double>(p.E);
         if (S.shape == 2 && !inside(P.geo, p)) {
             acc.esc(p.E); // a phase-space record outside the phantom: escaped at birth
@@ -441,21 +441,25 @@ template <class V>
 static const void *persistent_variant(bool smem, int threads)
 {
     if (threads == kPThreadsDefault) return smem ? (const void *)k_persistent<V, true, kPThreadsDefault> : (const void *)k_persistent<V, false, kPThreadsDefault>;
-    if (V::TALLY == TALLY_F64) return smem ? (const void *)k_persistent<Variant<V::TRACE, V::MULTI, TALLY_F64>, true, 1024>
-                                           : (const void *)k_persistent<Variant<V::TRACE, V::MULTI, TALLY_F64>, false, 1024>;
+    if (V::TALLY == TALLY_F64 && !V::PHSP)
+        return smem ? (const void *)k_persistent<Variant<V::TRACE, V::MULTI, TALLY_F64>, true, 1024>
+                    : (const void *)k_persistent<Variant<V::TRACE, V::MULTI, TALLY_F64>, false, 1024>;
     return nullptr;
 }
-static const void *persistent_kernel(bool trace, bool multi, int tally, bool smem, int threads)
+template <bool MULTI, bool PHSP>
+static const void *persistent_tally(int tally, bool smem, int threads)
 {
-    if (trace) return persistent_variant<Variant<true, false, TALLY_F64>>(smem, threads); // a trace run tallies nothing of interest
-    if (multi) {
-        if (tally == TALLY_WARP) return persistent_variant<Variant<false, true, TALLY_WARP>>(smem, threads);
-        if (tally == TALLY_FIXED) return persistent_variant<Variant<false, true, TALLY_FIXED>>(smem, threads);
-        return persistent_variant<Variant<false, true, TALLY_F64>>(smem, threads);
-    }
-    if (tally == TALLY_WARP) return persistent_variant<Variant<false, false, TALLY_WARP>>(smem, threads);
-    if (tally == TALLY_FIXED) return persistent_variant<Variant<false, false, TALLY_FIXED>>(smem, threads);
-    return persistent_variant<Variant<false, false, TALLY_F64>>(smem, threads);
+    if (tally == TALLY_WARP) return persistent_variant<Variant<false, MULTI, TALLY_WARP, PHSP>>(smem, threads);
+    if (tally == TALLY_FIXED) return persistent_variant<Variant<false, MULTI, TALLY_FIXED, PHSP>>(smem, threads);
+    return persistent_variant<Variant<false, MULTI, TALLY_F64, PHSP>>(smem, threads);
+}
+// nullptr: the combination is not built (1024 threads per CTA with another tally than fp64 or a phase space)
+static const void *persistent_kernel(bool trace, bool multi, int tally, bool phsp, bool smem, int threads)
+{
+    if (trace) return phsp ? persistent_variant<Variant<true, false, TALLY_F64, true>>(smem, threads)
+                           : persistent_variant<Variant<true, false, TALLY_F64>>(smem, threads); // a trace run tallies nothing of interest
+    if (multi) return phsp ? persistent_tally<true, true>(tally, smem, threads) : persistent_tally<true, false>(tally, smem, threads);
+    return phsp ? persistent_tally<false, true>(tally, smem, threads) : persistent_tally<false, false>(tally, smem, threads);
 }
 
 // cudaFuncAttributeMaxDynamicSharedMemorySize belongs to the kernel function, not to a context: it is only
@@ -621,7 +625,7 @@ static int create_impl(gpumcd_ctx **out, const float *density, const uint8_t *ma
         if (!coop) { set_error(ctx, "device does not support cooperative launches (scheduler 1)"); return GPUMCD_ERR_CUDA; }
         const size_t table_bytes = static_cast<size_t>(ctx->table_floats) * sizeof(float);
         const int threads = opt.cta_threads ? static_cast<int>(opt.cta_threads) : kPThreadsDefault;
-        const void *fn = persistent_kernel(false, opt.hom_tol > 0.f, opt.tally_mode, true, threads);
+        const void *fn = persistent_kernel(false, opt.hom_tol > 0.f, opt.tally_mode, false, true, threads);
         cudaFuncAttributes fa{};
         CK(cudaFuncGetAttributes(&fa, fn));
         ctx->smem_tables = opt.table_memory == 0 && table_bytes + fa.sharedSizeBytes + 1024 <= static_cast<size_t>(max_smem);
@@ -630,7 +634,7 @@ static int create_impl(gpumcd_ctx **out, const float *density, const uint8_t *ma
         if (ctx->smem_tables && table_bytes + kSpecSmemBytes + fa.sharedSizeBytes + 1024 <= static_cast<size_t>(max_smem))
             ctx->spec_smem_bytes = kSpecSmemBytes;
         const size_t dyn = ctx->smem_tables ? table_bytes + ctx->spec_smem_bytes : 0;
-        fn = persistent_kernel(false, opt.hom_tol > 0.f, opt.tally_mode, ctx->smem_tables, threads);
+        fn = persistent_kernel(false, opt.hom_tol > 0.f, opt.tally_mode, false, ctx->smem_tables, threads);
         { const int rc = allow_dynamic_smem(ctx, fn, dyn); if (rc != GPUMCD_OK) return rc; }
         int per_sm = 0;
         CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, threads, dyn));
@@ -907,7 +911,8 @@ static int run_persistent(gpumcd_ctx *ctx, uint64_t h_begin, uint64_t n_hist, ui
         void *args[] = {&a};
         // the kernel variant: trace (photon-only replay) | multi-voxel steps x tally mode; tables in shared memory; CTA size
         const bool multi = ctx->opt.hom_tol > 0.f && !trace; // a trace run tracks no electrons
-        const void *fn = persistent_kernel(trace != nullptr, multi, ctx->opt.tally_mode, ctx->smem_tables, threads);
+        const void *fn = persistent_kernel(trace != nullptr, multi, ctx->opt.tally_mode, ctx->src.shape == 2, ctx->smem_tables, threads);
+        if (!fn) { set_error(ctx, "a phase-space source needs the default CTA size (cta_threads 0)"); return GPUMCD_ERR_INVALID_ARG; }
         const size_t dyn = ctx->smem_tables ? static_cast<size_t>(ctx->table_floats) * sizeof(float) + ctx->spec_smem_bytes : 0;
         { const int rc = allow_dynamic_smem(ctx, fn, dyn); if (rc != GPUMCD_OK) return rc; }
         { LaunchScope ls(ctx, st, CLS_ELECTRON);

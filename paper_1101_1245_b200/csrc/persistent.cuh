@@ -71,6 +71,7 @@ struct SourceDev {
 // `type` returns the primary's particle type (0 photon, 1 electron).  A phase-space primary (shape 2, PAPER.md
 // L389, R35) is record hist mod n_phsp exactly as given: no block is drawn for it, and it may lie
 // outside the phantom (the caller checks).
+template <bool PHSP>
 __device__ __forceinline__ Particle make_primary(const Params &P, const SourceDev &S, unsigned long long hist,
                                                  const double *__restrict__ cdf, const float *__restrict__ edges,
                                                  int &type)
@@ -80,12 +81,11 @@ __device__ __forceinline__ Particle make_primary(const Params &P, const SourceDe
     p.track = 0u;
     p.ctr = 0u;
     type = S.particle;
-    if (S.shape == 2) {
+    if (PHSP) {
         const unsigned long long r = hist % S.n_phsp;
         const float4 a = __ldg(&S.phsp[2 * r]), b = __ldg(&S.phsp[2 * r + 1]);
-        const double inv_h = 1.0 / static_cast<double>(P.geo.h);
-        const double vx = static_cast<double>(a.x) * inv_h, vy = static_cast<double>(a.y) * inv_h,
-                     vz = static_cast<double>(a.z) * inv_h;
+        const double hd = static_cast<double>(P.geo.h); // (divisions, as in the oracle's floor(x / h))
+        const double vx = static_cast<double>(a.x) / hd, vy = static_cast<double>(a.y) / hd, vz = static_cast<double>(a.z) / hd;
         const double fx = floor(vx), fy = floor(vy), fz = floor(vz);
         // (cells far outside the phantom are clamped to just outside, so that they fit the packed record)
         p.ix = static_cast<int>(fmin(fmax(fx, -1.0), 1024.0));
@@ -130,9 +130,10 @@ __device__ __forceinline__ Particle make_primary(const Params &P, const SourceDe
     return p;
 }
 
+template <bool PHSP>
 __device__ __forceinline__ Particle make_primary(const Params &P, const SourceDev &S, unsigned long long hist, int &type)
 {
-    return make_primary(P, S, hist, S.cdf, S.edges, type);
+    return make_primary<PHSP>(P, S, hist, S.cdf, S.edges, type);
 }
 
 // the kernel's dynamic shared memory: [table blob | spectrum cdf (double) | spectrum edges (float)]
@@ -280,11 +281,13 @@ struct Warp {
     // them like any other ready particle: the source code (H0) then always runs with full lanes.  Returns false if
     // the source is dry or a stack has no room for them right now.
     template <class V>
-    __device__ __forceinline__ bool bank_primaries(const PersistArgs &a, Claim &cl)
+    __device__ __forceinline__ bool bank_primaries(const PersistArgs &a, Claim &cl, int s_mode)
     {
         cl.refill(a.head, a.n_hist);
         const unsigned k = cl.end - cl.next;
-        if (k == 0u || (a.S.has_e && n[SK_ES] + k > cap_r) || (a.S.has_g && n[SK_GS] + k > cap_r)) return false;
+        if (k == 0u) return false;
+        if (V::PHSP ? (a.S.has_e && n[SK_ES] + k > cap_r) || (a.S.has_g && n[SK_GS] + k > cap_r)
+                    : n[s_mode] + k > cap_r) return false;
         const unsigned lane = threadIdx.x & 31;
         bool on = lane < k;
         int type = a.S.particle;
@@ -298,20 +301,24 @@ struct Warp {
                 cdf = reinterpret_cast<const double *>(dyn_smem() + a.table_floats);
                 edges = reinterpret_cast<const float *>(cdf + (a.S.n_spec + 1));
             }
-            q = make_primary(a.P, a.S, a.hist0 + (cl.next + lane), cdf, edges, type);
+            q = make_primary<V::PHSP>(a.P, a.S, a.hist0 + (cl.next + lane), cdf, edges, type);
             *e_inc += static_cast<double>(q.E);
-            if (a.S.shape == 2 && !inside(a.P.geo, q)) { // a phase-space record outside the phantom: escaped at birth
+            if (V::PHSP && !inside(a.P.geo, q)) { // a phase-space record outside the phantom: escaped at birth
                 Acc(a.P).esc(q.E);
                 on = false;
-            } else if (type == 1 ? !electron_tracked(a.P, q.E) : (a.S.shape == 2 && q.E < a.P.tab.p_cut)) {
+            } else if (type == 1 ? !electron_tracked(a.P, q.E) : (V::PHSP && q.E < a.P.tab.p_cut)) {
                 // below its cutoff (or photon_only): deposited where it is born (R5)
                 deposit<V>(a.P, voxel_index(a.P.geo, q), q.E);
                 Acc(a.P).cut(q.E);
                 on = false;
             }
         }
-        if (a.S.has_e) push(a.P, SK_ES, on && type == 1, q, 0u);
-        if (a.S.has_g) push(a.P, SK_GS, on && type == 0, q, 0u);
+        if (V::PHSP) { // a phase space may hold both types
+            if (a.S.has_e) push(a.P, SK_ES, on && type == 1, q, 0u);
+            if (a.S.has_g) push(a.P, SK_GS, on && type == 0, q, 0u);
+        } else { // s_mode: the ready stack of the calling mode, which is the source's type when it asks for primaries
+            push(a.P, s_mode, on, q, 0u);
+        }
         cl.next += k;
         return true;
     }
@@ -382,7 +389,7 @@ __device__ __forceinline__ int electron_mode(const PersistArgs &a, const float *
         if (~live) {
             uint32_t extra;
             bool got = w.pop(SK_ES, !alive, p, extra);
-            if (src_e && __any_sync(kFull, !alive && !got) && w.template bank_primaries<V>(a, cl))
+            if (src_e && __any_sync(kFull, !alive && !got) && w.template bank_primaries<V>(a, cl, SK_ES))
                 got = w.pop(SK_ES, !alive && !got, p, extra) || got;
             if (got) {
                 lnT = flog(p.E);
@@ -486,7 +493,7 @@ __device__ __forceinline__ int photon_mode(const PersistArgs &a, const float *__
         if (~live) {
             uint32_t extra;
             bool got = w.pop(SK_GS, !alive, p, extra);
-            if (src_g && __any_sync(kFull, !alive && !got) && w.template bank_primaries<V>(a, cl))
+            if (src_g && __any_sync(kFull, !alive && !got) && w.template bank_primaries<V>(a, cl, SK_GS))
                 got = w.pop(SK_GS, !alive && !got, p, extra) || got;
             if (got) alive = true;
         }

@@ -41,11 +41,12 @@ struct Opts {
 
 // Compile-time variant of the transport code: TRACE records the primary track's event codes
 // (gpumcd_run_trace), MULTI selects multi-voxel electron steps (R32), TALLY the tally arithmetic
-// (gpumcd_options.tally_mode).
+// (gpumcd_options.tally_mode), PHSP a phase-space source (gpumcd_source.shape 2: primaries of both types, possibly
+// outside the phantom or below a cutoff; kept out of the other variants, where its code cost 4 % of the run time).
 enum : int { TALLY_F64 = 0, TALLY_WARP = 1, TALLY_FIXED = 2 };
-template <bool TRACE_, bool MULTI_, int TALLY_>
+template <bool TRACE_, bool MULTI_, int TALLY_, bool PHSP_ = false>
 struct Variant {
-    static constexpr bool TRACE = TRACE_, MULTI = MULTI_;
+    static constexpr bool TRACE = TRACE_, MULTI = MULTI_, PHSP = PHSP_;
     static constexpr int TALLY = TALLY_;
 };
 
@@ -193,6 +194,10 @@ __device__ __forceinline__ double tally_value(const Params &P, size_t i)
     return P.edep[i];
 }
 
+// A record that finds its queue full is counted, never dropped silently (R18).  Out of line: the push code is
+// inlined a dozen times and this never runs in a valid run.
+__device__ __noinline__ void count_overflow(DevCounters *cnt) { atomicAdd(&cnt->overflow, 1ull); }
+
 // ---- records ---------------------------------------------------------------------------------
 __device__ __forceinline__ void store_rec(float4 *A, float4 *B, uint4 *C, size_t i, const Particle &c, uint32_t extra)
 {
@@ -243,7 +248,7 @@ __device__ __forceinline__ void push(const Params &P, const Queue &q, const Part
     base = __shfl_sync(mask, base, leader);
     const unsigned slot = base + __popc(mask & ((1u << lane) - 1u));
     if (slot < q.cap) store_rec(q.A, q.B, q.C, slot, c, 0u);
-    else atomicAdd(&P.cnt->overflow, 1ull);
+    else count_overflow(P.cnt);
 }
 __device__ __forceinline__ void push(const Params &P, const WarpStack &q, const Particle &c)
 {
@@ -261,7 +266,7 @@ __device__ __forceinline__ void push(const Params &P, const WarpStack &q, const 
         store_rec(q.A, q.B, q.C, slot, c, 0u);
     } else {
         atomicSub(q.count, 1u);
-        atomicAdd(&P.cnt->overflow, 1ull);
+        count_overflow(P.cnt);
     }
 }
 __device__ __forceinline__ void push_e(const Params &P, const Queue &q, const Particle &c) { push(P, q, c, &P.cnt->pushes_e); }
