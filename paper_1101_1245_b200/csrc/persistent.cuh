@@ -258,7 +258,7 @@ struct Warp {
             if (on) {
                 const unsigned slot = n[s] + __popc(m & lt);
                 if (slot < cap(s)) store_rec(A, B, C, off(s) + slot, c, extra);
-                else atomicAdd(&P.cnt->overflow, 1ull);
+                else count_overflow(P.cnt);
             }
             n[s] = min(n[s] + static_cast<unsigned>(__popc(m)), cap(s));
             __syncwarp(); // the records are read back by other lanes of this warp
