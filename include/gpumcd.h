@@ -129,6 +129,12 @@ typedef struct {
                               how much work of one type is done before the other type is picked up      */
     uint32_t bank_low;     /* scheduler 1, tuning (0 = 24, at most 64): once the source is exhausted a warp with
                               fewer ready particles of its type than this changes to the other type      */
+    uint32_t steps_per_refill; /* scheduler 1: condensed-history steps a warp makes at most before it looks at its
+                              stacks again (refills free lanes, banks hard-event candidates, may change type): the
+                              paper's N, "stream compaction after N simulation steps" (L180).  Lanes whose electron
+                              ended wait meanwhile, so the loop goes on only while 24 of the 32 lanes still step.
+                              0 = automatic: 4 for an electron beam, 1 otherwise; at most 64.  Ignored (1) with a
+                              phase-space source and with cta_threads 1024                                   */
     int32_t l2_persist;    /* scheduler 1: 1 = the packed phantom (4 bytes per voxel) is read through a persisting
                               L2 access window, so that the tally and the particle stacks cannot evict it
                               (raises the device-wide cudaLimitPersistingL2CacheSize to the phantom's size, up

@@ -43,7 +43,8 @@ class gpumcd_options(C.Structure):
                 ("wave_size", C.c_uint32), ("bank_factor", C.c_uint32), ("scheduler", C.c_int32),
                 ("warp_stack", C.c_uint32), ("cta_threads", C.c_uint32), ("hom_tol", C.c_float),
                 ("tally_mode", C.c_int32), ("table_memory", C.c_int32), ("bank_high_g", C.c_uint32),
-                ("bank_high_e", C.c_uint32), ("bank_low", C.c_uint32), ("l2_persist", C.c_int32)]
+                ("bank_high_e", C.c_uint32), ("bank_low", C.c_uint32), ("steps_per_refill", C.c_uint32),
+                ("l2_persist", C.c_int32)]
 
 
 class gpumcd_source(C.Structure):

@@ -407,6 +407,7 @@ extern "C" int gpumcd_default_options(gpumcd_options *opt)
     opt->bank_high_g = 0;
     opt->bank_high_e = 0;
     opt->bank_low = 0;
+    opt->steps_per_refill = 0;
     opt->l2_persist = 0;
     return GPUMCD_OK;
 }
@@ -441,25 +442,27 @@ template <class V>
 static const void *persistent_variant(bool smem, int threads)
 {
     if (threads == kPThreadsDefault) return smem ? (const void *)k_persistent<V, true, kPThreadsDefault> : (const void *)k_persistent<V, false, kPThreadsDefault>;
-    if (V::TALLY == TALLY_F64 && !V::PHSP)
+    if (V::TALLY == TALLY_F64 && !V::PHSP && !V::INNER)
         return smem ? (const void *)k_persistent<Variant<V::TRACE, V::MULTI, TALLY_F64>, true, 1024>
                     : (const void *)k_persistent<Variant<V::TRACE, V::MULTI, TALLY_F64>, false, 1024>;
     return nullptr;
 }
-template <bool MULTI, bool PHSP>
+template <bool MULTI, bool PHSP, bool INNER>
 static const void *persistent_tally(int tally, bool smem, int threads)
 {
-    if (tally == TALLY_WARP) return persistent_variant<Variant<false, MULTI, TALLY_WARP, PHSP>>(smem, threads);
-    if (tally == TALLY_FIXED) return persistent_variant<Variant<false, MULTI, TALLY_FIXED, PHSP>>(smem, threads);
-    return persistent_variant<Variant<false, MULTI, TALLY_F64, PHSP>>(smem, threads);
+    if (tally == TALLY_WARP) return persistent_variant<Variant<false, MULTI, TALLY_WARP, PHSP, INNER>>(smem, threads);
+    if (tally == TALLY_FIXED) return persistent_variant<Variant<false, MULTI, TALLY_FIXED, PHSP, INNER>>(smem, threads);
+    return persistent_variant<Variant<false, MULTI, TALLY_F64, PHSP, INNER>>(smem, threads);
 }
-// nullptr: the combination is not built (1024 threads per CTA with another tally than fp64 or a phase space)
-static const void *persistent_kernel(bool trace, bool multi, int tally, bool phsp, bool smem, int threads)
+// nullptr: the combination is not built (1024 threads per CTA with another tally than fp64, a phase space or
+// several steps per refill; a phase space with several steps per refill)
+static const void *persistent_kernel(bool trace, bool multi, int tally, bool phsp, bool inner, bool smem, int threads)
 {
     if (trace) return phsp ? persistent_variant<Variant<true, false, TALLY_F64, true>>(smem, threads)
                            : persistent_variant<Variant<true, false, TALLY_F64>>(smem, threads); // a trace run tallies nothing of interest
-    if (multi) return phsp ? persistent_tally<true, true>(tally, smem, threads) : persistent_tally<true, false>(tally, smem, threads);
-    return phsp ? persistent_tally<false, true>(tally, smem, threads) : persistent_tally<false, false>(tally, smem, threads);
+    if (phsp) return multi ? persistent_tally<true, true, false>(tally, smem, threads) : persistent_tally<false, true, false>(tally, smem, threads);
+    if (inner) return multi ? persistent_tally<true, false, true>(tally, smem, threads) : persistent_tally<false, false, true>(tally, smem, threads);
+    return multi ? persistent_tally<true, false, false>(tally, smem, threads) : persistent_tally<false, false, false>(tally, smem, threads);
 }
 
 // cudaFuncAttributeMaxDynamicSharedMemorySize belongs to the kernel function, not to a context: it is only
@@ -557,7 +560,7 @@ static int create_impl(gpumcd_ctx **out, const float *density, const uint8_t *ma
         !(opt.majorant_scale >= 1.f) || opt.wave_size == 0 || opt.bank_factor == 0 || opt.warp_stack > (1u << 20) ||
         (opt.cta_threads != 0 && opt.cta_threads != kPThreadsDefault && opt.cta_threads != 1024) || !(opt.hom_tol >= 0.f) ||
         opt.tally_mode < 0 || opt.tally_mode > 2 || (opt.tally_mode != 0 && opt.cta_threads == 1024) ||
-        opt.table_memory < 0 || opt.table_memory > 1 || opt.bank_low > 64 || opt.l2_persist < 0 || opt.l2_persist > 1 ||
+        opt.table_memory < 0 || opt.table_memory > 1 || opt.bank_low > 64 || opt.steps_per_refill > 64 || opt.l2_persist < 0 || opt.l2_persist > 1 ||
         static_cast<unsigned long long>(opt.wave_size) * opt.bank_factor > 0x7fffffffull) {
         set_error(nullptr, "bad options");
         return GPUMCD_ERR_INVALID_ARG;
@@ -625,7 +628,7 @@ static int create_impl(gpumcd_ctx **out, const float *density, const uint8_t *ma
         if (!coop) { set_error(ctx, "device does not support cooperative launches (scheduler 1)"); return GPUMCD_ERR_CUDA; }
         const size_t table_bytes = static_cast<size_t>(ctx->table_floats) * sizeof(float);
         const int threads = opt.cta_threads ? static_cast<int>(opt.cta_threads) : kPThreadsDefault;
-        const void *fn = persistent_kernel(false, opt.hom_tol > 0.f, opt.tally_mode, false, true, threads);
+        const void *fn = persistent_kernel(false, opt.hom_tol > 0.f, opt.tally_mode, false, false, true, threads);
         cudaFuncAttributes fa{};
         CK(cudaFuncGetAttributes(&fa, fn));
         ctx->smem_tables = opt.table_memory == 0 && table_bytes + fa.sharedSizeBytes + 1024 <= static_cast<size_t>(max_smem);
@@ -634,7 +637,7 @@ static int create_impl(gpumcd_ctx **out, const float *density, const uint8_t *ma
         if (ctx->smem_tables && table_bytes + kSpecSmemBytes + fa.sharedSizeBytes + 1024 <= static_cast<size_t>(max_smem))
             ctx->spec_smem_bytes = kSpecSmemBytes;
         const size_t dyn = ctx->smem_tables ? table_bytes + ctx->spec_smem_bytes : 0;
-        fn = persistent_kernel(false, opt.hom_tol > 0.f, opt.tally_mode, false, ctx->smem_tables, threads);
+        fn = persistent_kernel(false, opt.hom_tol > 0.f, opt.tally_mode, false, false, ctx->smem_tables, threads);
         { const int rc = allow_dynamic_smem(ctx, fn, dyn); if (rc != GPUMCD_OK) return rc; }
         int per_sm = 0;
         CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, threads, dyn));
@@ -908,10 +911,15 @@ static int run_persistent(gpumcd_ctx *ctx, uint64_t h_begin, uint64_t n_hist, ui
         a.high_g = ctx->opt.bank_high_g ? ctx->opt.bank_high_g : (threads != 1024 ? 80u : 512u);
         a.high_e = ctx->opt.bank_high_e ? ctx->opt.bank_high_e : (threads != 1024 ? 160u : 512u);
         a.low = ctx->opt.bank_low ? ctx->opt.bank_low : kLowDefault;
+        // steps per refill (the paper's N, L180): several pay for long electron tracks, i.e. an electron beam;
+        // measured: 15 MeV electrons in water 2.78 -> 2.63 ms with 4, photon beams in heterogeneous phantoms lose 1-2 %
+        const bool phsp = ctx->src.shape == 2;
+        a.inner = ctx->opt.steps_per_refill ? ctx->opt.steps_per_refill : (ctx->src.particle == 1 && !phsp && threads != 1024 ? 4u : 1u);
+        if (phsp || threads == 1024 || trace) a.inner = 1u; // (variants that are not built: one step per refill)
         void *args[] = {&a};
         // the kernel variant: trace (photon-only replay) | multi-voxel steps x tally mode; tables in shared memory; CTA size
         const bool multi = ctx->opt.hom_tol > 0.f && !trace; // a trace run tracks no electrons
-        const void *fn = persistent_kernel(trace != nullptr, multi, ctx->opt.tally_mode, ctx->src.shape == 2, ctx->smem_tables, threads);
+        const void *fn = persistent_kernel(trace != nullptr, multi, ctx->opt.tally_mode, phsp, a.inner > 1u, ctx->smem_tables, threads);
         if (!fn) { set_error(ctx, "a phase-space source needs the default CTA size (cta_threads 0)"); return GPUMCD_ERR_INVALID_ARG; }
         const size_t dyn = ctx->smem_tables ? static_cast<size_t>(ctx->table_floats) * sizeof(float) + ctx->spec_smem_bytes : 0;
         { const int rc = allow_dynamic_smem(ctx, fn, dyn); if (rc != GPUMCD_OK) return rc; }

@@ -41,6 +41,7 @@ constexpr int kPThreadsMax = 1024;
 constexpr unsigned kFull = 0xffffffffu;
 constexpr unsigned kChunk = 32;            // primaries a warp claims per atomic on the source head
 constexpr unsigned kPend = 64;             // capacity of a waiting stack (EH, GI, GR): < 32 before a move, + 32 after
+constexpr unsigned kKeep = 24;             // lanes that must be able to go on for another step inside one iteration
 constexpr unsigned kLowDefault = 24;       // own-type particles below which a warp with no source changes type
 // Forced type changes.  Between two looks at the rules below photon mode banks at most 96 electrons (one Compton
 // batch: 32, one batch of pair events: 64) and electron mode at most 32 photons (one hard-event batch).
@@ -189,6 +190,7 @@ struct PersistArgs {
     unsigned cap_r;                // capacity of a ready stack (ES, GS)
     unsigned high_g, high_e;       // banked photons / electrons that make a warp change to that type
     unsigned low;                  // own-type ready particles below which a warp with no source changes type
+    unsigned inner;                // condensed-history steps a warp makes at most between two looks at its stacks
     unsigned stride;               // 2 cap_r + 3 kPend
     unsigned long long hist0;      // first history of the launch (low word never wraps inside a launch)
     unsigned n_hist;               // histories of the launch (< 2^32)
@@ -398,12 +400,26 @@ __device__ __forceinline__ int electron_mode(const PersistArgs &a, const float *
         }
         const unsigned sm = __ballot_sync(kFull, alive);
         if (sm == 0u) continue;
-        // ---- one condensed-history step for every lane that holds an electron
-        int st = ST_ALIVE;
-        if (alive) st = electron_step<V>(P, TB, p, lnT, M);
-        w.count(WC_STEP, sm);
-        w.push(P, SK_EH, alive && st == ST_HARD, p, __float_as_uint(M));
-        if (st != ST_ALIVE) alive = false;
+        int st = alive ? ST_ALIVE : ST_DEAD;
+        if (!V::INNER) {
+            // ---- one condensed-history step for every lane that holds an electron
+            if (alive) st = electron_step<V>(P, TB, p, lnT, M);
+            w.count(WC_STEP, sm);
+        } else {
+            // ---- or several (the paper's N, L180: steps between two compactions): the lanes go on stepping while
+            // enough of them still can (kKeep) or nothing could refill the others anyway; a lane whose step ended
+            // the electron or on a hard-event candidate waits.  Pays for long tracks (an electron beam in water).
+            const bool can_refill = w.n[SK_ES] != 0u || src_e;
+            unsigned act = sm, k = 0u;
+#pragma unroll 1
+            do {
+                if (st == ST_ALIVE) st = electron_step<V>(P, TB, p, lnT, M);
+                w.count(WC_STEP, act);
+                act = __ballot_sync(kFull, st == ST_ALIVE);
+            } while (act != 0u && ++k < a.inner && (static_cast<unsigned>(__popc(act)) >= kKeep || !can_refill));
+        }
+        w.push(P, SK_EH, st == ST_HARD, p, __float_as_uint(M));
+        alive = st == ST_ALIVE;
     }
 }
 

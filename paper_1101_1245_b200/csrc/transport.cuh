@@ -44,9 +44,11 @@ struct Opts {
 // (gpumcd_options.tally_mode), PHSP a phase-space source (gpumcd_source.shape 2: primaries of both types, possibly
 // outside the phantom or below a cutoff; kept out of the other variants, where its code cost 4 % of the run time).
 enum : int { TALLY_F64 = 0, TALLY_WARP = 1, TALLY_FIXED = 2 };
-template <bool TRACE_, bool MULTI_, int TALLY_, bool PHSP_ = false>
+// INNER: scheduler 1 makes up to `steps_per_refill` condensed-history steps per look at its stacks (the paper's N,
+// L180); a variant of its own because the loop form costs the single-step form 2 % where it does not pay.
+template <bool TRACE_, bool MULTI_, int TALLY_, bool PHSP_ = false, bool INNER_ = false>
 struct Variant {
-    static constexpr bool TRACE = TRACE_, MULTI = MULTI_, PHSP = PHSP_;
+    static constexpr bool TRACE = TRACE_, MULTI = MULTI_, PHSP = PHSP_, INNER = INNER_;
     static constexpr int TALLY = TALLY_;
 };
 

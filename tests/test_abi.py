@@ -38,7 +38,7 @@ def test_library_exports_every_declared_symbol(lib):
 
 def test_struct_layouts_match_the_header(lib):
     from paper_1101_1245_b200 import binding as b
-    assert ctypes.sizeof(b.gpumcd_options) == 72
+    assert ctypes.sizeof(b.gpumcd_options) == 76
     assert ctypes.sizeof(b.gpumcd_counters) == 14 * 8 + 5 * 8
     assert ctypes.sizeof(b.gpumcd_tables) == 64
     assert ctypes.sizeof(b.gpumcd_source) == 72
