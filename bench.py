@@ -294,12 +294,17 @@ def ablation(args):
                 ("high_e80", {"bank_high_e": 80}), ("high_e320", {"bank_high_e": 320}), ("high_e640", {"bank_high_e": 640}),
                 ("low8", {"bank_low": 8}), ("low48", {"bank_low": 48}),
                 ("stack256", {"warp_stack": 256}), ("stack512", {"warp_stack": 512}),
+                ("steps_per_refill1", {"steps_per_refill": 1}), ("steps_per_refill2", {"steps_per_refill": 2}),
+                ("steps_per_refill4", {"steps_per_refill": 4}), ("steps_per_refill8", {"steps_per_refill": 8}),
                 ("hom_tol0.1", {"hom_tol": 0.1})]
+    small = ("default", "scheduler0", "tally_warp", "tally_fixed")   # config 1 (1e5 histories): these only
     out = {"what": "ms per gpumcd_run (median of %d, device time), full history counts" % args.steps, "configs": {}}
-    for c in (2, 3, 4, 5):
+    for c in (1, 2, 3, 4, 5):
         w = make_config(c)
         row = {}
         for name, o in variants:
+            if c == 1 and name not in small:
+                continue
             if c == 5 and o.get("scheduler") == 0 and o.get("wave_size", 1 << 20) > (1 << 20):
                 continue                      # 4 queues x 2^22 x 4 x 48 B does not leave room for the rest
             t, cnt = time_gpu(g, torch, w, w.n_histories, args.steps, **o)
@@ -322,10 +327,10 @@ def load_traffic_table():
     return out
 
 
-# algorithmic DRAM bytes of one run: first touch of the phantom (8 B / voxel), the tally read + written back
-# (2 x 8 B / voxel) and the dose written (4 B / voxel); DESIGN.md 7 "Rooflines"
+# algorithmic DRAM bytes of one run: first touch of the packed phantom (4 B / voxel), the tally zeroed, read and
+# written back (2 x 8 B / voxel) and the dose written (4 B / voxel); DESIGN.md 7 "Rooflines"
 def algorithmic_dram_bytes(w):
-    return int(w.density.size) * (8 + 16 + 4)
+    return int(w.density.size) * (4 + 16 + 4)
 
 
 def measure(g, torch, dist, w, n, opts, steps, warmup, dev, rank, world, flush, e2e=True, probe=True):
@@ -459,7 +464,8 @@ def measure(g, torch, dist, w, n, opts, steps, warmup, dev, rank, world, flush, 
                       "ms_per_step": e2e_t * 1e3,
                       "what": "gpumcd_set_phantom_host + gpumcd_set_source + gpumcd_run_host per step, wall clock, pinned host buffers"}
     out["options"] = {"scheduler": int(opt.scheduler), "hom_tol": float(opt.hom_tol), "wave_size": int(opt.wave_size),
-                      "tally_mode": int(opt.tally_mode), "cta_threads": int(opt.cta_threads) or 512}
+                      "tally_mode": int(opt.tally_mode), "cta_threads": int(opt.cta_threads) or 512,
+                      "steps_per_refill": int(opt.steps_per_refill) or "auto (4 for an electron beam, else 1)"}
     g.gpumcd_destroy(ctx)
     return out
 
