@@ -201,13 +201,13 @@ def time_gpu(g, torch, w, n, reps, **opts):
     return float(np.median(ts)), c
 
 
-def s_gpu(g, torch, ev, w, n, nb=40):
+def s_gpu(g, torch, ev, w, n, nb=40, **opts):
     dev = torch.device("cuda:0")
     rho = torch.from_numpy(w.density).to(dev)
     mat = torch.from_numpy(w.material).to(dev)
     dose = torch.empty(rho.shape, dtype=torch.float32, device=dev)
     sig = torch.empty(rho.shape, dtype=torch.float32, device=dev)
-    with g.gpumcd_create(rho, mat, w.voxel_cm, w.tables) as ctx:
+    with g.gpumcd_create(rho, mat, w.voxel_cm, w.tables, g.gpumcd_default_options(**opts)) as ctx:
         g.gpumcd_set_source(ctx, w.source)
         g.gpumcd_run_uncertainty(ctx, n, nb, w.seed, dose, sig)
         torch.cuda.synchronize()
@@ -239,6 +239,8 @@ def paper_tables(args):
             tm, cm = time_gpu(g, torch, w, n, args.steps, hom_tol=0.1)
             s = s_gpu(g, torch, ev, w, n)
             eps = ev.efficiency(s, t1 * 1e-3)
+            s_m = s_gpu(g, torch, ev, w, n, hom_tol=0.1)      # R32: the one-point deposit adds variance per step
+            eps_m = ev.efficiency(s_m, tm * 1e-3)
             # the oracle on a bounded sample; s scales as 1/sqrt(N) (L334), time as N
             n_o = max(2000, int(n * args.oracle_fraction))
             tw = time.perf_counter()
@@ -253,7 +255,8 @@ def paper_tables(args):
             rows5.append(f"| {pname} | Geom{geom} | {t_o:.1f} | {t_o / (t1 * 1e-3):.0f} | {s * 100:.3f} | {s_o * 100:.3f} | "
                          f"{eps:.3g} | {eps_o:.3g} | {eps / eps_o:.0f} |")
             rows6.append(f"| {pname} | Geom{geom} | {t0:.3f} | {t0 / t1:.2f} | {t0 / ta:.2f} | {t0 / tb:.2f} | "
-                         f"{t0 / tm:.2f} ({tm:.3f} ms, {c['ch_steps'] / cm['ch_steps']:.2f} x fewer steps) |")
+                         f"{t0 / tm:.2f} ({tm:.3f} ms, {c['ch_steps'] / cm['ch_steps']:.2f} x fewer steps) | "
+                         f"{s_m * 100:.3f} ({s * 100:.3f}) | {eps_m / eps:.2f} |")
     print("## Tab. IV analogue: absolute times of `gpumcd_run` (device time, CUDA events, median of "
           f"{args.steps}, L2 flushed between runs)\n")
     print("| particles | geometry | histories | ms | M histories/s | G CH steps/s | paper, GTX480, ms (context) |")
@@ -267,8 +270,9 @@ def paper_tables(args):
     print("\n".join(rows5))
     print("\n## Tab. VI analogue: scheduling strategies against the paper's base scheme (scheduler 0)\n")
     print("| particles | geometry | T_base = scheduler 0, ms | A, scheduler 1 (default CTA size) | A, 512 threads/SM | "
-          "A, 1024 threads/SM | A, scheduler 1 + multi-voxel steps (hom_tol 0.1, another step algorithm: DESIGN.md R32) |")
-    print("|---|---|---|---|---|---|---|")
+          "A, 1024 threads/SM | A, scheduler 1 + multi-voxel steps (hom_tol 0.1, another step algorithm: DESIGN.md R32) | "
+          "s, % with multi-voxel steps (Eq. 4 steps) at equal N | efficiency gain of multi-voxel steps, eps_m / eps (Eq. 11) |")
+    print("|---|---|---|---|---|---|---|---|---|")
     print("\n".join(rows6))
 
 
@@ -560,14 +564,16 @@ def main():
     if not args.no_per_config and not args.histories:
         for c in (1, 2, 3, 4, 5):
             if c == args.config:
-                per_config[f"cfg{c}"] = {k: head[k] for k in ("workload", "ms_per_step", "value", "ch_steps_per_s",
-                                                               "photon_flights_per_s", "roofline", "roofline_tally", "e2e")}
+                per_config[f"cfg{c}"] = {k: head[k] for k in ("workload", "histories_per_step_per_gpu", "ms_per_step", "value",
+                                                               "ch_steps_per_s", "photon_flights_per_s", "roofline",
+                                                               "roofline_tally", "roofline_hbm", "e2e")}
                 continue
             wc = make_config(c)
             m = measure(g, torch, dist, wc, wc.n_histories, opts, args.steps, args.warmup, dev, rank, world, flush,
                         e2e=not args.no_e2e)
-            per_config[f"cfg{c}"] = {k: m[k] for k in ("workload", "ms_per_step", "value", "ch_steps_per_s",
-                                                        "photon_flights_per_s", "roofline", "roofline_tally", "e2e")}
+            per_config[f"cfg{c}"] = {k: m[k] for k in ("workload", "histories_per_step_per_gpu", "ms_per_step", "value",
+                                                        "ch_steps_per_s", "photon_flights_per_s", "roofline",
+                                                        "roofline_tally", "roofline_hbm", "e2e")}
             del wc
     clocks = sampler.stop()
 

@@ -109,3 +109,9 @@ def test_device_records_equal_host_records_and_errors():
         with pytest.raises(g.GpumcdError) as e:   # a failed set_source leaves the context without a source
             g.gpumcd_run(ctx, 10, 1, torch.empty(rho.shape, dtype=torch.float32, device="cuda:0"))
         assert e.value.status == g.GPUMCD_ERR_NO_SOURCE
+    # the 1024-thread CTA exists for the ablation of plain sources only
+    with g.gpumcd_create(rho, mat, w.voxel_cm, w.tables, g.gpumcd_default_options(cta_threads=1024)) as ctx:
+        g.gpumcd_set_source(ctx, w.source)
+        with pytest.raises(g.GpumcdError) as e:
+            g.gpumcd_run(ctx, 10, 1, torch.empty(rho.shape, dtype=torch.float32, device="cuda:0"))
+        assert e.value.status == g.GPUMCD_ERR_INVALID_ARG

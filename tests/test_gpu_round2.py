@@ -322,3 +322,20 @@ def test_thresholds_on_the_device():
     src = dataclasses.replace(w2.source, energy=0.3995)
     g = run_gpu(dataclasses.replace(w2, source=src), 300_000, majorant_scale=200.0)
     assert g["counters"]["hard_moller"] == 0 and g["counters"]["hard_fict"] > 100_000
+
+
+# ------------------------------------------------------------------ steps per refill (the paper's N)
+@pytest.mark.parametrize("cfg,n", [(2, 60_000), (5, 300_000)])
+def test_steps_per_refill_changes_the_schedule_not_the_histories(cfg, n):
+    """Several condensed-history steps between two looks at the stacks: who steps when changes, no history does."""
+    w = make_config(cfg)
+    ref = run_gpu(w, n, steps_per_refill=1)
+    for nsteps in (0, 2, 4, 8):          # 0 = automatic (4 for config 2's electron beam, 1 for config 5)
+        g = run_gpu(w, n, steps_per_refill=nsteps)
+        for k in INT_KEYS:
+            assert g["counters"][k] == ref["counters"][k], (nsteps, k)
+        assert g["counters"]["overflow_count"] == 0
+        assert np.abs(g["edep"] - ref["edep"]).max() <= 1e-12 * ref["edep"].max()
+    m = run_gpu(w, n, steps_per_refill=4, hom_tol=0.1, tally_mode=2)
+    m1 = run_gpu(w, n, steps_per_refill=1, hom_tol=0.1, tally_mode=2)
+    assert np.array_equal(m["edep"], m1["edep"])
