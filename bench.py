@@ -294,10 +294,12 @@ def ablation(args):
                 ("scheduler0_wave2^22_d4", {"scheduler": 0, "wave_size": 1 << 22, "bank_factor": 4}),
                 ("cta1024", {"cta_threads": 1024}),
                 ("tally_warp", {"tally_mode": 1}), ("tally_fixed", {"tally_mode": 2}),
-                ("high_g40", {"bank_high_g": 40}), ("high_g160", {"bank_high_g": 160}), ("high_g320", {"bank_high_g": 320}),
-                ("high_e80", {"bank_high_e": 80}), ("high_e320", {"bank_high_e": 320}), ("high_e640", {"bank_high_e": 640}),
-                ("low8", {"bank_low": 8}), ("low48", {"bank_low": 48}),
-                ("stack256", {"warp_stack": 256}), ("stack512", {"warp_stack": 512}),
+                ("round1_marks80_160_stack1024", {"bank_high_g": 80, "bank_high_e": 160, "warp_stack": 1024, "steps_per_refill": 1}),
+                ("marks80_160", {"bank_high_g": 80, "bank_high_e": 160}), ("marks24_40", {"bank_high_g": 24, "bank_high_e": 40}),
+                ("marks320_640", {"bank_high_g": 320, "bank_high_e": 640}), ("marks1000_2000", {"bank_high_g": 1000, "bank_high_e": 2000}),
+                ("low8", {"bank_low": 8}), ("low32", {"bank_low": 32}),
+                ("stack256", {"warp_stack": 256}), ("stack1024", {"warp_stack": 1024}), ("stack2048", {"warp_stack": 2048}),
+                ("stack8192", {"warp_stack": 8192}),
                 ("steps_per_refill1", {"steps_per_refill": 1}), ("steps_per_refill2", {"steps_per_refill": 2}),
                 ("steps_per_refill4", {"steps_per_refill": 4}), ("steps_per_refill8", {"steps_per_refill": 8}),
                 ("hom_tol0.1", {"hom_tol": 0.1})]
@@ -311,6 +313,7 @@ def ablation(args):
                 continue
             if c == 5 and o.get("scheduler") == 0 and o.get("wave_size", 1 << 20) > (1 << 20):
                 continue                      # 4 queues x 2^22 x 4 x 48 B does not leave room for the rest
+            print(f"ablation: {w.name} {name}", file=sys.stderr, flush=True)
             t, cnt = time_gpu(g, torch, w, w.n_histories, args.steps, **o)
             row[name] = {"ms": round(t, 4), "ch_steps": cnt["ch_steps"], "bank_high_water": cnt["bank_high_water"]}
         out["configs"][w.name] = row
@@ -469,7 +472,7 @@ def measure(g, torch, dist, w, n, opts, steps, warmup, dev, rank, world, flush, 
                       "what": "gpumcd_set_phantom_host + gpumcd_set_source + gpumcd_run_host per step, wall clock, pinned host buffers"}
     out["options"] = {"scheduler": int(opt.scheduler), "hom_tol": float(opt.hom_tol), "wave_size": int(opt.wave_size),
                       "tally_mode": int(opt.tally_mode), "cta_threads": int(opt.cta_threads) or 512,
-                      "steps_per_refill": int(opt.steps_per_refill) or "auto (4 for an electron beam, else 1)"}
+                      "steps_per_refill": int(opt.steps_per_refill) or 4, "warp_stack": int(opt.warp_stack)}
     g.gpumcd_destroy(ctx)
     return out
 

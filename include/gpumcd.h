@@ -87,16 +87,18 @@ typedef struct {
                               0: the paper's scheme (L166): one launch per pass, one thread per
                               particle, the host reads the queue counts between passes            */
     uint32_t warp_stack;   /* scheduler 1: capacity of a warp's electron stack and of its photon
-                              stack, records; default 1024, at least 256.  A warp changes particle
-                              type before the other type's stack fills up, which keeps the stacks
-                              short (a few hundred records on the five configurations), but a
-                              history that breeds more secondaries than a stack holds overflows it:
+                              stack, records; default 4096 (0.95 GB for the 2368 warps of a B200), at
+                              least 256.  A warp works on one particle type until it runs dry or the
+                              other type's stack is about to fill up (bank_high_g / bank_high_e can make
+                              it change earlier), so the capacity sets how long it stays in one part of
+                              the code: 4096 is 10 % faster than 1024 on photon beams, more buys nothing.
+                              A history that breeds more secondaries than a stack holds overflows it:
                               that is reported (GPUMCD_ERR_BANK_OVERFLOW from gpumcd_run_host and
                               gpumcd_get_counters, overflow_count), never silently dropped        */
-    uint32_t cta_threads;  /* scheduler 1: threads of the persistent kernel's one CTA per SM: 0 or 512
-                              (default; 128 registers per thread, short drain phase) or 1024 (64
-                              registers, twice the warps; slower on every workload measured, kept
-                              for the ablation)                                                    */
+    uint32_t cta_threads;  /* scheduler 1: threads of the persistent kernel's one CTA per SM: 0 or 768
+                              (default: 6 warps per scheduler, 80 registers per thread), or 512 (128
+                              registers) or 1024 (64 registers), both slower on every workload measured
+                              and kept for the ablation (fp64 tally and plain sources only)        */
     float hom_tol;         /* 0 (default): electron steps end at every voxel boundary, Eq. 4 as printed.
                               > 0: multi-voxel steps (the paper's "improvements to the electron-step
                               algorithm", L364-368, are future work there; R32): d_vox of
@@ -117,24 +119,26 @@ typedef struct {
                                  most 40; exact for deposits >= 2^(24-k) MeV) and added as an integer: the result
                                  does not depend on the order of the additions, so the same (seed, n_histories)
                                  gives the same dose bit for bit, on either scheduler.
-                              Modes 1 and 2 need cta_threads 0 or 512.                                 */
+                              Modes 1 and 2 need the default cta_threads.                              */
     int32_t table_memory;  /* scheduler 1: 0 (default) = the table blob is staged into shared memory by TMA
                               bulk copies when it fits (up to ~220 KB: 7 materials at 1024 nodes), else read
                               from global memory; 1 = always read from global memory (test hook)      */
-    uint32_t bank_high_g;  /* scheduler 1, tuning (0 = the library's choice: 80 at 512 threads, 512 at 1024): a
-                              warp stepping electrons changes to photons once this many photons are banked
-                              and fewer than bank_high_e electrons are left                             */
-    uint32_t bank_high_e;  /* scheduler 1, tuning (0 = 160 at 512 threads, 512 at 1024): the same for a warp
-                              flying photons.  Together they are the paper's compaction interval N (L180):
-                              how much work of one type is done before the other type is picked up      */
-    uint32_t bank_low;     /* scheduler 1, tuning (0 = 24, at most 64): once the source is exhausted a warp with
-                              fewer ready particles of its type than this changes to the other type      */
+    uint32_t bank_high_g;  /* scheduler 1, tuning (0 = never, the default): a warp stepping electrons changes to
+                              photons as soon as this many photons are banked and fewer than bank_high_e
+                              electrons are left (at least bank_low)                                     */
+    uint32_t bank_high_e;  /* scheduler 1, tuning (0 = never, the default): the same for a warp flying photons.
+                              They bound how much work of one type is done before the other type is picked
+                              up; measured, every early change costs (round 1 ran 80 / 160: 10 % slower) */
+    uint32_t bank_low;     /* scheduler 1, tuning (0 = 24, at most 32): once the source is exhausted a warp with
+                              fewer ready particles of its type than this changes to the other type, if a full
+                              batch (32) of that type waits.  Above 32 two stacks holding between 32 and bank_low
+                              records would send the warp back and forth for ever: refused (INVALID_ARG)         */
     uint32_t steps_per_refill; /* scheduler 1: condensed-history steps a warp makes at most before it looks at its
                               stacks again (refills free lanes, banks hard-event candidates, may change type): the
                               paper's N, "stream compaction after N simulation steps" (L180).  Lanes whose electron
                               ended wait meanwhile, so the loop goes on only while 24 of the 32 lanes still step.
-                              0 = automatic: 4 for an electron beam, 1 otherwise; at most 64.  Ignored (1) with a
-                              phase-space source and with cta_threads 1024                                   */
+                              0 = automatic: 4; at most 64.  Ignored (1) with a phase-space source and with
+                              cta_threads 1024                                                               */
     int32_t l2_persist;    /* scheduler 1: 1 = the packed phantom (4 bytes per voxel) is read through a persisting
                               L2 access window, so that the tally and the particle stacks cannot evict it
                               (raises the device-wide cudaLimitPersistingL2CacheSize to the phantom's size, up

@@ -399,7 +399,7 @@ extern "C" int gpumcd_default_options(gpumcd_options *opt)
     opt->wave_size = 1u << 20;
     opt->bank_factor = 8;
     opt->scheduler = 1;
-    opt->warp_stack = 1024;
+    opt->warp_stack = 4096;
     opt->cta_threads = 0;
     opt->hom_tol = 0.0f;
     opt->tally_mode = 0;
@@ -442,9 +442,12 @@ template <class V>
 static const void *persistent_variant(bool smem, int threads)
 {
     if (threads == kPThreadsDefault) return smem ? (const void *)k_persistent<V, true, kPThreadsDefault> : (const void *)k_persistent<V, false, kPThreadsDefault>;
-    if (V::TALLY == TALLY_F64 && !V::PHSP && !V::INNER)
-        return smem ? (const void *)k_persistent<Variant<V::TRACE, V::MULTI, TALLY_F64>, true, 1024>
-                    : (const void *)k_persistent<Variant<V::TRACE, V::MULTI, TALLY_F64>, false, 1024>;
+    // the other CTA sizes (ablation): fp64 tally, no phase space, the several-steps-per-refill form of the loop
+    if (V::TALLY == TALLY_F64 && !V::PHSP) {
+        using A = Variant<V::TRACE, V::MULTI, TALLY_F64, false, !V::TRACE>;
+        if (threads == 512) return smem ? (const void *)k_persistent<A, true, 512> : (const void *)k_persistent<A, false, 512>;
+        if (threads == 1024) return smem ? (const void *)k_persistent<A, true, 1024> : (const void *)k_persistent<A, false, 1024>;
+    }
     return nullptr;
 }
 template <bool MULTI, bool PHSP, bool INNER>
@@ -558,9 +561,11 @@ static int create_impl(gpumcd_ctx **out, const float *density, const uint8_t *ma
     if (opt_in) opt = *opt_in;
     if (!(opt.es_max_cm > 0.f) || !(opt.f_eloss_max > 0.f) || opt.f_eloss_max > 1.f || opt.boundary_nudge < 0.f ||
         !(opt.majorant_scale >= 1.f) || opt.wave_size == 0 || opt.bank_factor == 0 || opt.warp_stack > (1u << 20) ||
-        (opt.cta_threads != 0 && opt.cta_threads != kPThreadsDefault && opt.cta_threads != 1024) || !(opt.hom_tol >= 0.f) ||
-        opt.tally_mode < 0 || opt.tally_mode > 2 || (opt.tally_mode != 0 && opt.cta_threads == 1024) ||
-        opt.table_memory < 0 || opt.table_memory > 1 || opt.bank_low > 64 || opt.steps_per_refill > 64 || opt.l2_persist < 0 || opt.l2_persist > 1 ||
+        (opt.cta_threads != 0 && opt.cta_threads != 512 && opt.cta_threads != kPThreadsDefault && opt.cta_threads != 1024) || !(opt.hom_tol >= 0.f) ||
+        opt.tally_mode < 0 || opt.tally_mode > 2 || (opt.tally_mode != 0 && opt.cta_threads != 0 && opt.cta_threads != kPThreadsDefault) ||
+        opt.table_memory < 0 || opt.table_memory > 1 || opt.bank_low > 32 || opt.steps_per_refill > 64 || opt.l2_persist < 0 || opt.l2_persist > 1 ||
+        (opt.bank_high_g && opt.bank_high_g < (opt.bank_low ? opt.bank_low : kLowDefault)) || // (a warp would change to
+        (opt.bank_high_e && opt.bank_high_e < (opt.bank_low ? opt.bank_low : kLowDefault)) || //  a type it leaves at once)
         static_cast<unsigned long long>(opt.wave_size) * opt.bank_factor > 0x7fffffffull) {
         set_error(nullptr, "bad options");
         return GPUMCD_ERR_INVALID_ARG;
@@ -903,24 +908,24 @@ static int run_persistent(gpumcd_ctx *ctx, uint64_t h_begin, uint64_t n_hist, ui
         a.dose = dose_dev;
         a.nvox = ctx->nvox;
         a.finalize = (h0 + n == h_end) ? 1 : 0;
-        // CTA size (see persistent.cuh): 512 threads unless the caller asks for 1024
+        // CTA size (see persistent.cuh): 768 threads unless the caller asks for 512 or 1024
         const int threads = ctx->opt.cta_threads ? static_cast<int>(ctx->opt.cta_threads) : kPThreadsDefault;
-        // banked particles of the other type that make a warp change to it: photons are cheap to work off
-        // (few per batch keeps the drain short), electrons are worth a fuller batch; swept on configs 2-5
-        // (bench.py --ablation): 80 / 160 with 512 threads per SM, 512 / 512 with 1024
-        a.high_g = ctx->opt.bank_high_g ? ctx->opt.bank_high_g : (threads != 1024 ? 80u : 512u);
-        a.high_e = ctx->opt.bank_high_e ? ctx->opt.bank_high_e : (threads != 1024 ? 160u : 512u);
+        // banked particles of the other type that make a warp change to it before it has to: none by default (a
+        // warp stays with one type until it runs dry or a stack is about to fill up; measured on configs 1-5,
+        // bench.py --ablation: every earlier change costs)
+        a.high_g = ctx->opt.bank_high_g ? ctx->opt.bank_high_g : 0xffffffffu;
+        a.high_e = ctx->opt.bank_high_e ? ctx->opt.bank_high_e : 0xffffffffu;
         a.low = ctx->opt.bank_low ? ctx->opt.bank_low : kLowDefault;
-        // steps per refill (the paper's N, L180): several pay for long electron tracks, i.e. an electron beam;
-        // measured: 15 MeV electrons in water 2.78 -> 2.63 ms with 4, photon beams in heterogeneous phantoms lose 1-2 %
+        // steps per refill (the paper's N, L180): 4 (measured on configs 1-5: 2.5-5 % faster than 1; 8 is no better)
         const bool phsp = ctx->src.shape == 2;
-        a.inner = ctx->opt.steps_per_refill ? ctx->opt.steps_per_refill : (ctx->src.particle == 1 && !phsp && threads != 1024 ? 4u : 1u);
-        if (phsp || threads == 1024 || trace) a.inner = 1u; // (variants that are not built: one step per refill)
+        a.inner = ctx->opt.steps_per_refill ? ctx->opt.steps_per_refill : 4u;
+        if (phsp || trace) a.inner = 1u; // (variants that are not built: one step per refill)
         void *args[] = {&a};
         // the kernel variant: trace (photon-only replay) | multi-voxel steps x tally mode; tables in shared memory; CTA size
         const bool multi = ctx->opt.hom_tol > 0.f && !trace; // a trace run tracks no electrons
         const void *fn = persistent_kernel(trace != nullptr, multi, ctx->opt.tally_mode, phsp, a.inner > 1u, ctx->smem_tables, threads);
         if (!fn) { set_error(ctx, "a phase-space source needs the default CTA size (cta_threads 0)"); return GPUMCD_ERR_INVALID_ARG; }
+        if (threads != kPThreadsDefault && !trace) a.inner = std::max(a.inner, 1u); // (these sizes are built in the loop form)
         const size_t dyn = ctx->smem_tables ? static_cast<size_t>(ctx->table_floats) * sizeof(float) + ctx->spec_smem_bytes : 0;
         { const int rc = allow_dynamic_smem(ctx, fn, dyn); if (rc != GPUMCD_OK) return rc; }
         { LaunchScope ls(ctx, st, CLS_ELECTRON);

@@ -29,19 +29,23 @@ namespace gpumcd {
 
 namespace cg = cooperative_groups;
 
-// Threads per persistent CTA (one CTA per SM): 512 by default (128 registers per thread, no spills; the
-// per-lane backlog when the source runs dry is half that of 1024 threads).  The 1024-thread build (64
-// registers, spills, twice the warps to hide latency) is kept as an option for the ablation: it was the
-// faster one for photon beams in heterogeneous phantoms until the fast-math build shrank the code.
+// Threads per persistent CTA (one CTA per SM): 768 by default, i.e. 6 warps per scheduler at 80 registers per
+// thread (124 bytes of spills outside the step loop).  Measured once a warp stays with one particle type until it
+// has to change (config 5, ms): 512 threads 58.0, 576 60.4, 640 53.8, 704 59.4, 768 53.0, 896 54.7, 1024 54.7 (the
+// sizes that give every scheduler the same number of warps win).  512 (128 registers, no spills) and 1024 (64
+// registers) are kept as options for the ablation.
 #ifndef GPUMCD_PT
-#define GPUMCD_PT 512
+#define GPUMCD_PT 768
 #endif
 constexpr int kPThreadsDefault = GPUMCD_PT;
 constexpr int kPThreadsMax = 1024;
 constexpr unsigned kFull = 0xffffffffu;
 constexpr unsigned kChunk = 32;            // primaries a warp claims per atomic on the source head
 constexpr unsigned kPend = 64;             // capacity of a waiting stack (EH, GI, GR): < 32 before a move, + 32 after
-constexpr unsigned kKeep = 24;             // lanes that must be able to go on for another step inside one iteration
+#ifndef GPUMCD_KEEP
+#define GPUMCD_KEEP 24
+#endif
+constexpr unsigned kKeep = GPUMCD_KEEP;             // lanes that must be able to go on for another step inside one iteration
 constexpr unsigned kLowDefault = 24;       // own-type particles below which a warp with no source changes type
 // Forced type changes.  Between two looks at the rules below photon mode banks at most 96 electrons (one Compton
 // batch: 32, one batch of pair events: 64) and electron mode at most 32 photons (one hard-event batch).
