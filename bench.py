@@ -299,7 +299,8 @@ def ablation(args):
                 ("marks320_640", {"bank_high_g": 320, "bank_high_e": 640}), ("marks1000_2000", {"bank_high_g": 1000, "bank_high_e": 2000}),
                 ("low8", {"bank_low": 8}), ("low32", {"bank_low": 32}),
                 ("stack256", {"warp_stack": 256}), ("stack1024", {"warp_stack": 1024}), ("stack2048", {"warp_stack": 2048}),
-                ("stack8192", {"warp_stack": 8192}),
+                ("stack4096", {"warp_stack": 4096}), ("stack16384", {"warp_stack": 16384}),
+                ("cta512", {"cta_threads": 512}),
                 ("steps_per_refill1", {"steps_per_refill": 1}), ("steps_per_refill2", {"steps_per_refill": 2}),
                 ("steps_per_refill4", {"steps_per_refill": 4}), ("steps_per_refill8", {"steps_per_refill": 8}),
                 ("hom_tol0.1", {"hom_tol": 0.1})]

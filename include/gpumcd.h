@@ -87,11 +87,11 @@ typedef struct {
                               0: the paper's scheme (L166): one launch per pass, one thread per
                               particle, the host reads the queue counts between passes            */
     uint32_t warp_stack;   /* scheduler 1: capacity of a warp's electron stack and of its photon
-                              stack, records; default 4096 (0.95 GB for the 2368 warps of a B200), at
+                              stack, records; default 8192 (2.8 GB for the 3552 warps of a B200), at
                               least 256.  A warp works on one particle type until it runs dry or the
                               other type's stack is about to fill up (bank_high_g / bank_high_e can make
                               it change earlier), so the capacity sets how long it stays in one part of
-                              the code: 4096 is 10 % faster than 1024 on photon beams, more buys nothing.
+                              the code: on photon beams 4096 is 10 % faster than 1024 and 8192 another 2-4 %.
                               A history that breeds more secondaries than a stack holds overflows it:
                               that is reported (GPUMCD_ERR_BANK_OVERFLOW from gpumcd_run_host and
                               gpumcd_get_counters, overflow_count), never silently dropped        */

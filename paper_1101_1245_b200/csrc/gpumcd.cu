@@ -399,7 +399,7 @@ extern "C" int gpumcd_default_options(gpumcd_options *opt)
     opt->wave_size = 1u << 20;
     opt->bank_factor = 8;
     opt->scheduler = 1;
-    opt->warp_stack = 4096;
+    opt->warp_stack = 8192;
     opt->cta_threads = 0;
     opt->hom_tol = 0.0f;
     opt->tally_mode = 0;

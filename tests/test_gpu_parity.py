@@ -151,8 +151,8 @@ def test_schedulers_agree_exactly(workloads):
 
 
 def test_cta_size_does_not_change_the_result(workloads):
-    """Scheduler 1 runs with 512 (default) or 1024 threads per SM: which lane works a particle off does not
-    matter."""
+    """Scheduler 1 runs with 768 (default), 512 or 1024 threads per SM: which lane works a particle off does
+    not matter."""
     for cfg in (2, 4):
         w = workloads[cfg]
         a = run_gpu(w, 60_000, scheduler=1, cta_threads=512)
@@ -161,6 +161,7 @@ def test_cta_size_does_not_change_the_result(workloads):
         for k in INT_KEYS:
             assert a["counters"][k] == b["counters"][k] == c["counters"][k], k
         assert np.abs(a["edep"] - b["edep"]).max() <= 1e-12 * a["edep"].max()
+        assert np.abs(a["edep"] - c["edep"]).max() <= 1e-12 * a["edep"].max()
 
 
 @pytest.mark.parametrize("scheduler", SCHEDULERS)
