@@ -129,7 +129,7 @@ typedef struct {
     uint32_t bank_high_e;  /* scheduler 1, tuning (0 = never, the default): the same for a warp flying photons.
                               They bound how much work of one type is done before the other type is picked
                               up; measured, every early change costs (round 1 ran 80 / 160: 10 % slower) */
-    uint32_t bank_low;     /* scheduler 1, tuning (0 = 24, at most 32): once the source is exhausted a warp with
+    uint32_t bank_low;     /* scheduler 1, tuning (0 = 8, at most 32): once the source is exhausted a warp with
                               fewer ready particles of its type than this changes to the other type, if a full
                               batch (32) of that type waits.  Above 32 two stacks holding between 32 and bank_low
                               records would send the warp back and forth for ever: refused (INVALID_ARG)         */

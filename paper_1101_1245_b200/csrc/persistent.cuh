@@ -46,7 +46,7 @@ constexpr unsigned kPend = 64;             // capacity of a waiting stack (EH, G
 #define GPUMCD_KEEP 24
 #endif
 constexpr unsigned kKeep = GPUMCD_KEEP;             // lanes that must be able to go on for another step inside one iteration
-constexpr unsigned kLowDefault = 24;       // own-type particles below which a warp with no source changes type
+constexpr unsigned kLowDefault = 8;        // own-type particles below which a warp with no source changes type
 // Forced type changes.  Between two looks at the rules below photon mode banks at most 96 electrons (one Compton
 // batch: 32, one batch of pair events: 64) and electron mode at most 32 photons (one hard-event batch).
 //   photon mode leaves once ES holds cap - kRoomE or more (its interactions could overflow it otherwise);
