@@ -297,7 +297,7 @@ def ablation(args):
                 ("round1_marks80_160_stack1024", {"bank_high_g": 80, "bank_high_e": 160, "warp_stack": 1024, "steps_per_refill": 1}),
                 ("marks80_160", {"bank_high_g": 80, "bank_high_e": 160}), ("marks24_40", {"bank_high_g": 24, "bank_high_e": 40}),
                 ("marks320_640", {"bank_high_g": 320, "bank_high_e": 640}), ("marks1000_2000", {"bank_high_g": 1000, "bank_high_e": 2000}),
-                ("low8", {"bank_low": 8}), ("low32", {"bank_low": 32}),
+                ("low24", {"bank_low": 24}), ("low32", {"bank_low": 32}),
                 ("stack256", {"warp_stack": 256}), ("stack1024", {"warp_stack": 1024}), ("stack2048", {"warp_stack": 2048}),
                 ("stack4096", {"warp_stack": 4096}), ("stack16384", {"warp_stack": 16384}),
                 ("cta512", {"cta_threads": 512}),

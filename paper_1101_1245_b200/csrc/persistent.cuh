@@ -14,8 +14,9 @@
 //     out to the waiting stack and takes the next ready record (stack first, then a primary), so the
 //     long step code and the rejection samplers both run with full warps ("grouping particles",
 //     L352; compaction by ballot + popc prefix sums);
-//   * secondaries of the other type pile up in that type's stack; the warp changes type when that
-//     stack passes a high-water mark or its own type runs dry, parking the particles in flight;
+//   * secondaries of the other type pile up in that type's stack; the warp changes type when its own
+//     type runs dry or that stack is about to fill up (or, optionally, passes a high-water mark),
+//     parking the particles in flight: the longer it stays with one type, the better;
 //   * tables are staged into shared memory once with TMA bulk copies (cp.async.bulk + mbarrier).
 // A particle's random stream depends only on its lineage (physics.cuh), so the order in which a
 // warp works through its stacks does not change any history.
@@ -34,18 +35,12 @@ namespace cg = cooperative_groups;
 // has to change (config 5, ms): 512 threads 58.0, 576 60.4, 640 53.8, 704 59.4, 768 53.0, 896 54.7, 1024 54.7 (the
 // sizes that give every scheduler the same number of warps win).  512 (128 registers, no spills) and 1024 (64
 // registers) are kept as options for the ablation.
-#ifndef GPUMCD_PT
-#define GPUMCD_PT 768
-#endif
-constexpr int kPThreadsDefault = GPUMCD_PT;
+constexpr int kPThreadsDefault = 768;
 constexpr int kPThreadsMax = 1024;
 constexpr unsigned kFull = 0xffffffffu;
 constexpr unsigned kChunk = 32;            // primaries a warp claims per atomic on the source head
 constexpr unsigned kPend = 64;             // capacity of a waiting stack (EH, GI, GR): < 32 before a move, + 32 after
-#ifndef GPUMCD_KEEP
-#define GPUMCD_KEEP 24
-#endif
-constexpr unsigned kKeep = GPUMCD_KEEP;             // lanes that must be able to go on for another step inside one iteration
+constexpr unsigned kKeep = 24;             // lanes that must be able to go on for another step inside one iteration
 constexpr unsigned kLowDefault = 8;        // own-type particles below which a warp with no source changes type
 // Forced type changes.  Between two looks at the rules below photon mode banks at most 96 electrons (one Compton
 // batch: 32, one batch of pair events: 64) and electron mode at most 32 photons (one hard-event batch).
