@@ -46,7 +46,9 @@ __device__ __noinline__ uint4 philox4x32_10_call(uint32_t c0, uint32_t c1, uint3
 // U(w) = ((w >> 9) + 1/2) 2^-23 in (0,1); exact in fp32 (Eq. 1 needs zeta in (0,1], L53).
 __device__ __forceinline__ float u01(uint32_t w)
 {
-    return fmaf(__uint2float_rz(w >> 9), 1.0f / 8388608.0f, 1.0f / 16777216.0f);
+    // as 1.m - (1 - 2^-24) = m 2^-23 + 2^-24: exact (an odd multiple of 2^-24 below 1), and without the integer-to-
+    // float conversion, which shares the quarter-rate XU pipe with the transcendentals (1-2 % of the run time)
+    return __uint_as_float(0x3f800000u | (w >> 9)) - 0.99999994f;
 }
 
 // ---------------------------------------------------------------------------------------------
