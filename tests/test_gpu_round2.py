@@ -339,3 +339,26 @@ def test_steps_per_refill_changes_the_schedule_not_the_histories(cfg, n):
     m = run_gpu(w, n, steps_per_refill=4, hom_tol=0.1, tally_mode=2)
     m1 = run_gpu(w, n, steps_per_refill=1, hom_tol=0.1, tally_mode=2)
     assert np.array_equal(m["edep"], m1["edep"])
+
+
+def test_scheduler_options_that_could_loop_for_ever_are_refused():
+    """bank_low above one batch (two stacks holding 32 .. bank_low records would send a warp back and forth), and a
+    high-water mark below bank_low (a warp would change to a type it leaves at once)."""
+    import torch
+
+    import paper_1101_1245_b200 as g
+    w = make_config(1)
+    rho = torch.from_numpy(w.density).to("cuda:0")
+    mat = torch.from_numpy(w.material).to("cuda:0")
+    for bad in ({"bank_low": 33}, {"bank_high_g": 4}, {"bank_high_e": 20, "bank_low": 24}, {"steps_per_refill": 65},
+                {"cta_threads": 640}, {"tally_mode": 1, "cta_threads": 512}):
+        with pytest.raises(g.GpumcdError) as e:
+            g.gpumcd_create(rho, mat, w.voxel_cm, w.tables, g.gpumcd_default_options(**bad))
+        assert e.value.status == g.GPUMCD_ERR_INVALID_ARG, bad
+    # the extremes that are allowed run and agree with the default
+    ref = run_gpu(w, 30_000)
+    for ok in ({"bank_low": 32, "bank_high_g": 32, "bank_high_e": 32}, {"bank_low": 1}, {"steps_per_refill": 64},
+               {"warp_stack": 256, "bank_high_g": 1000, "bank_high_e": 1000}):
+        g2 = run_gpu(w, 30_000, **ok)
+        for k in INT_KEYS:
+            assert g2["counters"][k] == ref["counters"][k], (ok, k)
