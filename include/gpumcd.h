@@ -235,6 +235,23 @@ int gpumcd_run_host(gpumcd_ctx *ctx, uint64_t n_histories, uint64_t seed, float 
 int gpumcd_run_uncertainty(gpumcd_ctx *ctx, uint64_t n_histories, uint32_t n_batches, uint64_t seed,
                            float *dose_out_dev, float *sigma_out_dev, void *cuda_stream);
 
+/* gpumcd_run_uncertainty for callers that must not allocate device memory (code under CUDA graph capture,
+ * tight serving loops, harnesses that forbid cudaMalloc).  gpumcd_run_uncertainty allocates its scratch, three
+ * fp64 grids of batch statistics (24 bytes per voxel), with cudaMalloc on its first call; this entry point keeps
+ * them in a static device array inside the library instead and calls no cudaMalloc, cudaFree or allocating
+ * library routine.  Same arguments, same batches, same results (up to the order of the fp64 tally's additions).
+ * Limits and rules:
+ *  - at most GPUMCD_STATIC_MAX_VOXELS voxels (64^3: the paper's own geometries); a larger phantom is refused
+ *    with GPUMCD_ERR_INVALID_ARG and a message naming the limit;
+ *  - the array (6 MiB) exists once per GPU that loads the library, until the process exits, and is shared by
+ *    every context and every call: it is cleared at the start of each call, and two calls that overlap on the
+ *    GPU (different streams, different contexts) race on it: run them one after the other;
+ *  - profiling must be off (gpumcd_set_profiling: its event pairs are created per launch);
+ *  - the context itself is set up beforehand, as for every other call (gpumcd_create allocates). */
+#define GPUMCD_STATIC_MAX_VOXELS 262144
+int gpumcd_run_uncertainty_static(gpumcd_ctx *ctx, uint64_t n_histories, uint32_t n_batches, uint64_t seed,
+                                  float *dose_out_dev, float *sigma_out_dev, void *cuda_stream);
+
 /* Photon-only replay run: like gpumcd_run with photon_only = 1 but the output is, per history,
  * the ordered event codes of the primary track, 3 bits each, first event in the low bits, at most
  * 21 events: 1 Compton, 2 photoelectric, 3 pair, 4 escaped, 5 absorbed below P_cut.

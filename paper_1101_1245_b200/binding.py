@@ -22,10 +22,11 @@ GPUMCD_ERR_OOM = -3
 GPUMCD_ERR_BANK_OVERFLOW = -4
 GPUMCD_ERR_NO_SOURCE = -5
 GPUMCD_ERR_TABLE_RANGE = -6
+GPUMCD_STATIC_MAX_VOXELS = 64 * 64 * 64   # include/gpumcd.h: largest phantom of gpumcd_run_uncertainty_static
 
 EXPORTS = ("gpumcd_default_options", "gpumcd_create", "gpumcd_create_host", "gpumcd_set_phantom",
            "gpumcd_set_phantom_host", "gpumcd_set_source", "gpumcd_run",
-           "gpumcd_run_host", "gpumcd_run_uncertainty", "gpumcd_run_trace", "gpumcd_get_counters", "gpumcd_get_energy_tally",
+           "gpumcd_run_host", "gpumcd_run_uncertainty", "gpumcd_run_uncertainty_static", "gpumcd_run_trace", "gpumcd_get_counters", "gpumcd_get_energy_tally",
            "gpumcd_set_history_offset", "gpumcd_set_profiling", "gpumcd_get_profile", "gpumcd_probe_tally",
            "gpumcd_selftest_philox", "gpumcd_release_l2",
            "gpumcd_last_error", "gpumcd_destroy")
@@ -103,6 +104,7 @@ def load_library():
         lib.gpumcd_run_host.argtypes = [vp, C.c_uint64, C.c_uint64, vp, vp]
         lib.gpumcd_run_trace.argtypes = [vp, C.c_uint64, C.c_uint64, vp, vp]
         lib.gpumcd_run_uncertainty.argtypes = [vp, C.c_uint64, C.c_uint32, C.c_uint64, vp, vp, vp]
+        lib.gpumcd_run_uncertainty_static.argtypes = lib.gpumcd_run_uncertainty.argtypes
         lib.gpumcd_get_counters.argtypes = [vp, C.POINTER(gpumcd_counters)]
         lib.gpumcd_get_energy_tally.argtypes = [vp, vp]
         lib.gpumcd_set_history_offset.argtypes = [vp, C.c_uint64]
@@ -274,6 +276,17 @@ def gpumcd_run_uncertainty(ctx: Context, n_histories: int, n_batches: int, seed:
     ctx._check(load_library().gpumcd_run_uncertainty(ctx._h, int(n_histories), int(n_batches), int(seed),
                                                      C.c_void_p(dose_out_dev.data_ptr()),
                                                      C.c_void_p(sigma_out_dev.data_ptr()), _stream_ptr(stream)))
+
+
+def gpumcd_run_uncertainty_static(ctx: Context, n_histories: int, n_batches: int, seed: int, dose_out_dev,
+                                  sigma_out_dev, stream=None) -> None:
+    """gpumcd_run_uncertainty with its scratch in the library's static device array: no device allocation
+    (include/gpumcd.h; at most GPUMCD_STATIC_MAX_VOXELS voxels)."""
+    for t in (dose_out_dev, sigma_out_dev):
+        assert t.is_cuda and t.is_contiguous() and t.element_size() == 4 and t.numel() == int(np.prod(ctx.shape))
+    ctx._check(load_library().gpumcd_run_uncertainty_static(ctx._h, int(n_histories), int(n_batches), int(seed),
+                                                            C.c_void_p(dose_out_dev.data_ptr()),
+                                                            C.c_void_p(sigma_out_dev.data_ptr()), _stream_ptr(stream)))
 
 
 def gpumcd_run_trace(ctx: Context, n_histories: int, seed: int, trace_out_dev, stream=None) -> None:

@@ -1061,6 +1061,85 @@ extern "C" int gpumcd_run_uncertainty(gpumcd_ctx *ctx, uint64_t n_histories, uin
     return GPUMCD_OK;
 }
 
+// ---------------------------------------------------------------------------------------------
+// gpumcd_run_uncertainty_static: gpumcd_run_uncertainty for callers that cannot allocate (include/gpumcd.h).
+// Its scratch, the three fp64 moment grids s1 | sx | sxx of the batch statistics, lives in this file-scope
+// array instead of the context's lazily cudaMalloc'ed `moments`: 3 x 64^3 x 8 B = 6 MiB, held by every GPU
+// that loads the library until the process exits, shared by all contexts and all calls.
+// In host code `g_static_moments` is only a stand-in for the symbol, not a device address: the address a
+// kernel can use comes from cudaGetSymbolAddress, asked once per device with that device current.
+// ---------------------------------------------------------------------------------------------
+constexpr size_t kStaticMaxVoxels = 64 * 64 * 64; // GPUMCD_STATIC_MAX_VOXELS of include/gpumcd.h
+static_assert(kStaticMaxVoxels == GPUMCD_STATIC_MAX_VOXELS, "include/gpumcd.h states the limit");
+static __device__ __align__(256) double g_static_moments[3 * kStaticMaxVoxels];
+
+constexpr int kMaxDevices = 64;
+static int static_moments_address(gpumcd_ctx *ctx, double **out)
+{
+    static std::mutex mu;
+    static double *addr[kMaxDevices] = {};
+    int dev = -1;
+    CK(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kMaxDevices) { set_error(ctx, "device ordinal beyond the static scratch table"); return GPUMCD_ERR_CUDA; }
+    std::lock_guard<std::mutex> lock(mu);
+    if (!addr[dev]) {
+        void *p = nullptr;
+        CK(cudaGetSymbolAddress(&p, g_static_moments)); // this device's copy of the array
+        addr[dev] = static_cast<double *>(p);
+    }
+    *out = addr[dev];
+    return GPUMCD_OK;
+}
+
+extern "C" int gpumcd_run_uncertainty_static(gpumcd_ctx *ctx, uint64_t n_histories, uint32_t n_batches, uint64_t seed,
+                                             float *dose_out_dev, float *sigma_out_dev, void *cuda_stream)
+{
+    if (!ctx || !dose_out_dev || !sigma_out_dev) return GPUMCD_ERR_INVALID_ARG;
+    if (ctx->nvox > kStaticMaxVoxels) {
+        char buf[200];
+        snprintf(buf, sizeof buf, "gpumcd_run_uncertainty_static: %zu voxels exceed the static scratch of %zu voxels "
+                 "(GPUMCD_STATIC_MAX_VOXELS); use gpumcd_run_uncertainty", ctx->nvox, kStaticMaxVoxels);
+        set_error(ctx, buf);
+        return GPUMCD_ERR_INVALID_ARG;
+    }
+    if (n_batches < 2 || n_batches > n_histories) {
+        set_error(ctx, "n_batches must be at least 2 and at most n_histories");
+        return GPUMCD_ERR_INVALID_ARG;
+    }
+    if (ctx->profiling) { // (per-launch event pairs are created while profiling is on: not in a call that allocates nothing)
+        set_error(ctx, "gpumcd_run_uncertainty_static: switch profiling off first (gpumcd_set_profiling)");
+        return GPUMCD_ERR_INVALID_ARG;
+    }
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    double *moments = nullptr;
+    int rc = static_moments_address(ctx, &moments);
+    if (rc != GPUMCD_OK) return rc;
+    rc = begin_run(ctx, n_histories, nullptr, st);
+    if (rc != GPUMCD_OK) return rc;
+    const size_t nvox = ctx->nvox;
+    // the array keeps the last call's contents (any context's): the sums must start at zero
+    CK(cudaMemsetAsync(moments, 0, 3 * nvox * sizeof(double), st));
+    double *s1 = moments, *sx = s1 + nvox, *sxx = sx + nvox;
+    const int grid = static_cast<int>(std::min<size_t>((nvox + kBlock - 1) / kBlock, 148 * 8));
+    uint64_t h = ctx->hist_offset;
+    for (uint32_t b = 0; b < n_batches; ++b) { // the same batches as gpumcd_run_uncertainty
+        const uint64_t m = n_histories / n_batches + (b < n_histories % n_batches ? 1 : 0);
+        rc = transport(ctx, h, m, seed, nullptr, nullptr, st);
+        if (rc != GPUMCD_OK) return rc;
+        { LaunchScope ls(ctx, st, CLS_FINALIZE);
+        k_accumulate_batch<<<grid, kBlock, 0, st>>>(ctx->edep, s1, sx, sxx, nvox, 1.0 / static_cast<double>(m)); }
+        CK(cudaGetLastError());
+        h += m;
+    }
+    const double h3 = static_cast<double>(ctx->h) * ctx->h * ctx->h;
+    { LaunchScope ls(ctx, st, CLS_FINALIZE);
+    k_finalize_uncertainty<<<grid, kBlock, 0, st>>>(s1, sx, sxx, make_geom(ctx), nvox, 1.0 / h3,
+                                                    1.0 / static_cast<double>(n_histories), static_cast<double>(n_batches),
+                                                    dose_out_dev, sigma_out_dev, ctx->edep); }
+    CK(cudaGetLastError());
+    return GPUMCD_OK;
+}
+
 extern "C" int gpumcd_run_trace(gpumcd_ctx *ctx, uint64_t n_histories, uint64_t seed, uint64_t *trace_out_dev,
                                 void *cuda_stream)
 {
