@@ -1226,14 +1226,16 @@ extern "C" int gpumcd_probe_tally(gpumcd_ctx *ctx, uint64_t n_updates, double *u
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     // the field's footprint on the grid (a pencil beam: a 3 x 3 voxel column)
     const double h = ctx->h;
+    double cx = ctx->src.cx, cy = ctx->src.cy, wx = ctx->src.wx, wy = ctx->src.wy;
     if (ctx->src.shape == 2) { // a phase space: its footprint is not known, take the whole face
-        ctx->src.cx = 0.5 * ctx->nx * h; ctx->src.cy = 0.5 * ctx->ny * h;
-        ctx->src.wx = (ctx->nx - 1) * h; ctx->src.wy = (ctx->ny - 1) * h;
+        cx = 0.5 * ctx->nx * h; cy = 0.5 * ctx->ny * h;
+        wx = (ctx->nx - 1) * h; wy = (ctx->ny - 1) * h;
     }
-    int x0 = static_cast<int>(std::floor((ctx->src.cx - 0.5 * ctx->src.wx) / h)) - (ctx->src.shape == 0 ? 1 : 0);
-    int y0 = static_cast<int>(std::floor((ctx->src.cy - 0.5 * ctx->src.wy) / h)) - (ctx->src.shape == 0 ? 1 : 0);
-    int x1 = static_cast<int>(std::floor((ctx->src.cx + 0.5 * ctx->src.wx) / h)) + (ctx->src.shape == 0 ? 1 : 0);
-    int y1 = static_cast<int>(std::floor((ctx->src.cy + 0.5 * ctx->src.wy) / h)) + (ctx->src.shape == 0 ? 1 : 0);
+    const int margin = ctx->src.shape == 0 ? 1 : 0;
+    int x0 = static_cast<int>(std::floor((cx - 0.5 * wx) / h)) - margin;
+    int y0 = static_cast<int>(std::floor((cy - 0.5 * wy) / h)) - margin;
+    int x1 = static_cast<int>(std::floor((cx + 0.5 * wx) / h)) + margin;
+    int y1 = static_cast<int>(std::floor((cy + 0.5 * wy) / h)) + margin;
     x0 = std::max(x0, 0); y0 = std::max(y0, 0);
     x1 = std::min(x1, ctx->nx - 1); y1 = std::min(y1, ctx->ny - 1);
     const int threads = 512, blocks = 148 * 2;
