@@ -166,8 +166,12 @@ def test_two_contexts_with_history_offsets_sum_to_one_run(scheduler):
     np.testing.assert_allclose(dose, whole["dose"], rtol=2e-6, atol=1e-12 * whole["dose"].max())
     # the offset run is the oracle's run over the same ids
     o = oracle.run_workload(w, spans[1][1], hist_begin=spans[1][0])
+    # (the ~0.5 % of the histories that an fp32 flip takes off the oracle's path are independent samples, DESIGN.md
+    # 4.5: a rare-event counter such as hard_fict, ~1000 here and clustered in few histories, then differs by a few
+    # times sqrt(0.01 c), which the relative bar alone does not allow for at this size)
     for k in INT_KEYS:
-        assert abs(parts[1][1][k] - o.counters[k]) <= 10 + 3e-3 * o.counters[k], k
+        c = o.counters[k]
+        assert abs(parts[1][1][k] - c) <= 10 + 3e-3 * c + np.sqrt(c), k
     assert parts[1][0].sum() == pytest.approx(o.edep.sum(), rel=2e-3)
 
 
