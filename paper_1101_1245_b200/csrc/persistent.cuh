@@ -249,7 +249,8 @@ struct Warp {
     __device__ __forceinline__ unsigned cap(int s) const { return s < 2 ? cap_r : kPend; }
     __device__ __forceinline__ void count(int k, unsigned mask) const
     {
-        if ((threadIdx.x & 31) == 0 && mask) ctl->wc[k] += static_cast<unsigned>(__popc(mask));
+        // (a shared-memory atomic by lane 0: one instruction instead of load, add, store; 0.5-1 % of the run)
+        if ((threadIdx.x & 31) == 0 && mask) atomicAdd(&ctl->wc[k], static_cast<unsigned>(__popc(mask)));
     }
     // Converged code: the lanes with `on` append their record to stack s (ballot + popc prefix).
     __device__ __forceinline__ unsigned push(const Params &P, int s, bool on, const Particle &c, uint32_t extra)
